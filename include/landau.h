@@ -1,0 +1,153 @@
+/*
+ * landau.h -- C ABI of liblandau.so: the B200 (sm_100a) hot path of the multispecies
+ * structure-preserving particle discretisation of the Landau collision operator
+ * (Zonta, Pusztay, Hirvijoki, arXiv:2212.00663; citations are PAPER.md:<line>).
+ *
+ * What the library computes (3-V restatement, DESIGN.md "Readings" D1, D2, S1-S10, U1-U3):
+ *
+ *   pass 1  G_p = (1/w_p) dS_eps/dv_p, the gradient of the Gaussian-regularised entropy by tensor
+ *           Gauss-Hermite quadrature                       Eq. (22); Eqs. 19-21
+ *   pass 2  V_p = (1/m_s) sum_s' nu_ss' sum_{p' in s'} w_p' Q(v_p - v_p') (G_p/m_s - G_p'/m_s'),
+ *           Q(z) = (|z|^2 I - z z^T)/|z|^3                 Eq. (23); Eqs. 4, 16, 17
+ *   step    v^{n+1} = v^n + dt V[(v^n + v^{n+1})/2 ; G^n]  by Jacobi fixed-point iteration
+ *                                                          Eqs. (24)-(25); Alg. 1
+ *   moments n_s, P_s, K_s, S_eps,s                         Eqs. 26, 28, 33, 20
+ *
+ * Conventions
+ *   - Every marker array argument is a DEVICE pointer (cudaMalloc'ed / torch CUDA tensor
+ *     data_ptr) unless the function name ends in _host, in which case it is a HOST pointer and the
+ *     library does the host<->device copies itself (on the context's stream, then synchronises).
+ *   - v is [N x 3] row-major FP64, w is [N] FP64 (> 0), species_id is [N] int32 in 0..S-1 in any
+ *     order.  Outputs are [N x 3] in the CALLER's marker order whatever the internal bucketing.
+ *   - Small per-species outputs (moments) and landau_step_info are HOST memory.
+ *   - Ownership: the caller owns every array it passes and may free or reuse it once the call
+ *     returns (device arrays: once the context's stream has passed the call).  The library copies
+ *     what it needs into its own SoA scratch and keeps no caller pointer.  The context owns its
+ *     scratch (grown lazily, released by landau_destroy).
+ *   - Streams: one context = one CUDA stream (opts->stream, NULL = the legacy default stream).
+ *     Device-pointer calls are asynchronous on that stream except for the final status read-back;
+ *     landau_step synchronises once at its end to fill landau_step_info.
+ *   - Errors: every call returns an int.  0 = LANDAU_OK; 1 = LANDAU_NOT_CONVERGED (the step is
+ *     still committed, as in the paper); negative = hard error, outputs are
+ *     unspecified: -1 invalid argument (NULL, N < 1, species_id out of range, w <= 0, m <= 0,
+ *     eps <= 0, non-symmetric nu, n_q out of range), -2 out of memory, -3 CUDA error,
+ *     -4 non-finite input or result, -5 marker cloud too wide for the factorised entropy kernel
+ *     AND the literal fallback disabled (never returned with default options).
+ *     No exception or abort crosses this boundary; landau_last_error() returns a message.
+ *   - There is NO CPU fallback: without a CUDA device landau_create fails with -3.
+ */
+#ifndef LANDAU_H
+#define LANDAU_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LANDAU_OK 0
+#define LANDAU_NOT_CONVERGED 1
+#define LANDAU_EINVAL (-1)
+#define LANDAU_ENOMEM (-2)
+#define LANDAU_ECUDA (-3)
+#define LANDAU_ENONFINITE (-4)
+#define LANDAU_ERANGE (-5)
+
+#define LANDAU_MAX_SPECIES 16
+#define LANDAU_MAX_NQ 8
+
+typedef struct landau_ctx landau_ctx; /* opaque, library-owned */
+
+typedef struct {
+    int n_q;          /* Gauss-Hermite knots per axis (reading S3); 0 -> 4; 2..8 */
+    double nu0;       /* nu_ss' = nu0 q_s^2 q_s'^2 (reading U1); 0 -> 1.0            */
+    const double* nu; /* optional HOST S x S override of nu_ss', must be symmetric; may be NULL   */
+    int precision;    /* 0 = FP64 everywhere; 1 = FP32 arithmetic inside the pairwise sum of
+                         landau_pair_field / landau_eval_field only (BASELINE config 4 variant)   */
+    void* stream;     /* cudaStream_t; NULL = default stream                                      */
+    int pair_kernel;  /* 0 = automatic; 1 = one-sided tiled kernel; 2 = symmetric (action-reaction)
+                         kernel.  For tests and per-kernel timing.                                */
+    int entropy_kernel; /* 0 = automatic; 1 = literal separable form (3 n_q exponentials per
+                         pair); 2 = factorised form (1 exponential per pair)                     */
+    int device;       /* CUDA device ordinal; -1 = current device                                 */
+} landau_opts;
+
+typedef struct {
+    int iterations;   /* fixed-point iterations done (k+1 of DESIGN.md O4) */
+    double residual;  /* r_k of the last iteration                          */
+    int converged;    /* 1 if r_k <= tol                                    */
+} landau_step_info;
+
+/* Fills *opts with the defaults (n_q 4, nu0 1, FP64, default stream, automatic kernels). */
+void landau_default_opts(landau_opts* opts);
+
+/* Species table: masses m_s > 0, charges q_s, mollifier covariances eps_s > 0 (Eq. 19,
+ * PAPER.md:112-116; units velocity^2), all HOST arrays of n_species <= LANDAU_MAX_SPECIES
+ * entries.  opts may be NULL (defaults). */
+int landau_create(landau_ctx** out, int n_species, const double* mass, const double* charge,
+                  const double* eps, const landau_opts* opts);
+void landau_destroy(landau_ctx* ctx);
+
+/* V_p of Eq. (23) with G from Eq. (22): pass 1 then pass 2.  Stateless with respect to the
+ * markers held by landau_set_markers. */
+int landau_eval_field(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                      const int32_t* species_id, double* out);
+int landau_eval_field_host(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                           const int32_t* species_id, double* out);
+
+/* Pass 1 alone: G_out[N x 3] = (1/w_p) dS_eps/dv_p (Eq. 22; Eq. 14).
+ * S_eps_out: optional HOST array of S entries receiving S_eps,s (Eq. 20); may be NULL. */
+int landau_entropy_grad(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                        const int32_t* species_id, double* G_out, double* S_eps_out);
+
+/* Pass 2 alone with the entropy gradient supplied: out[N x 3] = V_p of Eq. (23) for G_in. */
+int landau_pair_field(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                      const int32_t* species_id, const double* G_in, double* out);
+
+/* Time stepping works on markers held by the context. */
+int landau_set_markers(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                       const int32_t* species_id);
+int landau_set_markers_host(landau_ctx* ctx, int64_t N, const double* v, const double* w,
+                            const int32_t* species_id);
+int landau_get_markers(landau_ctx* ctx, double* v_out /* device, N x 3, caller order */);
+int landau_get_markers_host(landau_ctx* ctx, double* v_out /* host */);
+
+/* One step of Eq. (24): pass 1 once at v^n, then Jacobi fixed-point iterations, each one pass 2 at
+ * the midpoint (Eq. 25) with G^n frozen, until r_k <= tol or max_iter iterations, where
+ *   r_k = sqrt( sum_p w_p m_s |v^(k+1)_p - v^(k)_p|^2 / sum_p w_p m_s |v^(k+1)_p|^2 )  (reading S7).
+ * The loop runs on the device (no host synchronisation per iteration).  info may be NULL.
+ * Returns 0, or 1 if not converged (state still advanced; reading S8). */
+int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
+
+/* n_steps consecutive steps with one host synchronisation at the end; info (optional, HOST,
+ * n_steps entries) receives each step's record.  Returns 1 if any step did not converge. */
+int landau_run(landau_ctx* ctx, int n_steps, double dt, double tol, int max_iter,
+               landau_step_info* info);
+
+/* Moments of the held markers, HOST outputs, any may be NULL:
+ * n[S] = sum w (Eq. 33), P[S x 3] = m_s sum w v (Eq. 26), K[S] = (m_s/2) sum w |v|^2 (Eq. 28),
+ * S_eps[S] = regularised entropy (Eq. 20; costs one pass 1). */
+int landau_moments(landau_ctx* ctx, double* n, double* P, double* K, double* S_eps);
+/* stress[S x 6] = m_s sum w v_i v_j (xx,yy,zz,xy,xz,yz); m4[S x 3] = sum w (v_i - u_i)^4
+ * (per-axis temperatures Eqs. 30-31 and kurtosis are derived from these by the caller). */
+int landau_moments_ext(landau_ctx* ctx, double* stress, double* m4);
+
+/* Gauss-Hermite rule the context uses (HOST outputs, n_q entries each). */
+int landau_get_quadrature(const landau_ctx* ctx, double* knots, double* weights);
+
+/* Names of the kernels the last field evaluation / step used, e.g. "pair=sym entropy=fact". */
+const char* landau_last_kernels(const landau_ctx* ctx);
+/* Number of kernel launches issued by this context so far. */
+int64_t landau_launch_count(const landau_ctx* ctx);
+
+/* FP64 ALU peak microbenchmark (dependent-free DFMA streams on every SM): runs `reps` launches and
+ * returns the best rate in FLOP/s (2 per DFMA) through *flops_out (HOST). Used by bench.py for the
+ * roofline denominator. */
+int landau_fp64_peak(landau_ctx* ctx, int reps, double* flops_out);
+
+const char* landau_last_error(const landau_ctx* ctx);
+const char* landau_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LANDAU_H */

@@ -1,0 +1,256 @@
+"""Thin ctypes binding over the C ABI of include/landau.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of liblandau.so.  PyTorch is used for device
+memory only: device-pointer calls take torch CUDA tensors (float64 / int32, contiguous) and
+return torch CUDA tensors; the *_host calls take numpy arrays and let the library do the copies.
+There is NO CPU fallback: a missing library or a missing CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+OK = 0
+NOT_CONVERGED = 1
+EINVAL, ENOMEM, ECUDA, ENONFINITE, ERANGE = -1, -2, -3, -4, -5
+
+# every symbol include/landau.h declares (tests check the .so exports exactly these)
+SYMBOLS = [
+    "landau_default_opts", "landau_create", "landau_destroy", "landau_eval_field",
+    "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
+    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step",
+    "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
+    "landau_last_kernels", "landau_launch_count", "landau_fp64_peak", "landau_last_error",
+    "landau_version",
+]
+
+
+class Opts(C.Structure):
+    _fields_ = [("n_q", C.c_int), ("nu0", C.c_double), ("nu", C.POINTER(C.c_double)),
+                ("precision", C.c_int), ("stream", C.c_void_p), ("pair_kernel", C.c_int),
+                ("entropy_kernel", C.c_int), ("device", C.c_int)]
+
+
+class StepInfo(C.Structure):
+    _fields_ = [("iterations", C.c_int), ("residual", C.c_double), ("converged", C.c_int)]
+
+
+class LandauError(RuntimeError):
+    def __init__(self, code, where, msg=""):
+        super().__init__(f"{where} failed with status {code}: {msg}")
+        self.code = code
+
+
+def library_path() -> Path:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """Load liblandau.so (building it with nvcc if needed).  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        _build.build()
+    if not _build.LIB.exists():
+        raise RuntimeError(f"{_build.LIB} is missing: build it with `python -m paper_2212_00663_b200.build` "
+                           "(the CUDA path has no fallback)")
+    lib = C.CDLL(str(_build.LIB))
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p   # raw addresses (device or host)
+    hd = C.POINTER(C.c_double)
+    lib.landau_default_opts.argtypes = [C.POINTER(Opts)]
+    lib.landau_default_opts.restype = None
+    lib.landau_create.argtypes = [C.POINTER(vp), C.c_int, hd, hd, hd, C.POINTER(Opts)]
+    lib.landau_destroy.argtypes = [vp]
+    lib.landau_destroy.restype = None
+    lib.landau_eval_field.argtypes = [vp, C.c_int64, dp, dp, ip, dp]
+    lib.landau_eval_field_host.argtypes = [vp, C.c_int64, dp, dp, ip, dp]
+    lib.landau_entropy_grad.argtypes = [vp, C.c_int64, dp, dp, ip, dp, hd]
+    lib.landau_pair_field.argtypes = [vp, C.c_int64, dp, dp, ip, dp, dp]
+    lib.landau_set_markers.argtypes = [vp, C.c_int64, dp, dp, ip]
+    lib.landau_set_markers_host.argtypes = [vp, C.c_int64, dp, dp, ip]
+    lib.landau_get_markers.argtypes = [vp, dp]
+    lib.landau_get_markers_host.argtypes = [vp, dp]
+    lib.landau_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
+    lib.landau_run.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
+    lib.landau_moments.argtypes = [vp, hd, hd, hd, hd]
+    lib.landau_moments_ext.argtypes = [vp, hd, hd]
+    lib.landau_get_quadrature.argtypes = [vp, hd, hd]
+    lib.landau_last_kernels.argtypes = [vp]
+    lib.landau_last_kernels.restype = C.c_char_p
+    lib.landau_launch_count.argtypes = [vp]
+    lib.landau_launch_count.restype = C.c_int64
+    lib.landau_fp64_peak.argtypes = [vp, C.c_int, hd]
+    lib.landau_last_error.argtypes = [vp]
+    lib.landau_last_error.restype = C.c_char_p
+    lib.landau_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _hd(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class Landau:
+    """One context = one species table + one CUDA stream (+ optionally held markers)."""
+
+    def __init__(self, mass, charge, eps, n_q: int = 4, nu0: float = 1.0, nu=None, precision: int = 0,
+                 stream=None, pair_kernel: int = 0, entropy_kernel: int = 0, device: int = -1):
+        import torch  # device memory + streams only
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2212_00663_b200 needs a CUDA device (no CPU fallback)")
+        self._torch = torch
+        self._lib = load()
+        self.mass, self.charge, self.eps = _f64(mass), _f64(charge), _f64(eps)
+        self.S = int(self.mass.shape[0])
+        self.n_q = int(n_q)
+        o = Opts()
+        self._lib.landau_default_opts(C.byref(o))
+        o.n_q, o.nu0, o.precision = int(n_q), float(nu0), int(precision)
+        o.pair_kernel, o.entropy_kernel, o.device = int(pair_kernel), int(entropy_kernel), int(device)
+        self._nu = None if nu is None else _f64(nu)
+        if self._nu is not None:
+            o.nu = _hd(self._nu)
+        if stream is not None:
+            o.stream = C.c_void_p(int(stream.cuda_stream if hasattr(stream, "cuda_stream") else stream))
+        self._dev = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
+        h = C.c_void_p()
+        rc = self._lib.landau_create(C.byref(h), self.S, _hd(self.mass), _hd(self.charge), _hd(self.eps), C.byref(o))
+        if rc:
+            raise LandauError(rc, "landau_create")
+        self._h = h
+        self.N = 0
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.landau_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, where, allow=(0,)):
+        if rc not in allow:
+            raise LandauError(rc, where, self._lib.landau_last_error(self._h).decode())
+        return rc
+
+    def _dev_in(self, v, w, sid):
+        t = self._torch
+        v = t.as_tensor(v, dtype=t.float64, device=self._dev).contiguous()
+        w = t.as_tensor(w, dtype=t.float64, device=self._dev).contiguous()
+        sid = t.as_tensor(sid, dtype=t.int32, device=self._dev).contiguous()
+        return v, w, sid, int(w.shape[0])
+
+    def last_kernels(self) -> str:
+        return self._lib.landau_last_kernels(self._h).decode()
+
+    def launch_count(self) -> int:
+        return int(self._lib.landau_launch_count(self._h))
+
+    def quadrature(self):
+        k, a = np.empty(self.n_q), np.empty(self.n_q)
+        self._check(self._lib.landau_get_quadrature(self._h, _hd(k), _hd(a)), "landau_get_quadrature")
+        return k, a
+
+    # -- field ------------------------------------------------------------------------------
+    def eval_field(self, v, w, sid):
+        v, w, sid, N = self._dev_in(v, w, sid)
+        out = self._torch.empty((N, 3), dtype=self._torch.float64, device=self._dev)
+        self._check(self._lib.landau_eval_field(self._h, N, v.data_ptr(), w.data_ptr(), sid.data_ptr(),
+                                                out.data_ptr()), "landau_eval_field")
+        return out
+
+    def eval_field_host(self, v, w, sid):
+        v, w = _f64(v), _f64(w)
+        sid = np.ascontiguousarray(sid, dtype=np.int32)
+        out = np.empty((w.shape[0], 3))
+        self._check(self._lib.landau_eval_field_host(self._h, w.shape[0], v.ctypes.data, w.ctypes.data,
+                                                     sid.ctypes.data, out.ctypes.data), "landau_eval_field_host")
+        return out
+
+    def entropy_grad(self, v, w, sid, with_entropy: bool = False):
+        v, w, sid, N = self._dev_in(v, w, sid)
+        G = self._torch.empty((N, 3), dtype=self._torch.float64, device=self._dev)
+        S = np.empty(self.S)
+        self._check(self._lib.landau_entropy_grad(self._h, N, v.data_ptr(), w.data_ptr(), sid.data_ptr(),
+                                                  G.data_ptr(), _hd(S) if with_entropy else None),
+                    "landau_entropy_grad")
+        return (G, S) if with_entropy else G
+
+    def pair_field(self, v, w, sid, G):
+        v, w, sid, N = self._dev_in(v, w, sid)
+        G = self._torch.as_tensor(G, dtype=self._torch.float64, device=self._dev).contiguous()
+        out = self._torch.empty((N, 3), dtype=self._torch.float64, device=self._dev)
+        self._check(self._lib.landau_pair_field(self._h, N, v.data_ptr(), w.data_ptr(), sid.data_ptr(),
+                                                G.data_ptr(), out.data_ptr()), "landau_pair_field")
+        return out
+
+    # -- stepping ---------------------------------------------------------------------------
+    def set_markers(self, v, w, sid):
+        v, w, sid, N = self._dev_in(v, w, sid)
+        self._check(self._lib.landau_set_markers(self._h, N, v.data_ptr(), w.data_ptr(), sid.data_ptr()),
+                    "landau_set_markers")
+        self.N = N
+
+    def set_markers_host(self, v, w, sid):
+        v, w = _f64(v), _f64(w)
+        sid = np.ascontiguousarray(sid, dtype=np.int32)
+        self._check(self._lib.landau_set_markers_host(self._h, w.shape[0], v.ctypes.data, w.ctypes.data,
+                                                      sid.ctypes.data), "landau_set_markers_host")
+        self.N = int(w.shape[0])
+
+    def get_markers(self):
+        out = self._torch.empty((self.N, 3), dtype=self._torch.float64, device=self._dev)
+        self._check(self._lib.landau_get_markers(self._h, out.data_ptr()), "landau_get_markers")
+        return out
+
+    def get_markers_host(self):
+        out = np.empty((self.N, 3))
+        self._check(self._lib.landau_get_markers_host(self._h, out.ctypes.data), "landau_get_markers_host")
+        return out
+
+    def step(self, dt, tol=1e-12, max_iter=50):
+        """Returns (status, iterations, residual, converged); status 1 = not converged."""
+        info = StepInfo()
+        rc = self._check(self._lib.landau_step(self._h, float(dt), float(tol), int(max_iter), C.byref(info)),
+                         "landau_step", allow=(0, 1))
+        return rc, int(info.iterations), float(info.residual), bool(info.converged)
+
+    def run(self, n_steps, dt, tol=1e-12, max_iter=50):
+        """n_steps steps, one host sync.  Returns (status, [(iterations, residual, converged)])."""
+        infos = (StepInfo * int(n_steps))()
+        rc = self._check(self._lib.landau_run(self._h, int(n_steps), float(dt), float(tol), int(max_iter), infos),
+                         "landau_run", allow=(0, 1))
+        return rc, [(int(i.iterations), float(i.residual), bool(i.converged)) for i in infos]
+
+    def moments(self, with_entropy: bool = True):
+        n, P, K, S = np.empty(self.S), np.empty((self.S, 3)), np.empty(self.S), np.empty(self.S)
+        self._check(self._lib.landau_moments(self._h, _hd(n), _hd(P), _hd(K), _hd(S) if with_entropy else None),
+                    "landau_moments")
+        return dict(n=n, P=P, K=K, S_eps=S if with_entropy else None)
+
+    def moments_ext(self):
+        stress, m4 = np.empty((self.S, 6)), np.empty((self.S, 3))
+        self._check(self._lib.landau_moments_ext(self._h, _hd(stress), _hd(m4)), "landau_moments_ext")
+        return stress, m4
+
+    def fp64_peak(self, reps: int = 5) -> float:
+        out = C.c_double(0.0)
+        self._check(self._lib.landau_fp64_peak(self._h, int(reps), C.byref(out)), "landau_fp64_peak")
+        return float(out.value)

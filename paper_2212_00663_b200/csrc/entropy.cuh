@@ -1,0 +1,148 @@
+// entropy.cuh -- steps a1/a2 of the hot path: mollified density at the Gauss-Hermite nodes and the
+// entropy gradient, 3-V restatement of Eq. (22) (Eqs. 19-21).
+//
+//   rho_p(k) = sum_{q in s(p)} w_q (2 pi eps_s)^(-3/2) exp(-|k + (v_p - v_q)/sqrt(2 eps_s)|^2)
+//   G_p      = -sqrt(2/eps_s) pi^(-3/2) sum_{ijl} a_i a_j a_l (k_i,k_j,k_l) [1 + ln rho_p(k_ijl)]
+//   s_p      = sum_{ijl} a_i a_j a_l ln rho_p(k_ijl)        (S_eps,s = -pi^(-3/2) sum_p w_p s_p)
+//
+// Two all-pairs kernels produce the node sums  A_p(k) = sum_q w_q exp(...)  :
+//   * literal-separable:  exp(-|k+d|^2) = prod_axis exp(-(k_i + d_axis)^2): 3 n_q exponentials per
+//     pair, every factor <= 1, no overflow anywhere; valid for any marker cloud.
+//   * factorised (entropy_fact.cuh): one exponential per pair, per-marker tables.
+// entropy_finalize_kernel turns node sums into G_p and s_p (n_q^3 logarithms per marker).
+#pragma once
+#include "common.cuh"
+
+namespace landau {
+
+constexpr int ENT_THREADS = 128;   // targets per block (one target per thread)
+constexpr int ENT_SRC_TILE = 64;   // sources staged in shared memory per tile
+
+// Node sums are stored node-major: part[((chunk * M + node) * npad_max) + slot].
+//
+// NQ knots per axis; each thread owns NI consecutive x-node indices i (i0 = blockIdx.z * NI) and all
+// (j,l): NI*NQ*NQ accumulators in registers.
+template <int NQ, int NI>
+__global__ void __launch_bounds__(ENT_THREADS)
+entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
+                       int nchunks, const double* __restrict__ x, const double* __restrict__ y,
+                       const double* __restrict__ z, const double* __restrict__ w,
+                       double* __restrict__ part) {
+    const int slot0 = blockIdx.x * ENT_THREADS;
+    if (slot0 >= L->npad) return;
+    const int S = T->S;
+    const int s = species_of_slot(L, S, slot0);
+    const double inv = T->inv_sqrt_2eps[s];
+    const int src0 = L->off[s], src1 = L->off[s + 1];
+    const int ntiles = (src1 - src0) / ENT_SRC_TILE;
+    const int tpc = ceil_div(ntiles, nchunks);
+    const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
+    const int i0 = (NI == NQ) ? 0 : blockIdx.z * NI;
+
+    __shared__ double sx[ENT_SRC_TILE], sy[ENT_SRC_TILE], sz[ENT_SRC_TILE], sw[ENT_SRC_TILE];
+    double kn[NQ];
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) kn[i] = T->knot[i];
+
+    const int p = slot0 + threadIdx.x;
+    const double px = x[p] * inv, py = y[p] * inv, pz = z[p] * inv;
+    double acc[NI][NQ][NQ];
+#pragma unroll
+    for (int i = 0; i < NI; ++i)
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+            for (int l = 0; l < NQ; ++l) acc[i][j][l] = 0.0;
+
+    for (int t = t0; t < t1; ++t) {
+        __syncthreads();
+        if (threadIdx.x < ENT_SRC_TILE) {
+            const int q = src0 + t * ENT_SRC_TILE + threadIdx.x;
+            sx[threadIdx.x] = x[q] * inv;
+            sy[threadIdx.x] = y[q] * inv;
+            sz[threadIdx.x] = z[q] * inv;
+            sw[threadIdx.x] = w[q];
+        }
+        __syncthreads();
+#pragma unroll 1
+        for (int j0 = 0; j0 < ENT_SRC_TILE; ++j0) {
+            const double dx = px - sx[j0], dy = py - sy[j0], dz = pz - sz[j0];
+            const double wq = sw[j0];
+            double ex[NI], ey[NQ], ez[NQ];
+#pragma unroll
+            for (int i = 0; i < NI; ++i) { const double a = kn[i0 + i] + dx; ex[i] = wq * exp(-a * a); }
+#pragma unroll
+            for (int i = 0; i < NQ; ++i) { const double a = kn[i] + dy; ey[i] = exp(-a * a); }
+#pragma unroll
+            for (int i = 0; i < NQ; ++i) { const double a = kn[i] + dz; ez[i] = exp(-a * a); }
+#pragma unroll
+            for (int i = 0; i < NI; ++i)
+#pragma unroll
+                for (int j = 0; j < NQ; ++j) {
+                    const double b = ex[i] * ey[j];
+#pragma unroll
+                    for (int l = 0; l < NQ; ++l) acc[i][j][l] = fma(b, ez[l], acc[i][j][l]);
+                }
+        }
+    }
+    const size_t M = (size_t)NQ * NQ * NQ;
+#pragma unroll
+    for (int i = 0; i < NI; ++i)
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+            for (int l = 0; l < NQ; ++l) {
+                const size_t node = ((size_t)(i0 + i) * NQ + j) * NQ + l;
+                part[((size_t)blockIdx.y * M + node) * (size_t)npad_max + p] = acc[i][j][l];
+            }
+}
+
+// Node sums -> G_p (unscaled: (1/w_p) dS_eps/dv_p) and s_p.  `shift` (optional) holds per-slot
+// log-space corrections used by the factorised kernel; NULL for the literal kernel.
+__global__ void __launch_bounds__(128)
+entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, int npad_max,
+                        int nchunks, const int* __restrict__ perm, const double* __restrict__ part,
+                        const double* __restrict__ px, const double* __restrict__ py,
+                        const double* __restrict__ pz, int factorised,
+                        double* __restrict__ Gx, double* __restrict__ Gy, double* __restrict__ Gz,
+                        double* __restrict__ snode) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npad_max || p >= L->npad) return;
+    if (perm[p] < 0) { Gx[p] = 0.0; Gy[p] = 0.0; Gz[p] = 0.0; snode[p] = 0.0; return; }
+    const int S = T->S, nq = T->n_q;
+    const int s = species_of_slot(L, S, p);
+    const double eps = T->eps[s];
+    const double PI = 3.14159265358979323846;
+    const double lognorm = -1.5 * log(2.0 * PI * eps);
+    const size_t M = (size_t)nq * nq * nq;
+    // factorised form: ln A_p(k) = -|k|^2 - 2 k.(p - c) + ln(sum); (p - c) in mollifier units
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    if (factorised) {
+        const double inv = T->inv_sqrt_2eps[s];
+        cx = (px[p] - L->center[s][0]) * inv;
+        cy = (py[p] - L->center[s][1]) * inv;
+        cz = (pz[p] - L->center[s][2]) * inv;
+    }
+    double gx = 0.0, gy = 0.0, gz = 0.0, sn = 0.0;
+    for (int i = 0; i < nq; ++i)
+        for (int j = 0; j < nq; ++j)
+            for (int l = 0; l < nq; ++l) {
+                const size_t node = ((size_t)i * nq + j) * nq + l;
+                double a = 0.0;
+                for (int c = 0; c < nchunks; ++c) a += part[((size_t)c * M + node) * (size_t)npad_max + p];
+                const double ki = T->knot[i], kj = T->knot[j], kl = T->knot[l];
+                double lnrho = lognorm + log(a);
+                if (factorised)
+                    lnrho -= (ki * ki + kj * kj + kl * kl) + 2.0 * (ki * cx + kj * cy + kl * cz);
+                const double aaa = T->gw[i] * T->gw[j] * T->gw[l];
+                const double t = aaa * (1.0 + lnrho);
+                gx = fma(t, ki, gx); gy = fma(t, kj, gy); gz = fma(t, kl, gz);
+                sn = fma(aaa, lnrho, sn);
+            }
+    const double pref = -sqrt(2.0 / eps) / (PI * sqrt(PI));
+    gx *= pref; gy *= pref; gz *= pref;
+    if (!(isfinite(gx) && isfinite(gy) && isfinite(gz) && isfinite(sn))) atomicMin(&L->err, -4);
+    Gx[p] = gx; Gy[p] = gy; Gz[p] = gz; snode[p] = sn;
+}
+
+}  // namespace landau

@@ -1,0 +1,682 @@
+// landau_api.cu -- the C ABI of include/landau.h: context, scratch management, launch logic.
+// Every arithmetic step of the path runs in the kernels of this directory; there is no CPU
+// fallback and nothing here touches oracle/.
+#include "../../include/landau.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "entropy.cuh"
+#include "moments.cuh"
+#include "pack.cuh"
+#include "pair.cuh"
+#include "step.cuh"
+
+using namespace landau;
+
+namespace {
+
+struct Buf {
+    void* p = nullptr;
+    size_t cap = 0;
+};
+
+// Packed marker cloud (device).  Two live in a context: `tmp` for the stateless calls and `state`
+// for the markers held by landau_set_markers.
+struct Cloud {
+    int64_t N = 0;
+    int npad_max = 0;
+    int pad = 0;
+    Buf lay, xyzw, perm, G, rec;
+    DevLayout* L() const { return (DevLayout*)lay.p; }
+    double* x() const { return (double*)xyzw.p; }
+    double* y() const { return x() + npad_max; }
+    double* z() const { return x() + 2 * (size_t)npad_max; }
+    double* w() const { return x() + 3 * (size_t)npad_max; }
+    int* prm() const { return (int*)perm.p; }
+    double* Gx() const { return (double*)G.p; }
+    double* Gy() const { return Gx() + npad_max; }
+    double* Gz() const { return Gx() + 2 * (size_t)npad_max; }
+    double* snode() const { return Gx() + 3 * (size_t)npad_max; }
+    double* recs() const { return (double*)rec.p; }
+};
+
+}  // namespace
+
+struct landau_ctx {
+    int S = 0;
+    int n_q = 4;
+    int precision = 0;
+    int pair_kernel = 0;
+    int entropy_kernel = 0;
+    int device = 0;
+    int sm_count = 148;
+    cudaStream_t stream = nullptr;
+    double mass[LD_MAX_SPECIES], charge[LD_MAX_SPECIES], eps[LD_MAX_SPECIES];
+    double nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
+    double knot[LD_MAX_NQ], gw[LD_MAX_NQ];
+    DevTable* d_tab = nullptr;
+    StepCtrl* d_ctrl = nullptr;
+    int* d_cursor = nullptr;
+    double* d_momout = nullptr;           // S x MOM_OUT
+    void* h_pin = nullptr;                // pinned read-back area
+    Cloud tmp, state;
+    Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
+    Buf facttab;
+    int64_t launches = 0;
+    char err[512];
+    char kernels[128];
+};
+
+namespace {
+
+constexpr size_t PIN_BYTES = 1 << 16;
+
+int fail(landau_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CU(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(c, e_ == cudaErrorMemoryAllocation ? LANDAU_ENOMEM : LANDAU_ECUDA,    \
+                        "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+#define RC(call)             \
+    do {                     \
+        int rc_ = (call);    \
+        if (rc_ < 0) return rc_; \
+    } while (0)
+
+int ensure(landau_ctx* c, Buf& b, size_t bytes) {
+    if (bytes <= b.cap) return 0;
+    if (b.p) CU(cudaFree(b.p));
+    b.p = nullptr; b.cap = 0;
+    size_t want = bytes + bytes / 8 + 256;
+    CU(cudaMalloc(&b.p, want));
+    b.cap = want;
+    return 0;
+}
+
+void release(Buf& b) {
+    if (b.p) cudaFree(b.p);
+    b.p = nullptr; b.cap = 0;
+}
+
+// Gauss-Hermite rule for the weight exp(-k^2) by Golub-Welsch: knots are the eigenvalues of the
+// symmetric tridiagonal Jacobi matrix J (zero diagonal, off-diagonal sqrt(i/2)), weights are
+// sqrt(pi) times the squared first components of the normalised eigenvectors.  Eigen-decomposition
+// by cyclic Jacobi rotations in long double (n <= 8).
+void gauss_hermite_gw(int n, double* knots, double* weights) {
+    long double A[LD_MAX_NQ][LD_MAX_NQ] = {}, V[LD_MAX_NQ][LD_MAX_NQ] = {};
+    for (int i = 0; i < n; ++i) V[i][i] = 1.0L;
+    for (int i = 1; i < n; ++i) A[i][i - 1] = A[i - 1][i] = sqrtl(0.5L * i);
+    for (int sweep = 0; sweep < 100; ++sweep) {
+        long double off = 0.0L;
+        for (int i = 0; i < n; ++i)
+            for (int j = i + 1; j < n; ++j) off += A[i][j] * A[i][j];
+        if (off < 1e-40L) break;
+        for (int p = 0; p < n; ++p)
+            for (int q = p + 1; q < n; ++q) {
+                if (fabsl(A[p][q]) < 1e-300L) continue;
+                const long double theta = (A[q][q] - A[p][p]) / (2.0L * A[p][q]);
+                const long double t = (theta >= 0 ? 1.0L : -1.0L) / (fabsl(theta) + sqrtl(theta * theta + 1.0L));
+                const long double cs = 1.0L / sqrtl(t * t + 1.0L), sn = t * cs;
+                for (int k = 0; k < n; ++k) {
+                    const long double akp = A[k][p], akq = A[k][q];
+                    A[k][p] = cs * akp - sn * akq;
+                    A[k][q] = sn * akp + cs * akq;
+                }
+                for (int k = 0; k < n; ++k) {
+                    const long double apk = A[p][k], aqk = A[q][k];
+                    A[p][k] = cs * apk - sn * aqk;
+                    A[q][k] = sn * apk + cs * aqk;
+                }
+                for (int k = 0; k < n; ++k) {
+                    const long double vkp = V[k][p], vkq = V[k][q];
+                    V[k][p] = cs * vkp - sn * vkq;
+                    V[k][q] = sn * vkp + cs * vkq;
+                }
+            }
+    }
+    int idx[LD_MAX_NQ];
+    for (int i = 0; i < n; ++i) idx[i] = i;
+    std::sort(idx, idx + n, [&](int a, int b) { return A[a][a] < A[b][b]; });
+    const long double sqrt_pi = 1.77245385090551602729816748334114518L;
+    for (int i = 0; i < n; ++i) {
+        knots[i] = (double)A[idx[i]][idx[i]];
+        weights[i] = (double)(sqrt_pi * V[0][idx[i]] * V[0][idx[i]]);
+    }
+    // enforce the exact antisymmetry of the knot set (k_i = -k_{n-1-i}; middle knot 0 for odd n)
+    for (int i = 0; i < n / 2; ++i) {
+        const double k = 0.5 * (knots[n - 1 - i] - knots[i]);
+        const double a = 0.5 * (weights[n - 1 - i] + weights[i]);
+        knots[i] = -k; knots[n - 1 - i] = k;
+        weights[i] = a; weights[n - 1 - i] = a;
+    }
+    if (n & 1) knots[n / 2] = 0.0;
+}
+
+int choose_pad(const landau_ctx* c, int64_t N) {
+    (void)c; (void)N;
+    return 128;
+}
+
+int npad_upper(int64_t N, int S, int pad) {
+    const int64_t up = N + (int64_t)S * (pad - 1);
+    return (int)(((up + pad - 1) / pad) * pad);
+}
+
+
+// ---- optimised kernels (filled in below when available) -------------------------------------
+int entropy_fact_available(int nq) { (void)nq; return 0; }
+int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) { (void)c; (void)cl; (void)nchunks; return LANDAU_ECUDA; }
+int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; (void)cl; return 0; }
+int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts) { (void)c; (void)cl; (void)ctrl; (void)nparts; return LANDAU_ECUDA; }
+
+// ---- a0: pack -----------------------------------------------------------------------------
+int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, const int32_t* sid) {
+    if (!c) return LANDAU_EINVAL;
+    if (N < 1 || !v || !w || !sid) return fail(c, LANDAU_EINVAL, "pack: NULL array or N < 1");
+    if (N > (int64_t)1 << 24) return fail(c, LANDAU_EINVAL, "pack: N = %lld exceeds 2^24 markers", (long long)N);
+    const int S = c->S;
+    const int pad = choose_pad(c, N);
+    const int npm = npad_upper(N, S, pad);
+    cl.N = N; cl.npad_max = npm; cl.pad = pad;
+    RC(ensure(c, cl.lay, sizeof(DevLayout)));
+    RC(ensure(c, cl.xyzw, sizeof(double) * 4 * (size_t)npm));
+    RC(ensure(c, cl.perm, sizeof(int) * (size_t)npm));
+    RC(ensure(c, cl.G, sizeof(double) * 4 * (size_t)npm));
+    RC(ensure(c, cl.rec, sizeof(double) * 8 * (size_t)npm));
+    const int nb = ceil_div((int)N, PACK_THREADS);
+    RC(ensure(c, c->blockcnt, sizeof(int) * (size_t)nb * S));
+    RC(ensure(c, c->blockoff, sizeof(int) * (size_t)nb * S));
+    cudaStream_t st = c->stream;
+    CU(cudaMemsetAsync(cl.lay.p, 0, sizeof(DevLayout), st));
+    CU(cudaMemsetAsync(cl.xyzw.p, 0, sizeof(double) * 4 * (size_t)npm, st));
+    CU(cudaMemsetAsync(cl.perm.p, 0xFF, sizeof(int) * (size_t)npm, st));
+    pack_count_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, sid, S, (int*)c->blockcnt.p, cl.L());
+    pack_scan_kernel<<<1, 32, 0, st>>>(nb, S, pad, (const int*)c->blockcnt.p, (int*)c->blockoff.p, cl.L());
+    pack_scatter_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, sid, S, (const int*)c->blockoff.p, cl.L(),
+                                                      cl.x(), cl.y(), cl.z(), cl.w(), cl.prm());
+    c->launches += 3;
+    CU(cudaGetLastError());
+    return 0;
+}
+
+// ---- a1/a2: entropy gradient of a packed cloud ---------------------------------------------
+template <int NQ, int NI>
+void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks) {
+    dim3 grid(cl.npad_max / ENT_THREADS, nchunks, NQ / NI);
+    entropy_literal_kernel<NQ, NI><<<grid, ENT_THREADS, 0, c->stream>>>(
+        c->d_tab, cl.L(), cl.npad_max, nchunks, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->part.p);
+}
+
+int entropy(landau_ctx* c, Cloud& cl) {
+    const int nq = c->n_q;
+    const size_t M = (size_t)nq * nq * nq;
+    const int ttiles = cl.npad_max / ENT_THREADS;
+    const int ig = nq <= 4 ? 1 : nq;
+    int nchunks = ceil_div(6 * c->sm_count, ttiles * ig);
+    nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / ENT_SRC_TILE)));
+    nchunks = std::min(nchunks, 64);
+    while (nchunks > 1 && (size_t)nchunks * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) --nchunks;
+    RC(ensure(c, c->part, (size_t)nchunks * M * cl.npad_max * sizeof(double)));
+    int use_fact = 0;
+    if (c->entropy_kernel == 2 || c->entropy_kernel == 0) use_fact = entropy_fact_available(nq);
+    if (use_fact) {
+        RC(launch_entropy_fact(c, cl, nchunks));
+    } else {
+        switch (nq) {
+            case 2: launch_entropy_literal<2, 2>(c, cl, nchunks); break;
+            case 3: launch_entropy_literal<3, 3>(c, cl, nchunks); break;
+            case 4: launch_entropy_literal<4, 4>(c, cl, nchunks); break;
+            case 5: launch_entropy_literal<5, 1>(c, cl, nchunks); break;
+            case 6: launch_entropy_literal<6, 1>(c, cl, nchunks); break;
+            case 7: launch_entropy_literal<7, 1>(c, cl, nchunks); break;
+            case 8: launch_entropy_literal<8, 1>(c, cl, nchunks); break;
+            default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
+        }
+        c->launches += 1;
+    }
+    entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
+        c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
+        use_fact, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
+    c->launches += 1;
+    CU(cudaGetLastError());
+    snprintf(c->kernels + 0, 32, "entropy=%s", use_fact ? "fact" : "literal");
+    return 0;
+}
+
+// ---- a3: pairwise field of source records -> partial fields ---------------------------------
+// Returns the number of partial slices written to c->vpart (to be summed in index order).
+int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
+    int use_sym = 0;
+    if (c->pair_kernel == 2 || c->pair_kernel == 0) use_sym = pair_sym_available(c, cl);
+    if (use_sym) {
+        RC(launch_pair_sym(c, cl, ctrl, nparts_out));
+        return 0;
+    }
+    constexpr int R = 2;
+    const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * R);
+    const int stiles = cl.npad_max / PAIR_SRC_TILE;
+    int nchunks = std::max(1, std::min(stiles, ceil_div(5 * c->sm_count, ttiles)));
+    nchunks = std::min(nchunks, 32);
+    RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
+    dim3 grid(ttiles, nchunks);
+    pair_onesided_kernel<R><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
+                                                                 cl.recs(), (double*)c->vpart.p);
+    c->launches += 1;
+    *nparts_out = nchunks;
+    return 0;
+}
+
+// Read the layout's error flag (one synchronisation).
+int finish(landau_ctx* c, Cloud& cl, const char* where) {
+    int* h = (int*)c->h_pin;
+    CU(cudaMemcpyAsync(h, &cl.L()->err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaGetLastError());
+    if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
+    if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
+    if (*h) return fail(c, *h, "%s: device-side error %d", where, *h);
+    return 0;
+}
+
+int field_of_cloud(landau_ctx* c, Cloud& cl, double* out) {
+    int nparts = 0;
+    build_rec_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
+                                                                        cl.z(), cl.w(), cl.Gx(), cl.Gy(), cl.Gz(),
+                                                                        cl.recs());
+    RC(pair(c, cl, nullptr, &nparts));
+    RC(ensure(c, c->V, sizeof(double) * 3 * (size_t)cl.npad_max));
+    double* Vx = (double*)c->V.p;
+    double* Vy = Vx + cl.npad_max;
+    double* Vz = Vy + cl.npad_max;
+    combine_field_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.L(), cl.npad_max, nparts,
+                                                                            (const double*)c->vpart.p, Vx, Vy, Vz);
+    scatter3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), Vx, Vy, Vz, out);
+    c->launches += 3;
+    CU(cudaGetLastError());
+    return 0;
+}
+
+int species_sums(landau_ctx* c, Cloud& cl, bool with_entropy, bool with_m4, double* h_out /* S x MOM_OUT */) {
+    const int nb = cl.npad_max / MOM_THREADS;
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(nb * MOM_NQ, 4096)));
+    CU(cudaMemsetAsync(c->d_momout, 0, sizeof(double) * LD_MAX_SPECIES * MOM_OUT, c->stream));
+    moments_block_kernel<<<nb, MOM_THREADS, 0, c->stream>>>(cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                            with_entropy ? cl.snode() : nullptr,
+                                                            (double*)c->blockpart.p);
+    moments_species_kernel<<<c->S, MOM_THREADS, 0, c->stream>>>(cl.L(), (const double*)c->blockpart.p, MOM_NQ, 0,
+                                                               c->d_momout);
+    c->launches += 2;
+    if (with_m4) {
+        moments_m4_block_kernel<<<nb, MOM_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
+                                                                   cl.z(), cl.w(), c->d_momout,
+                                                                   (double*)c->blockpart.p);
+        moments_species_kernel<<<c->S, MOM_THREADS, 0, c->stream>>>(cl.L(), (const double*)c->blockpart.p, 3, 12,
+                                                                   c->d_momout);
+        c->launches += 2;
+    }
+    CU(cudaMemcpyAsync(h_out, c->d_momout, sizeof(double) * c->S * MOM_OUT, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaGetLastError());
+    return 0;
+}
+
+int stage_in(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid, const double** dv,
+             const double** dw, const int32_t** ds) {
+    if (N < 1 || !v || !w || !sid) return fail(c, LANDAU_EINVAL, "NULL array or N < 1");
+    RC(ensure(c, c->stage_v, sizeof(double) * 3 * (size_t)N));
+    RC(ensure(c, c->stage_w, sizeof(double) * (size_t)N));
+    RC(ensure(c, c->stage_s, sizeof(int32_t) * (size_t)N));
+    CU(cudaMemcpyAsync(c->stage_v.p, v, sizeof(double) * 3 * (size_t)N, cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->stage_w.p, w, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->stage_s.p, sid, sizeof(int32_t) * (size_t)N, cudaMemcpyHostToDevice, c->stream));
+    *dv = (const double*)c->stage_v.p; *dw = (const double*)c->stage_w.p; *ds = (const int32_t*)c->stage_s.p;
+    return 0;
+}
+
+__global__ void fp64_peak_kernel(double* out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) out[0] = s;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+void landau_default_opts(landau_opts* o) {
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->n_q = 4; o->nu0 = 1.0; o->nu = nullptr; o->precision = 0; o->stream = nullptr;
+    o->pair_kernel = 0; o->entropy_kernel = 0; o->device = -1;
+}
+
+const char* landau_version(void) { return "landau-b200 0.1 (sm_100a)"; }
+
+const char* landau_last_error(const landau_ctx* c) { return c ? c->err : "NULL context"; }
+const char* landau_last_kernels(const landau_ctx* c) { return c ? c->kernels : ""; }
+int64_t landau_launch_count(const landau_ctx* c) { return c ? c->launches : 0; }
+
+int landau_create(landau_ctx** out, int S, const double* mass, const double* charge, const double* eps,
+                  const landau_opts* opts) {
+    if (!out) return LANDAU_EINVAL;
+    *out = nullptr;
+    if (S < 1 || S > LD_MAX_SPECIES || !mass || !charge || !eps) return LANDAU_EINVAL;
+    landau_opts o;
+    landau_default_opts(&o);
+    if (opts) o = *opts;
+    if (o.n_q == 0) o.n_q = 4;
+    if (o.nu0 == 0.0) o.nu0 = 1.0;
+    if (o.n_q < 2 || o.n_q > LD_MAX_NQ) return LANDAU_EINVAL;
+    if (o.precision < 0 || o.precision > 1 || o.pair_kernel < 0 || o.pair_kernel > 2 || o.entropy_kernel < 0 ||
+        o.entropy_kernel > 2)
+        return LANDAU_EINVAL;
+    for (int s = 0; s < S; ++s)
+        if (!(mass[s] > 0.0) || !(eps[s] > 0.0) || !isfinite(charge[s]) || !isfinite(mass[s]) || !isfinite(eps[s]))
+            return LANDAU_EINVAL;
+    landau_ctx* c = new (std::nothrow) landau_ctx();
+    if (!c) return LANDAU_ENOMEM;
+    c->err[0] = 0; c->kernels[0] = 0;
+    c->S = S; c->n_q = o.n_q; c->precision = o.precision; c->pair_kernel = o.pair_kernel;
+    c->entropy_kernel = o.entropy_kernel; c->stream = (cudaStream_t)o.stream;
+    for (int s = 0; s < S; ++s) { c->mass[s] = mass[s]; c->charge[s] = charge[s]; c->eps[s] = eps[s]; }
+    for (int s = 0; s < S; ++s)
+        for (int t = 0; t < S; ++t)
+            c->nu[s * S + t] = o.nu ? o.nu[s * S + t] : o.nu0 * charge[s] * charge[s] * charge[t] * charge[t];
+    for (int s = 0; s < S; ++s)
+        for (int t = 0; t < S; ++t)
+            if (c->nu[s * S + t] != c->nu[t * S + s] || !isfinite(c->nu[s * S + t])) { delete c; return LANDAU_EINVAL; }
+    gauss_hermite_gw(c->n_q, c->knot, c->gw);
+
+    auto bail = [&](int code) { landau_destroy(c); return code; };
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete c; return LANDAU_ECUDA; }
+    if (o.device >= 0) { if (cudaSetDevice(o.device) != cudaSuccess) { delete c; return LANDAU_ECUDA; } }
+    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return LANDAU_ECUDA; }
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
+    DevTable t;
+    memset(&t, 0, sizeof(t));
+    t.S = S; t.n_q = c->n_q; t.pad = 128;
+    for (int s = 0; s < S; ++s) {
+        t.mass[s] = mass[s]; t.inv_mass[s] = 1.0 / mass[s]; t.eps[s] = eps[s];
+        t.inv_sqrt_2eps[s] = 1.0 / sqrt(2.0 * eps[s]);
+    }
+    for (int i = 0; i < S * S; ++i) t.nu[i] = c->nu[i];
+    for (int i = 0; i < c->n_q; ++i) { t.knot[i] = c->knot[i]; t.gw[i] = c->gw[i]; }
+    if (cudaMalloc(&c->d_tab, sizeof(DevTable)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMallocHost(&c->h_pin, PIN_BYTES) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMemcpy(c->d_tab, &t, sizeof(t), cudaMemcpyHostToDevice) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMemset(c->d_ctrl, 0, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    *out = c;
+    return LANDAU_OK;
+}
+
+void landau_destroy(landau_ctx* c) {
+    if (!c) return;
+    if (c->d_tab) cudaFree(c->d_tab);
+    if (c->d_ctrl) cudaFree(c->d_ctrl);
+    if (c->d_cursor) cudaFree(c->d_cursor);
+    if (c->d_momout) cudaFree(c->d_momout);
+    if (c->h_pin) cudaFreeHost(c->h_pin);
+    for (Cloud* cl : {&c->tmp, &c->state}) {
+        release(cl->lay); release(cl->xyzw); release(cl->perm); release(cl->G); release(cl->rec);
+    }
+    for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
+                   &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab})
+        release(*b);
+    delete c;
+}
+
+int landau_get_quadrature(const landau_ctx* c, double* knots, double* weights) {
+    if (!c || !knots || !weights) return LANDAU_EINVAL;
+    for (int i = 0; i < c->n_q; ++i) { knots[i] = c->knot[i]; weights[i] = c->gw[i]; }
+    return 0;
+}
+
+int landau_entropy_grad(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid, double* G_out,
+                        double* S_eps_out) {
+    if (!c) return LANDAU_EINVAL;
+    if (!G_out) return fail(c, LANDAU_EINVAL, "entropy_grad: NULL output");
+    Cloud& cl = c->tmp;
+    RC(pack(c, cl, N, v, w, sid));
+    RC(entropy(c, cl));
+    scatter3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), cl.Gx(), cl.Gy(),
+                                                                       cl.Gz(), G_out);
+    c->launches += 1;
+    if (S_eps_out) {
+        double* h = (double*)c->h_pin + 64;
+        RC(species_sums(c, cl, true, false, h));
+        const double PI = 3.14159265358979323846;
+        for (int s = 0; s < c->S; ++s) S_eps_out[s] = -h[s * MOM_OUT + 11] / (PI * sqrt(PI));
+    }
+    return finish(c, cl, "entropy_grad");
+}
+
+int landau_pair_field(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid,
+                      const double* G_in, double* out) {
+    if (!c) return LANDAU_EINVAL;
+    if (!G_in || !out) return fail(c, LANDAU_EINVAL, "pair_field: NULL array");
+    Cloud& cl = c->tmp;
+    RC(pack(c, cl, N, v, w, sid));
+    gather3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), G_in, cl.Gx(),
+                                                                      cl.Gy(), cl.Gz());
+    c->launches += 1;
+    c->kernels[0] = 0;
+    RC(field_of_cloud(c, cl, out));
+    return finish(c, cl, "pair_field");
+}
+
+int landau_eval_field(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid, double* out) {
+    if (!c) return LANDAU_EINVAL;
+    if (!out) return fail(c, LANDAU_EINVAL, "eval_field: NULL output");
+    Cloud& cl = c->tmp;
+    RC(pack(c, cl, N, v, w, sid));
+    RC(entropy(c, cl));
+    RC(field_of_cloud(c, cl, out));
+    return finish(c, cl, "eval_field");
+}
+
+int landau_eval_field_host(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid,
+                           double* out) {
+    if (!c) return LANDAU_EINVAL;
+    if (!out) return fail(c, LANDAU_EINVAL, "eval_field_host: NULL output");
+    const double *dv, *dw;
+    const int32_t* ds;
+    RC(stage_in(c, N, v, w, sid, &dv, &dw, &ds));
+    RC(ensure(c, c->stage_o, sizeof(double) * 3 * (size_t)N));
+    Cloud& cl = c->tmp;
+    RC(pack(c, cl, N, dv, dw, ds));
+    RC(entropy(c, cl));
+    RC(field_of_cloud(c, cl, (double*)c->stage_o.p));
+    CU(cudaMemcpyAsync(out, c->stage_o.p, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, c->stream));
+    return finish(c, cl, "eval_field_host");
+}
+
+int landau_set_markers(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    cl.N = 0;
+    RC(pack(c, cl, N, v, w, sid));
+    int rc = finish(c, cl, "set_markers");
+    if (rc < 0) cl.N = 0;
+    return rc;
+}
+
+int landau_set_markers_host(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid) {
+    if (!c) return LANDAU_EINVAL;
+    const double *dv, *dw;
+    const int32_t* ds;
+    RC(stage_in(c, N, v, w, sid, &dv, &dw, &ds));
+    return landau_set_markers(c, N, dv, dw, ds);
+}
+
+int landau_get_markers(landau_ctx* c, double* v_out) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "get_markers: no markers held");
+    if (!v_out) return fail(c, LANDAU_EINVAL, "get_markers: NULL output");
+    scatter3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), cl.x(), cl.y(),
+                                                                       cl.z(), v_out);
+    c->launches += 1;
+    return finish(c, cl, "get_markers");
+}
+
+int landau_get_markers_host(landau_ctx* c, double* v_out) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "get_markers: no markers held");
+    if (!v_out) return fail(c, LANDAU_EINVAL, "get_markers: NULL output");
+    RC(ensure(c, c->stage_o, sizeof(double) * 3 * (size_t)cl.N));
+    scatter3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), cl.x(), cl.y(),
+                                                                       cl.z(), (double*)c->stage_o.p);
+    c->launches += 1;
+    CU(cudaMemcpyAsync(v_out, c->stage_o.p, sizeof(double) * 3 * (size_t)cl.N, cudaMemcpyDeviceToHost, c->stream));
+    return finish(c, cl, "get_markers_host");
+}
+
+int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, landau_step_info* info) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step: no markers held (landau_set_markers first)");
+    if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
+        return fail(c, LANDAU_EINVAL, "step: need n_steps >= 1, max_iter >= 1, dt > 0, tol >= 0");
+    const int npm = cl.npad_max;
+    RC(ensure(c, c->vk, sizeof(double) * 3 * (size_t)npm));
+    RC(ensure(c, c->records, sizeof(StepRecord) * (size_t)n_steps));
+    const int nub = ceil_div(npm, UPD_THREADS);
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(2 * nub, 4096)));
+    double* xk = (double*)c->vk.p;
+    double* yk = xk + npm;
+    double* zk = yk + npm;
+    cudaStream_t st = c->stream;
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
+    CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
+    for (int n = 0; n < n_steps; ++n) {
+        RC(entropy(c, cl));
+        step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
+                                                               cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
+                                                               cl.recs());
+        c->launches += 1;
+        for (int k = 0; k < max_iter; ++k) {
+            int nparts = 0;
+            RC(pair(c, cl, c->d_ctrl, &nparts));
+            step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
+                                                             (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
+                                                             cl.w(), xk, yk, zk, cl.recs(), (double*)c->blockpart.p);
+            c->launches += 1;
+        }
+        step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,
+                                                                zk, (StepRecord*)c->records.p, c->d_cursor);
+        c->launches += 1;
+    }
+    CU(cudaGetLastError());
+    // one synchronisation: records + error flags
+    std::vector<StepRecord> h(n_steps);
+    StepCtrl* hc = (StepCtrl*)c->h_pin;
+    CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(h.data(), c->records.p, sizeof(StepRecord) * (size_t)n_steps, cudaMemcpyDeviceToHost, st));
+    int rc = finish(c, cl, "step");
+    if (rc < 0) return rc;
+    if (hc->err) return fail(c, hc->err, "step: non-finite residual");
+    int any_unconverged = 0;
+    for (int n = 0; n < n_steps; ++n) {
+        if (info) { info[n].iterations = h[n].iterations; info[n].residual = h[n].residual; info[n].converged = h[n].converged; }
+        if (!h[n].converged) any_unconverged = 1;
+    }
+    return any_unconverged ? LANDAU_NOT_CONVERGED : LANDAU_OK;
+}
+
+int landau_step(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {
+    return landau_run(c, 1, dt, tol, max_iter, info);
+}
+
+int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "moments: no markers held");
+    if (S_eps) RC(entropy(c, cl));
+    double* h = (double*)c->h_pin + 64;
+    RC(species_sums(c, cl, S_eps != nullptr, false, h));
+    const double PI = 3.14159265358979323846;
+    for (int s = 0; s < c->S; ++s) {
+        const double* r = h + s * MOM_OUT;
+        if (n) n[s] = r[0];
+        if (P) { P[3 * s] = c->mass[s] * r[1]; P[3 * s + 1] = c->mass[s] * r[2]; P[3 * s + 2] = c->mass[s] * r[3]; }
+        if (K) K[s] = 0.5 * c->mass[s] * r[4];
+        if (S_eps) S_eps[s] = -r[11] / (PI * sqrt(PI));
+    }
+    return finish(c, cl, "moments");
+}
+
+int landau_moments_ext(landau_ctx* c, double* stress, double* m4) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "moments_ext: no markers held");
+    double* h = (double*)c->h_pin + 64;
+    RC(species_sums(c, cl, false, m4 != nullptr, h));
+    for (int s = 0; s < c->S; ++s) {
+        const double* r = h + s * MOM_OUT;
+        if (stress) for (int i = 0; i < 6; ++i) stress[6 * s + i] = c->mass[s] * r[5 + i];
+        if (m4) for (int i = 0; i < 3; ++i) m4[3 * s + i] = r[12 + i];
+    }
+    return finish(c, cl, "moments_ext");
+}
+
+int landau_fp64_peak(landau_ctx* c, int reps, double* flops_out) {
+    if (!c || !flops_out || reps < 1) return LANDAU_EINVAL;
+    RC(ensure(c, c->V, 1024));
+    const int blocks = c->sm_count * 4, threads = 256, iters = 4096;
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int r = 0; r < reps + 1; ++r) {
+        CU(cudaEventRecord(e0, c->stream));
+        fp64_peak_kernel<<<blocks, threads, 0, c->stream>>>((double*)c->V.p, iters, 0.999999, 1e-9);
+        CU(cudaEventRecord(e1, c->stream));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        const double fl = 2.0 * 8.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3);
+        if (r > 0 && fl > best) best = fl;
+    }
+    c->launches += reps + 1;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *flops_out = best;
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,289 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C ABI vs the CPU oracle, element by element
+on the same seeded inputs (paper_2212_00663_b200.workloads).
+
+Tolerances: field and entropy gradient <= 1e-10 relative L2 over markers,
+overall and per species (north_star); per-step relative drift of momentum and energy <= 1e-12;
+bucketing/permutation work is exact.
+"""
+import numpy as np
+import pytest
+
+from paper_2212_00663_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-10
+TOL_DRIFT = 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the CUDA path has no fallback")
+    from paper_2212_00663_b200 import binding
+    binding.load()
+    return binding
+
+
+def make_pair(B, oracle_mod, wl, **kw):
+    n_q = kw.pop("n_q", wl.n_q)
+    nu = kw.pop("nu", None)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=n_q, nu0=wl.nu0, nu=nu, **kw)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=n_q, nu0=wl.nu0, nu=nu)
+    return g, o
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def assert_field_close(got, ref, sid, S, tol=TOL_FIELD, what="field"):
+    assert np.all(np.isfinite(got))
+    assert rel_l2(got, ref) <= tol, f"{what}: rel L2 {rel_l2(got, ref):.3e}"
+    for s in range(S):
+        m = sid == s
+        if m.any() and np.linalg.norm(ref[m]) > 0:
+            assert rel_l2(got[m], ref[m]) <= tol, f"{what} species {s}: rel L2 {rel_l2(got[m], ref[m]):.3e}"
+
+
+KERNEL_VARIANTS = [dict(pair_kernel=1, entropy_kernel=1), dict(pair_kernel=0, entropy_kernel=0)]
+
+
+# ------------------------------------------------------------------------------------ quadrature
+@pytest.mark.parametrize("n_q", [2, 3, 4, 5, 6, 7, 8])
+def test_quadrature_table_matches_oracle(B, oracle_mod, n_q):
+    g = B.Landau([1.0], [1.0], [0.1], n_q=n_q)
+    k, a = g.quadrature()
+    ko, ao = oracle_mod.gauss_hermite(n_q)
+    np.testing.assert_allclose(k, ko, rtol=0, atol=4e-16 * max(1.0, np.abs(ko).max()))
+    np.testing.assert_allclose(a, ao, rtol=4e-15, atol=0)
+
+
+# ------------------------------------------------------------------------------------ pass 2
+@pytest.mark.parametrize("variant", KERNEL_VARIANTS)
+@pytest.mark.parametrize("cfg,n,shuffled", [(0, 256, False), (0, 256, True), (0, 173, True), (4, 300, True),
+                                            (1, 1100, True)])
+def test_pair_field_matches_oracle(B, oracle_mod, variant, cfg, n, shuffled):
+    wl = W.make(cfg, n_per_species=n, shuffled=shuffled)
+    g, o = make_pair(B, oracle_mod, wl, **variant)
+    rng = np.random.default_rng(100 + cfg)
+    G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+    ref = o.pair_field(wl.v, wl.w, wl.species_id, G)
+    got = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    assert_field_close(got, ref, wl.species_id, wl.n_species)
+
+
+# ------------------------------------------------------------------------------------ pass 1
+@pytest.mark.parametrize("variant", KERNEL_VARIANTS)
+@pytest.mark.parametrize("cfg,n,n_q", [(0, 256, 4), (0, 97, 4), (4, 200, 4), (0, 64, 2), (0, 64, 3), (0, 48, 5),
+                                       (0, 40, 6), (0, 33, 8), (3, 300, 4)])
+def test_entropy_grad_matches_oracle(B, oracle_mod, variant, cfg, n, n_q):
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl, n_q=n_q, **variant)
+    Gref, Sref = o.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    Ggot, Sgot = g.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    assert_field_close(Ggot.cpu().numpy(), Gref, wl.species_id, wl.n_species, what="entropy gradient")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------ full field
+@pytest.mark.parametrize("variant", KERNEL_VARIANTS)
+@pytest.mark.parametrize("cfg,n", [(0, 256), (2, 500), (4, 384)])
+def test_eval_field_matches_oracle(B, oracle_mod, variant, cfg, n):
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl, **variant)
+    ref = o.eval_field(wl.v, wl.w, wl.species_id)
+    got = g.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(got, ref, wl.species_id, wl.n_species)
+    got_h = g.eval_field_host(wl.v, wl.w, wl.species_id)
+    np.testing.assert_array_equal(got_h, got)     # same kernels, same order: bit-identical
+
+
+def test_nu_override_matrix(B, oracle_mod):
+    wl = W.make(4, n_per_species=150, shuffled=True)
+    rng = np.random.default_rng(5)
+    a = rng.uniform(0.5, 2.0, (3, 3))
+    nu = a + a.T
+    g, o = make_pair(B, oracle_mod, wl, nu=nu)
+    ref = o.eval_field(wl.v, wl.w, wl.species_id)
+    got = g.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(got, ref, wl.species_id, 3)
+
+
+# ------------------------------------------------------------------------------------ invariants
+def test_field_conservation_identities_on_gpu(B):
+    """Eq. 27 / 29 hold for the GPU field with an arbitrary G."""
+    wl = W.make(4, n_per_species=700, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps)
+    rng = np.random.default_rng(7)
+    G = rng.standard_normal((wl.n_markers, 3))
+    V = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    scaleP = np.abs(wm * V).sum()
+    assert np.abs((wm * V).sum(axis=0)).max() <= 1e-13 * scaleP
+    assert abs((wm * wl.v * V).sum()) <= 1e-13 * np.abs(wm * wl.v * V).sum()
+
+
+def test_coincident_and_single_marker(B, oracle_mod):
+    mass, charge, eps = [1.0, 4.0], [-1.0, 2.0], [0.05, 0.02]
+    g = B.Landau(mass, charge, eps)
+    o = oracle_mod.LandauRef(mass, charge, eps)
+    v = np.array([[0.1, 0.2, 0.3], [0.1, 0.2, 0.3], [0.5, -0.2, 0.0], [0.1, 0.2, 0.3]])
+    w = np.array([1.0, 2.0, 0.5, 0.7])
+    sid = np.array([0, 1, 0, 0], dtype=np.int32)
+    ref = o.eval_field(v, w, sid)
+    got = g.eval_field(v, w, sid).cpu().numpy()
+    np.testing.assert_allclose(got, ref, rtol=1e-10, atol=1e-14 * np.abs(ref).max())
+    one = g.eval_field(v[:1], w[:1], sid[:1]).cpu().numpy()
+    np.testing.assert_array_equal(one, np.zeros((1, 3)))
+    G1, S1 = g.entropy_grad(v[:1], w[:1], sid[:1], with_entropy=True)
+    np.testing.assert_allclose(G1.cpu().numpy(), 0.0, atol=1e-13)
+    _, S1o = o.entropy_grad(v[:1], w[:1], sid[:1], with_entropy=True)
+    np.testing.assert_allclose(S1, S1o, rtol=1e-12, atol=1e-13)
+
+
+def test_species_with_no_markers(B, oracle_mod):
+    wl = W.random_cloud([200, 0, 77], [1.0, 10.0, 100.0], [-1.0, 1.0, 2.0], [1.0, 1.0, 2.0], seed=3)
+    g, o = make_pair(B, oracle_mod, wl)
+    ref = o.eval_field(wl.v, wl.w, wl.species_id)
+    got = g.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(got, ref, wl.species_id, 3)
+
+
+def test_sixteen_species_ragged(B, oracle_mod):
+    S = 16
+    rng = np.random.default_rng(11)
+    counts = rng.integers(1, 90, S)
+    wl = W.random_cloud(counts, 10 ** rng.uniform(0, 4, S), rng.choice([-1.0, 1.0, 2.0], S),
+                        rng.uniform(0.5, 2.0, S), seed=12)
+    g, o = make_pair(B, oracle_mod, wl)
+    ref = o.eval_field(wl.v, wl.w, wl.species_id)
+    got = g.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(got, ref, wl.species_id, S)
+
+
+# ------------------------------------------------------------------------------------ errors
+def test_argument_errors(B):
+    import torch
+    g = B.Landau([1.0, 2.0], [1.0, -1.0], [0.1, 0.1])
+    v = np.zeros((4, 3)); v[:, 0] = np.arange(4)
+    w = np.ones(4)
+    sid = np.array([0, 1, 0, 1], dtype=np.int32)
+    bad = sid.copy(); bad[2] = 2
+    with pytest.raises(B.LandauError) as e:
+        g.eval_field(v, w, bad)
+    assert e.value.code == B.EINVAL
+    wz = w.copy(); wz[1] = 0.0
+    with pytest.raises(B.LandauError) as e:
+        g.eval_field(v, wz, sid)
+    assert e.value.code == B.EINVAL
+    vn = v.copy(); vn[3, 1] = np.nan
+    with pytest.raises(B.LandauError) as e:
+        g.eval_field(v=vn, w=w, sid=sid)
+    assert e.value.code == B.ENONFINITE
+    with pytest.raises(B.LandauError):
+        g.step(0.01)                      # no markers held
+    g.set_markers(v, w, sid)
+    with pytest.raises(B.LandauError):
+        g.step(-1.0)
+    with pytest.raises(B.LandauError):
+        B.Landau([1.0], [1.0], [-0.1])
+    with pytest.raises(B.LandauError):
+        B.Landau([1.0, 1.0], [1.0, 1.0], [0.1, 0.1], nu=np.array([[1.0, 2.0], [3.0, 1.0]]))
+    with pytest.raises(B.LandauError):
+        B.Landau([1.0], [1.0], [0.1], n_q=9)
+    assert torch.cuda.is_available()
+
+
+# ------------------------------------------------------------------------------------ step
+def totals(wl, v):
+    wm = wl.w * wl.mass[wl.species_id]
+    return (wm[:, None] * v).sum(axis=0), 0.5 * (wm * (v ** 2).sum(axis=1)).sum(), (wm[:, None] * np.abs(v)).sum()
+
+
+@pytest.mark.parametrize("variant", KERNEL_VARIANTS)
+def test_config0_step_matches_oracle_and_conserves(B, oracle_mod, variant):
+    wl = W.make(0, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl, **variant)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    rc_g, it_g, res_g, conv_g = g.step(wl.dt, wl.tol, wl.max_iter)
+    rc_o, it_o, res_o, conv_o = o.step(wl.dt, wl.tol, wl.max_iter)
+    assert (rc_g, conv_g) == (rc_o, conv_o) == (0, True)
+    assert abs(it_g - it_o) <= 1 and 5 <= it_g <= 10
+    vg, vo = g.get_markers().cpu().numpy(), o.get_markers()
+    # unique fixed point: both sides converge to it within ~tol (reading N4)
+    dv = vg - wl.v
+    assert rel_l2(vg - wl.v, vo - wl.v) <= 1e-8
+    assert rel_l2(vg, vo) <= 1e-11
+    P0, K0, Pabs = totals(wl, wl.v)
+    P1, K1, _ = totals(wl, vg)
+    assert np.abs(P1 - P0).max() <= TOL_DRIFT * Pabs
+    assert abs(K1 - K0) <= TOL_DRIFT * K0
+    assert np.abs(dv).max() > 0
+
+
+def test_momentum_conserved_when_not_converged(B, oracle_mod):
+    """momentum is conserved by every iterate; energy only at convergence."""
+    wl = W.make(0, n_per_species=200, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = g.step(wl.dt, 1e-14, 2)
+    rco, ito, reso, convo = o.step(wl.dt, 1e-14, 2)
+    assert (rc, it, conv) == (1, 2, False) == (rco, ito, convo)
+    assert abs(res - reso) <= 1e-6 * reso
+    vg, vo = g.get_markers().cpu().numpy(), o.get_markers()
+    assert rel_l2(vg - wl.v, vo - wl.v) <= 1e-10          # same iterate count, Jacobi both sides (N4)
+    P0, K0, Pabs = totals(wl, wl.v)
+    P1, K1, _ = totals(wl, vg)
+    assert np.abs(P1 - P0).max() <= TOL_DRIFT * Pabs
+    assert abs(K1 - K0) > 1e-10 * K0
+
+
+def test_multi_step_history_matches_oracle(B, oracle_mod):
+    """Multi-step runs are compared by their moment histories (north_star)."""
+    wl = W.make(1, n_per_species=300, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    rc, infos = g.run(5, wl.dt, wl.tol, wl.max_iter)
+    assert rc == 0 and all(c for _, _, c in infos)
+    for _ in range(5):
+        o.step(wl.dt, wl.tol, wl.max_iter)
+    mg, mo = g.moments(), o.moments()
+    np.testing.assert_allclose(mg["n"], mo["n"], rtol=1e-13)
+    np.testing.assert_allclose(mg["K"], mo["K"], rtol=1e-10)
+    np.testing.assert_allclose(mg["S_eps"], mo["S_eps"], rtol=1e-10, atol=1e-10)
+    np.testing.assert_allclose(mg["P"], mo["P"], rtol=0, atol=1e-10 * np.abs(mo["P"]).max() + 1e-13)
+    sg, m4g = g.moments_ext()
+    so, m4o = o.moments_ext()
+    np.testing.assert_allclose(sg, so, rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(m4g, m4o, rtol=1e-9)
+    # five single steps == one run of five (device loop is the same code)
+    g2 = B.Landau(wl.mass, wl.charge, wl.eps)
+    g2.set_markers_host(wl.v, wl.w, wl.species_id)
+    for _ in range(5):
+        g2.step(wl.dt, wl.tol, wl.max_iter)
+    np.testing.assert_array_equal(g2.get_markers_host(), g.get_markers().cpu().numpy())
+
+
+def test_moments_match_oracle(B, oracle_mod):
+    wl = W.make(4, n_per_species=1000, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    mg, mo = g.moments(), o.moments()
+    for k in ("n", "K", "S_eps"):
+        np.testing.assert_allclose(mg[k], mo[k], rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(mg["P"], mo["P"], rtol=0, atol=1e-13 * np.abs(wl.w * wl.mass[wl.species_id]).sum())
+
+
+def test_eval_field_does_not_touch_held_markers(B):
+    wl = W.make(0, n_per_species=100)
+    g = B.Landau(wl.mass, wl.charge, wl.eps)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    other = W.make(0, n_per_species=333, seed=9, shuffled=True)
+    g.eval_field(other.v, other.w, other.species_id)
+    np.testing.assert_array_equal(g.get_markers().cpu().numpy(), wl.v)
