@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arXiv:2212.00663 on B200 (contract: DESIGN.md "Measurement").
+
+A "step" is one pass of the WHOLE hot path over one synthetic marker
+cloud: pack/bucket (landau_set_markers), pass 1 (entropy gradient), the implicit step of Eq. (24) with
+pass 2 once per fixed-point iteration, update/residual, diagnostics (landau_moments incl. S_eps, which
+costs a second pass 1) and the read-back of the new velocities (landau_get_markers).
+
+    python bench.py --gpus 1 --steps 5 --warmup 3                  # the CUDA path
+    python bench.py --impl reference --steps 2 --warmup 1          # the CPU oracle, bounded sample
+
+metric  = pair interactions per second (FP64): ordered (target, source) evaluations of Eq. (23) done by
+          the fixed-point iterations of the timed steps, divided by the time of the whole steps.
+e2e     = the same, through the *_host entry points: host->device copies of (v, w, species_id) and the
+          device->host read of the new velocities inside the timed region, every step.
+N > 1   : the path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent
+          replicas ("replicas only"), value = pairs of all replicas / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2212_00663_b200 import workloads as W  # noqa: E402
+
+METRIC = "pair_interactions_per_s"
+UNIT = "pairs/s"
+FLOPS_PER_PAIR = 33.0          # canonical algorithmic count of one ordered pair
+# nominal FP64 vector peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9
+
+WORKLOADS = {
+    # name: (config index, markers per species)
+    "c4_2e16": (4, 1 << 16),
+    "c4_2e15": (4, 1 << 15),
+    "c4_2e14": (4, 1 << 14),
+    "c4_2e17": (4, 1 << 17),
+    "c1": (1, 4096),
+    "c0": (0, 256),
+    "c2": (2, 8192),
+    "c3": (3, 32768),
+}
+DEFAULT_WORKLOAD = "c4_2e16"     # >= 1e5 markers: the size north_star's roofline target is quoted on
+# fixed-point iterations one step of each workload takes (measured on the GPU path, used only to
+# scale the oracle's bounded sample in --impl reference, which must not touch the GPU)
+REF_ITERS = {"c0": 9, "c1": 13, "c2": 10, "c3": 6, "c4_2e14": 9, "c4_2e15": 12, "c4_2e16": 16, "c4_2e17": 20}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the oracle sample")
+    ap.add_argument("--pair-kernel", type=int, default=0)
+    ap.add_argument("--entropy-kernel", type=int, default=0)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(wl, iters, seconds, name):
+    """The oracle, as it stands, on a bounded sample: a random subset of target rows of pass 1 and
+    pass 2 against all sources.  Returns (pairs/s extrapolated to the whole path, dict)."""
+    from oracle import landau_ref
+    landau_ref.build()
+    o = landau_ref.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    N = wl.n_markers
+    rng = np.random.default_rng(12345)
+    G = rng.standard_normal((N, 3))
+    # calibrate on a few rows, then size the sample for ~`seconds`
+    rows = rng.choice(N, size=min(N, 16), replace=False).astype(np.int64)
+    t0 = time.perf_counter(); o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows); tp = (time.perf_counter() - t0) / len(rows)
+    t0 = time.perf_counter(); o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows[:8]); te = (time.perf_counter() - t0) / 8
+    per_row = te + iters * tp
+    m = int(max(8, min(N, seconds / max(per_row, 1e-9))))
+    rows = rng.choice(N, size=m, replace=False).astype(np.int64)
+    t0 = time.perf_counter()
+    o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows)
+    t_e = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    for _ in range(iters):
+        o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows)
+    t_p = time.perf_counter() - t0
+    pairs = float(iters) * m * (N - 1)
+    value = pairs / (t_e + t_p)
+    info = {"value": value, "unit": UNIT, "cores": landau_ref.num_threads(), "kind": "oracle",
+            "sample": f"{name}: {m} of {N} target rows against all sources; pass 1 once ({t_e:.2f} s) + pass 2 x {iters} "
+                      f"iterations ({t_p:.2f} s); pairs = iterations*rows*(N-1); pass-2-only rate "
+                      f"{pairs / t_p:.3e} pairs/s"}
+    return value, info, (t_e + t_p)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, nps = WORKLOADS[args.workload]
+    wl = W.make(cfg, n_per_species=nps)
+    iters = REF_ITERS[args.workload]
+    per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(wl, iters, per_step, args.workload)
+    vals, infos, times = [], [], []
+    for _ in range(args.steps):
+        v, info, t = oracle_sample(wl, iters, per_step, args.workload)
+        vals.append(v); infos.append(info); times.append(t)
+    value = float(np.mean(vals))
+    info = dict(infos[-1]); info["value"] = value
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": config_dict(args, wl, iters), "cpu_baseline": info,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(args, wl, iters=None):
+    d = {"workload": f"{args.workload}: {wl.name}, {wl.n_species} species x {int(wl.counts()[0])} markers "
+                     f"(N = {wl.n_markers}), FP64, n_q = {wl.n_q}, dt = {wl.dt}, tol = {wl.tol}, max_iter = {wl.max_iter}",
+         "n_markers": wl.n_markers, "n_species": wl.n_species,
+         "step": "set_markers + landau_step (pass 1, fixed-point iterations of pass 2) + moments(S_eps) + get_markers",
+         "l2": "inputs re-packed every step; pass-2 working set is L2-resident by design (56 B/marker); "
+               "compute-bound path, cache state does not change the timing",
+         "parallelism": "replicas only" if args.gpus > 1 else "single GPU"}
+    if iters is not None:
+        d["iterations_per_step"] = iters
+    return d
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2212_00663_b200 import binding as B
+
+    cfg, nps = WORKLOADS[args.workload]
+    wl = W.make(cfg, n_per_species=nps, seed=cfg + 1000 * rank)       # replicas differ by seed
+    N = wl.n_markers
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, pair_kernel=args.pair_kernel,
+                 entropy_kernel=args.entropy_kernel)
+    dev = torch.device("cuda", local)
+    v_d = torch.tensor(wl.v, device=dev); w_d = torch.tensor(wl.w, device=dev)
+    s_d = torch.tensor(wl.species_id, device=dev)
+    v_h = torch.from_numpy(wl.v).pin_memory(); w_h = torch.from_numpy(wl.w).pin_memory()
+    s_h = torch.from_numpy(wl.species_id).pin_memory()
+    out_h = torch.empty((N, 3), dtype=torch.float64).pin_memory()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device():
+        g.set_markers(v_d, w_d, s_d)
+        rc, it, res, conv = g.step(wl.dt, wl.tol, wl.max_iter)
+        m = g.moments(with_entropy=True)
+        vnew = g.get_markers()
+        return it, conv, m, vnew
+
+    lib, h = g._lib, g._h
+
+    def step_host():
+        rc = lib.landau_set_markers_host(h, N, v_h.data_ptr(), w_h.data_ptr(), s_h.data_ptr())
+        assert rc == 0, rc
+        g.N = N
+        rc, it, res, conv = g.step(wl.dt, wl.tol, wl.max_iter)
+        m = g.moments(with_entropy=True)
+        rc = lib.landau_get_markers_host(h, out_h.data_ptr())
+        assert rc == 0, rc
+        return it, conv, m
+
+    g.set_markers(v_d, w_d, s_d)
+    m0 = g.moments(with_entropy=False)          # invariants of the initial cloud
+    for _ in range(max(args.warmup, 1)):
+        step_device()
+    # ---- device-resident timed region
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    g.profile_enable(True)
+    l0 = g.launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    iters_total, all_conv = 0, True
+    e0.record()
+    for _ in range(args.steps):
+        it, conv, m1, vnew = step_device()
+        iters_total += it; all_conv &= bool(conv)
+    e1.record()
+    barrier()
+    t_dev = e0.elapsed_time(e1) * 1e-3
+    prof = g.profile_read()
+    g.profile_enable(False)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop()
+    # ---- end-to-end timed region (host buffers)
+    step_host()
+    barrier()
+    e0.record()
+    it_h = 0
+    for _ in range(args.steps):
+        it, conv, _m = step_host()
+        it_h += it
+    e1.record()
+    barrier()
+    t_e2e = e0.elapsed_time(e1) * 1e-3
+
+    times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+    pairs = torch.tensor([float(iters_total) * N * (N - 1), float(it_h) * N * (N - 1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(pairs, op=dist.ReduceOp.SUM)
+    t_dev_max, t_e2e_max = times.tolist()
+    pairs_dev, pairs_e2e = pairs.tolist()
+
+    if rank == 0:
+        value = pairs_dev / t_dev_max
+        # roofline of the dominant kernel (pass 2), timed live with CUDA events on the context's stream
+        pair_s = prof["pair_ms"] * 1e-3 / max(prof["pair_launches"], 1)
+        achieved = FLOPS_PER_PAIR * N * (N - 1) / pair_s / 1e12
+        peak_meas = g.fp64_peak(5) / 1e12
+        roofline = {"bound": "alu", "kernel": g.last_kernels(), "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12,
+                    "unit": "TFLOP/s", "frac": achieved / (FP64_PEAK_NOMINAL / 1e12), "traffic": None,
+                    "peak_source": "nominal FP64 FMA rate 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md); "
+                                   "MEASURED_PEAKS.json has no FP64 figure",
+                    "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
+                    "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": float(N) * (N - 1),
+                    "avg_launch_ms": pair_s * 1e3, "launches_timed": prof["pair_launches"],
+                    "pair_kernel_pairs_per_s": N * (N - 1) / pair_s,
+                    "pair_share_of_step": prof["pair_ms"] * 1e-3 / t_dev,
+                    "entropy_kernel_ms": prof["entropy_ms"] / max(prof["entropy_launches"], 1),
+                    "entropy_same_species_pairs_per_s": float((wl.counts().astype(float) ** 2).sum()) /
+                                                        (prof["entropy_ms"] * 1e-3 / max(prof["entropy_launches"], 1)),
+                    "entropy_share_of_step": prof["entropy_ms"] * 1e-3 / t_dev}
+        h2d = int(v_h.numel() * 8 + w_h.numel() * 8 + s_h.numel() * 4)
+        d2h = int(out_h.numel() * 8 + 4 * 8 * wl.n_species)
+        K0 = float(m0["K"].sum()); K1 = float(m1["K"].sum())
+        wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
+        dP = float(np.abs(m1["P"].sum(axis=0) - m0["P"].sum(axis=0)).max()) / wm_abs
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 1), "ms_per_step": 1e3 * t_dev_max / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": config_dict(args, wl, iters_total / args.steps),
+                "steps_per_s": args.steps * world / t_dev_max, "all_converged": bool(all_conv),
+                "energy_drift_rel": abs(K1 - K0) / K0, "momentum_drift_rel": dP,
+                "e2e": {"value": pairs_e2e / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                        "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e_max / args.steps},
+                "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        if not args.no_cpu_baseline and world == 1:
+            _, info, _ = oracle_sample(wl, max(1, round(iters_total / args.steps)), args.cpu_seconds, args.workload)
+            line["cpu_baseline"] = info
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -139,6 +139,15 @@ const char* landau_last_kernels(const landau_ctx* ctx);
 /* Number of kernel launches issued by this context so far. */
 int64_t landau_launch_count(const landau_ctx* ctx);
 
+/* Per-kernel timing for bench.py's roofline: when enabled, CUDA events are recorded on the
+ * context's stream around every launch of the two all-pairs kernels (pass 2 "pair", pass 1
+ * "entropy"); launches of fixed-point iterations that exited at once because the step had already
+ * converged are not counted.  landau_profile_enable(ctx, on) also clears the sums.  Times are
+ * accumulated when a call synchronises; read them after the call returns (HOST outputs). */
+int landau_profile_enable(landau_ctx* ctx, int on);
+int landau_profile_read(landau_ctx* ctx, double* pair_ms, int64_t* pair_launches, double* entropy_ms,
+                        int64_t* entropy_launches);
+
 /* FP64 ALU peak microbenchmark (dependent-free DFMA streams on every SM): runs `reps` launches and
  * returns the best rate in FLOP/s (2 per DFMA) through *flops_out (HOST). Used by bench.py for the
  * roofline denominator. */

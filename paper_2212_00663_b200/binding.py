@@ -26,7 +26,8 @@ SYMBOLS = [
     "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
     "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
-    "landau_last_kernels", "landau_launch_count", "landau_fp64_peak", "landau_last_error",
+    "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
+    "landau_fp64_peak", "landau_last_error",
     "landau_version",
 ]
 
@@ -86,6 +87,8 @@ def load(build_if_missing: bool = True):
     lib.landau_last_kernels.restype = C.c_char_p
     lib.landau_launch_count.argtypes = [vp]
     lib.landau_launch_count.restype = C.c_int64
+    lib.landau_profile_enable.argtypes = [vp, C.c_int]
+    lib.landau_profile_read.argtypes = [vp, hd, C.POINTER(C.c_int64), hd, C.POINTER(C.c_int64)]
     lib.landau_fp64_peak.argtypes = [vp, C.c_int, hd]
     lib.landau_last_error.argtypes = [vp]
     lib.landau_last_error.restype = C.c_char_p
@@ -249,6 +252,17 @@ class Landau:
         stress, m4 = np.empty((self.S, 6)), np.empty((self.S, 3))
         self._check(self._lib.landau_moments_ext(self._h, _hd(stress), _hd(m4)), "landau_moments_ext")
         return stress, m4
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.landau_profile_enable(self._h, int(bool(on))), "landau_profile_enable")
+
+    def profile_read(self):
+        """dict(pair_ms, pair_launches, entropy_ms, entropy_launches) since profile_enable."""
+        pm, em = C.c_double(0.0), C.c_double(0.0)
+        pn, en = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.landau_profile_read(self._h, C.byref(pm), C.byref(pn), C.byref(em), C.byref(en)),
+                    "landau_profile_read")
+        return dict(pair_ms=pm.value, pair_launches=pn.value, entropy_ms=em.value, entropy_launches=en.value)
 
     def fp64_peak(self, reps: int = 5) -> float:
         out = C.c_double(0.0)

@@ -72,6 +72,15 @@ struct landau_ctx {
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
     int64_t launches = 0;
+    // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
+    bool prof_on = false;
+    bool in_run = false;
+    struct ProfEv { cudaEvent_t e0, e1; int kind; int step; int iter; };
+    std::vector<ProfEv> prof_events;
+    std::vector<cudaEvent_t> prof_pool;
+    int prof_step = 0, prof_iter = 0;
+    double prof_ms[2] = {0.0, 0.0};
+    int64_t prof_n[2] = {0, 0};
     char err[512];
     char kernels[128];
 };
@@ -117,6 +126,45 @@ int ensure(landau_ctx* c, Buf& b, size_t bytes) {
 void release(Buf& b) {
     if (b.p) cudaFree(b.p);
     b.p = nullptr; b.cap = 0;
+}
+
+cudaEvent_t prof_get_event(landau_ctx* c) {
+    cudaEvent_t e = nullptr;
+    if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+
+// kind 0 = pairwise kernel (pass 2), 1 = entropy node-sum kernel (pass 1)
+struct ProfScope {
+    landau_ctx* c; int kind; cudaEvent_t e0 = nullptr;
+    ProfScope(landau_ctx* c_, int kind_) : c(c_), kind(kind_) {
+        if (c->prof_on) { e0 = prof_get_event(c); cudaEventRecord(e0, c->stream); }
+    }
+    ~ProfScope() {
+        if (!e0) return;
+        cudaEvent_t e1 = prof_get_event(c);
+        cudaEventRecord(e1, c->stream);
+        c->prof_events.push_back({e0, e1, kind, c->prof_step, c->prof_iter});
+    }
+};
+
+// Resolve recorded events after a synchronisation.  iters_per_step (may be NULL) gives, for step
+// records of the call just finished, how many fixed-point iterations really ran: pair launches
+// beyond that exited at once and are not counted.
+void prof_resolve(landau_ctx* c, const int* iters_per_step, int n_steps) {
+    for (auto& ev : c->prof_events) {
+        float ms = 0.f;
+        bool count = true;
+        if (ev.kind == 0 && iters_per_step && ev.step < n_steps && ev.iter >= iters_per_step[ev.step]) count = false;
+        if (count && cudaEventElapsedTime(&ms, ev.e0, ev.e1) == cudaSuccess) {
+            c->prof_ms[ev.kind] += ms;
+            c->prof_n[ev.kind] += 1;
+        }
+        c->prof_pool.push_back(ev.e0);
+        c->prof_pool.push_back(ev.e1);
+    }
+    c->prof_events.clear();
 }
 
 // Gauss-Hermite rule for the weight exp(-k^2) by Golub-Welsch: knots are the eigenvalues of the
@@ -240,6 +288,8 @@ int entropy(landau_ctx* c, Cloud& cl) {
     RC(ensure(c, c->part, (size_t)nchunks * M * cl.npad_max * sizeof(double)));
     int use_fact = 0;
     if (c->entropy_kernel == 2 || c->entropy_kernel == 0) use_fact = entropy_fact_available(nq);
+    {
+    ProfScope prof(c, 1);
     if (use_fact) {
         RC(launch_entropy_fact(c, cl, nchunks));
     } else {
@@ -255,6 +305,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
         }
         c->launches += 1;
     }
+    }
     entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
         use_fact, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
@@ -269,6 +320,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
 int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     int use_sym = 0;
     if (c->pair_kernel == 2 || c->pair_kernel == 0) use_sym = pair_sym_available(c, cl);
+    ProfScope prof(c, 0);
     if (use_sym) {
         RC(launch_pair_sym(c, cl, ctrl, nparts_out));
         return 0;
@@ -293,6 +345,7 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     CU(cudaMemcpyAsync(h, &cl.L()->err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
+    if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
     if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
     if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
     if (*h) return fail(c, *h, "%s: device-side error %d", where, *h);
@@ -301,6 +354,7 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
 
 int field_of_cloud(landau_ctx* c, Cloud& cl, double* out) {
     int nparts = 0;
+    c->prof_step = 0; c->prof_iter = 0;
     build_rec_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
                                                                         cl.z(), cl.w(), cl.Gx(), cl.Gy(), cl.Gz(),
                                                                         cl.recs());
@@ -445,6 +499,8 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
 
 void landau_destroy(landau_ctx* c) {
     if (!c) return;
+    for (auto& ev : c->prof_events) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
+    for (auto e : c->prof_pool) cudaEventDestroy(e);
     if (c->d_tab) cudaFree(c->d_tab);
     if (c->d_ctrl) cudaFree(c->d_ctrl);
     if (c->d_cursor) cudaFree(c->d_cursor);
@@ -584,6 +640,7 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
     for (int n = 0; n < n_steps; ++n) {
+        c->prof_step = n; c->prof_iter = 0;
         RC(entropy(c, cl));
         step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
                                                                cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
@@ -591,6 +648,7 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
         c->launches += 1;
         for (int k = 0; k < max_iter; ++k) {
             int nparts = 0;
+            c->prof_iter = k;
             RC(pair(c, cl, c->d_ctrl, &nparts));
             step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                              (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
@@ -607,9 +665,16 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     StepCtrl* hc = (StepCtrl*)c->h_pin;
     CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(h.data(), c->records.p, sizeof(StepRecord) * (size_t)n_steps, cudaMemcpyDeviceToHost, st));
+    c->in_run = true;
     int rc = finish(c, cl, "step");
-    if (rc < 0) return rc;
+    c->in_run = false;
+    if (rc < 0) { if (c->prof_on) prof_resolve(c, nullptr, 0); return rc; }
     if (hc->err) return fail(c, hc->err, "step: non-finite residual");
+    if (c->prof_on) {
+        std::vector<int> its(n_steps);
+        for (int n = 0; n < n_steps; ++n) its[n] = h[n].iterations;
+        prof_resolve(c, its.data(), n_steps);
+    }
     int any_unconverged = 0;
     for (int n = 0; n < n_steps; ++n) {
         if (info) { info[n].iterations = h[n].iterations; info[n].residual = h[n].residual; info[n].converged = h[n].converged; }
@@ -652,6 +717,24 @@ int landau_moments_ext(landau_ctx* c, double* stress, double* m4) {
         if (m4) for (int i = 0; i < 3; ++i) m4[3 * s + i] = r[12 + i];
     }
     return finish(c, cl, "moments_ext");
+}
+
+int landau_profile_enable(landau_ctx* c, int on) {
+    if (!c) return LANDAU_EINVAL;
+    c->prof_on = on != 0;
+    c->prof_ms[0] = c->prof_ms[1] = 0.0;
+    c->prof_n[0] = c->prof_n[1] = 0;
+    return 0;
+}
+
+int landau_profile_read(landau_ctx* c, double* pair_ms, int64_t* pair_launches, double* entropy_ms,
+                        int64_t* entropy_launches) {
+    if (!c) return LANDAU_EINVAL;
+    if (pair_ms) *pair_ms = c->prof_ms[0];
+    if (pair_launches) *pair_launches = c->prof_n[0];
+    if (entropy_ms) *entropy_ms = c->prof_ms[1];
+    if (entropy_launches) *entropy_launches = c->prof_n[1];
+    return 0;
 }
 
 int landau_fp64_peak(landau_ctx* c, int reps, double* flops_out) {
