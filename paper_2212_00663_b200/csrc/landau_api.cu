@@ -18,6 +18,7 @@
 #include "moments.cuh"
 #include "pack.cuh"
 #include "pair.cuh"
+#include "pair_sym.cuh"
 #include "step.cuh"
 
 using namespace landau;
@@ -35,7 +36,8 @@ struct Cloud {
     int64_t N = 0;
     int npad_max = 0;
     int pad = 0;
-    Buf lay, xyzw, perm, G, rec;
+    Buf lay, xyzw, perm, G, rec, soa;
+    int sym = 0;   // 1: the symmetric pair kernel's layout (pad = its target tile) and SoA source copy
     DevLayout* L() const { return (DevLayout*)lay.p; }
     double* x() const { return (double*)xyzw.p; }
     double* y() const { return x() + npad_max; }
@@ -47,6 +49,7 @@ struct Cloud {
     double* Gz() const { return Gx() + 2 * (size_t)npad_max; }
     double* snode() const { return Gx() + 3 * (size_t)npad_max; }
     double* recs() const { return (double*)rec.p; }
+    double* soas() const { return (double*)soa.p; }
 };
 
 }  // namespace
@@ -83,6 +86,8 @@ struct landau_ctx {
     int64_t prof_n[2] = {0, 0};
     char err[512];
     char kernels[128];
+    const char* k_pair = "-";
+    const char* k_entropy = "-";
 };
 
 namespace {
@@ -221,10 +226,19 @@ void gauss_hermite_gw(int n, double* knots, double* weights) {
     if (n & 1) knots[n / 2] = 0.0;
 }
 
-int choose_pad(const landau_ctx* c, int64_t N) {
-    (void)c; (void)N;
-    return 128;
+// The symmetric pair kernel (pair_sym.cuh) in its large configuration: 8 warps, 4 targets per
+// lane, 2 sources per lane and step: target tiles of 1024 slots, source units of 512.
+constexpr int SYM_W = 8, SYM_RT = 4, SYM_RS = 2;
+using SymL = SymCfg<SYM_W, SYM_RT, SYM_RS>;
+constexpr int64_t SYM_MIN_MARKERS = 16384;
+
+int want_sym(const landau_ctx* c, int64_t N) {
+    if (c->pair_kernel == 1 || c->precision == 1) return 0;
+    if (c->pair_kernel == 2) return 1;
+    return N >= SYM_MIN_MARKERS;
 }
+
+int choose_pad(const landau_ctx* c, int64_t N) { return want_sym(c, N) ? SymL::BT : 128; }
 
 int npad_upper(int64_t N, int S, int pad) {
     const int64_t up = N + (int64_t)S * (pad - 1);
@@ -235,8 +249,24 @@ int npad_upper(int64_t N, int S, int pad) {
 // ---- optimised kernels (filled in below when available) -------------------------------------
 int entropy_fact_available(int nq) { (void)nq; return 0; }
 int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) { (void)c; (void)cl; (void)nchunks; return LANDAU_ECUDA; }
-int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; (void)cl; return 0; }
-int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts) { (void)c; (void)cl; (void)ctrl; (void)nparts; return LANDAU_ECUDA; }
+
+int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; return cl.sym; }
+int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts) {
+    const int G = c->sm_count;
+    const size_t n = (size_t)G * 3 * cl.npad_max;
+    RC(ensure(c, c->vpart, sizeof(double) * n));
+    static bool attr_done = false;
+    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS>;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SymL::SMEM));
+        attr_done = true;
+    }
+    zero_slices_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(ctrl, (double2*)c->vpart.p, n / 2);
+    kern<<<G, SymL::THREADS, SymL::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, cl.soas(), (double*)c->vpart.p);
+    c->launches += 2;
+    *nparts = G;
+    return 0;
+}
 
 // ---- a0: pack -----------------------------------------------------------------------------
 int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, const int32_t* sid) {
@@ -246,7 +276,8 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
     const int S = c->S;
     const int pad = choose_pad(c, N);
     const int npm = npad_upper(N, S, pad);
-    cl.N = N; cl.npad_max = npm; cl.pad = pad;
+    cl.N = N; cl.npad_max = npm; cl.pad = pad; cl.sym = want_sym(c, N);
+    if (cl.sym) RC(ensure(c, cl.soa, sizeof(double) * 7 * (size_t)npm));
     RC(ensure(c, cl.lay, sizeof(DevLayout)));
     RC(ensure(c, cl.xyzw, sizeof(double) * 4 * (size_t)npm));
     RC(ensure(c, cl.perm, sizeof(int) * (size_t)npm));
@@ -311,7 +342,8 @@ int entropy(landau_ctx* c, Cloud& cl) {
         use_fact, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
     c->launches += 1;
     CU(cudaGetLastError());
-    snprintf(c->kernels + 0, 32, "entropy=%s", use_fact ? "fact" : "literal");
+    c->k_entropy = use_fact ? "fact" : "literal";
+    snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     return 0;
 }
 
@@ -321,6 +353,8 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     int use_sym = 0;
     if (c->pair_kernel == 2 || c->pair_kernel == 0) use_sym = pair_sym_available(c, cl);
     ProfScope prof(c, 0);
+    c->k_pair = use_sym ? "sym" : "onesided";
+    snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (use_sym) {
         RC(launch_pair_sym(c, cl, ctrl, nparts_out));
         return 0;
@@ -355,9 +389,14 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
 int field_of_cloud(landau_ctx* c, Cloud& cl, double* out) {
     int nparts = 0;
     c->prof_step = 0; c->prof_iter = 0;
-    build_rec_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
-                                                                        cl.z(), cl.w(), cl.Gx(), cl.Gy(), cl.Gz(),
-                                                                        cl.recs());
+    if (cl.sym)
+        build_soa_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
+                                                                            cl.z(), cl.w(), cl.Gx(), cl.Gy(), cl.Gz(),
+                                                                            cl.soas());
+    else
+        build_rec_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
+                                                                            cl.z(), cl.w(), cl.Gx(), cl.Gy(), cl.Gz(),
+                                                                            cl.recs());
     RC(pair(c, cl, nullptr, &nparts));
     RC(ensure(c, c->V, sizeof(double) * 3 * (size_t)cl.npad_max));
     double* Vx = (double*)c->V.p;
@@ -507,7 +546,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_momout) cudaFree(c->d_momout);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     for (Cloud* cl : {&c->tmp, &c->state}) {
-        release(cl->lay); release(cl->xyzw); release(cl->perm); release(cl->G); release(cl->rec);
+        release(cl->lay); release(cl->xyzw); release(cl->perm); release(cl->G); release(cl->rec); release(cl->soa);
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab})
@@ -549,7 +588,6 @@ int landau_pair_field(landau_ctx* c, int64_t N, const double* v, const double* w
     gather3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), G_in, cl.Gx(),
                                                                       cl.Gy(), cl.Gz());
     c->launches += 1;
-    c->kernels[0] = 0;
     RC(field_of_cloud(c, cl, out));
     return finish(c, cl, "pair_field");
 }
@@ -644,7 +682,7 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
         RC(entropy(c, cl));
         step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
                                                                cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
-                                                               cl.recs());
+                                                               cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
         c->launches += 1;
         for (int k = 0; k < max_iter; ++k) {
             int nparts = 0;
@@ -652,7 +690,8 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
             RC(pair(c, cl, c->d_ctrl, &nparts));
             step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                              (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
-                                                             cl.w(), xk, yk, zk, cl.recs(), (double*)c->blockpart.p);
+                                                             cl.w(), xk, yk, zk, cl.sym ? nullptr : cl.recs(),
+                                                             cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p);
             c->launches += 1;
         }
         step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,

@@ -1,0 +1,303 @@
+// pair_sym.cuh -- step a3, symmetric (action-reaction) form of the pairwise Landau sum.
+//
+// Eq. (23) is antisymmetric under p <-> q up to the weights (this is what the
+// paper's conservation proofs use, Eqs. 27 and 29):
+//     term(p <- q) = (nu_ss'/m_s ) w_q Q(z) (g_p - g_q)
+//     term(q <- p) = -(nu_ss'/m_s') w_p Q(z) (g_p - g_q)          (Q(-z) = Q(z))
+// so Q(z)(g_p - g_q)/|z| is computed ONCE per unordered pair and applied to both markers:
+// 30 FP64-pipe instructions per unordered pair = 15 per ordered pair, against 26 in the one-sided
+// kernel (pair.cuh).  That is what lets the kernel exceed "100 % pipe = 61-74 % of peak FLOP/s"
+// of the one-sided form.
+//
+// Schedule.  Slots are cut into target tiles of BT = W*32*RT markers and source units of
+// BS = W*32*RS markers (BT % BS == 0; the packed layout pads every species to a multiple of BT, so
+// every tile and unit is species-uniform and nu_ss' is hoisted per task).  A task is (target tile
+// I, source unit j) with j >= first unit of I:
+//     j inside tile I  -> "diagonal" task, evaluated one-sidedly (every ordered pair by its target);
+//     j beyond tile I  -> symmetric task, both sides accumulated.
+// Tasks are numbered I-major and dealt to the G persistent CTAs in contiguous, equal runs (static
+// schedule => deterministic summation order).  Inside a task warp w works through the W sub-tiles
+// of 32*RS sources in the order (w + phase) % W (a Latin square: in any phase each sub-tile belongs
+// to exactly one warp), and inside a sub-tile lane l visits source group (l + k) % 32 at step k
+// while the source-side accumulators travel with their sources by one warp shuffle per step.  Each
+// lane keeps RT targets (and their accumulators) in registers.  Sources come from a structure-of-
+// arrays copy {x,y,z,w,gx,gy,gz}[npad] staged into shared memory by TMA bulk copies
+// (cp.async.bulk + mbarrier), double buffered across tasks.
+//
+// Output: every CTA adds into its own slice  vpart[cta][3][npad_max]  (zeroed before the launch),
+// already scaled by nu/m; the combine/update kernels sum the G slices in index order.
+#pragma once
+#include "common.cuh"
+
+namespace landau {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    }
+}
+
+template <int W, int RT, int RS>
+struct SymCfg {
+    static constexpr int THREADS = W * 32;
+    static constexpr int BT = W * 32 * RT;   // targets per tile (registers)
+    static constexpr int BS = W * 32 * RS;   // sources per unit (shared memory)
+    static constexpr int SUB = 32 * RS;      // sources per warp and phase
+    static constexpr int NCOMP = 7;          // x y z w gx gy gz
+    static constexpr size_t SMEM = sizeof(double) * (2 * NCOMP * BS + 3 * BS) + 64;
+    static_assert(BT % BS == 0, "target tile must be a whole number of source units");
+};
+
+// number of tasks before target tile I:  sum_{i<I} (TU - rho*i)
+__device__ __host__ inline long long sym_tasks_before(int I, int TU, int rho) {
+    return (long long)I * TU - (long long)rho * I * (I - 1) / 2;
+}
+
+template <bool SYM, int RT, int RS>
+__device__ __forceinline__ void sym_step(const double (&px)[RT], const double (&py)[RT], const double (&pz)[RT],
+                                         const double (&gx)[RT], const double (&gy)[RT], const double (&gz)[RT],
+                                         const double (&wp)[RT], double (&ax)[RT], double (&ay)[RT],
+                                         double (&az)[RT], const double (&qx)[RS], const double (&qy)[RS],
+                                         const double (&qz)[RS], const double (&hx)[RS], const double (&hy)[RS],
+                                         const double (&hz)[RS], const double (&wq)[RS], double (&bx)[RS],
+                                         double (&by)[RS], double (&bz)[RS]) {
+#pragma unroll
+    for (int s = 0; s < RS; ++s) {
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const double zx = px[r] - qx[s], zy = py[r] - qy[s], zz = pz[r] - qz[s];
+            const double cx = gx[r] - hx[s], cy = gy[r] - hy[s], cz = gz[r] - hz[s];
+            const double r2 = fma(zz, zz, fma(zy, zy, zx * zx));
+            const double d = fma(zz, cz, fma(zy, cy, zx * cx));
+            const double yv = rsqrt_or_zero(r2);
+            const double h = d * (yv * yv);
+            const double ux = fma(-zx, h, cx), uy = fma(-zy, h, cy), uz = fma(-zz, h, cz);
+            const double a = wq[s] * yv;
+            ax[r] = fma(a, ux, ax[r]); ay[r] = fma(a, uy, ay[r]); az[r] = fma(a, uz, az[r]);
+            if (SYM) {
+                const double b = wp[r] * yv;
+                bx[s] = fma(b, ux, bx[s]); by[s] = fma(b, uy, by[s]); bz[s] = fma(b, uz, bz[s]);
+            }
+        }
+    }
+}
+
+template <int W, int RT, int RS>
+__global__ void __launch_bounds__(W * 32, 1)
+pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
+                const StepCtrl* __restrict__ ctrl, int npad_max, const double* __restrict__ soa,
+                double* __restrict__ vpart) {
+    using C = SymCfg<W, RT, RS>;
+    if (ctrl && ctrl->done) return;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* s_src = reinterpret_cast<double*>(smem_raw);              // [2][NCOMP][BS]
+    double* s_acc = s_src + 2 * C::NCOMP * C::BS;                     // [3][BS]
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_acc + 3 * C::BS); // [2]
+    __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
+    __shared__ double s_im[LD_MAX_SPECIES];
+
+    const int S = T->S;
+    const int npad = L->npad;
+    constexpr int rho = C::BT / C::BS;
+    const int TI = npad / C::BT, TU = npad / C::BS;
+    const long long ntasks = sym_tasks_before(TI, TU, rho);
+    const long long t0 = ntasks * blockIdx.x / gridDim.x, t1 = ntasks * (blockIdx.x + 1) / gridDim.x;
+    if (t0 >= t1) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+    for (int i = tid; i < S * S; i += C::THREADS) s_nu[i] = T->nu[i];
+    if (tid < S) s_im[tid] = T->inv_mass[tid];
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // decode the first task
+    int I = 0;
+    while (I + 1 < TI && sym_tasks_before(I + 1, TU, rho) <= t0) ++I;
+    int j = rho * I + (int)(t0 - sym_tasks_before(I, TU, rho));
+
+    auto issue_load = [&](int unit, int stage) {
+        if (tid == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(&s_bar[stage], C::NCOMP * C::BS * (uint32_t)sizeof(double));
+#pragma unroll
+            for (int c = 0; c < C::NCOMP; ++c)
+                bulk_g2s(s_src + ((size_t)stage * C::NCOMP + c) * C::BS,
+                         soa + (size_t)c * npad_max + (size_t)unit * C::BS, C::BS * (uint32_t)sizeof(double),
+                         &s_bar[stage]);
+        }
+    };
+
+    double* myslice = vpart + (size_t)blockIdx.x * 3 * (size_t)npad_max;
+    double px[RT], py[RT], pz[RT], gx[RT], gy[RT], gz[RT], w0[RT], wp[RT], ax[RT], ay[RT], az[RT];
+    int curI = -1, sI = 0;
+    uint32_t phase_bits = 0;   // bit s = parity to wait for on stage s
+    int stage = 0;
+    issue_load(j, 0);
+
+    for (long long t = t0; t < t1; ++t) {
+        if (I != curI) {
+            if (curI >= 0) {
+                const double im = s_im[sI];
+#pragma unroll
+                for (int r = 0; r < RT; ++r) {
+                    const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
+                    myslice[p] += ax[r] * im;
+                    myslice[(size_t)npad_max + p] += ay[r] * im;
+                    myslice[2 * (size_t)npad_max + p] += az[r] * im;
+                }
+            }
+            curI = I;
+            sI = species_of_slot(L, S, I * C::BT);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const int p = I * C::BT + wv * 32 * RT + r * 32 + lane;
+                px[r] = soa[p]; py[r] = soa[(size_t)npad_max + p]; pz[r] = soa[2 * (size_t)npad_max + p];
+                w0[r] = soa[3 * (size_t)npad_max + p];
+                gx[r] = soa[4 * (size_t)npad_max + p]; gy[r] = soa[5 * (size_t)npad_max + p];
+                gz[r] = soa[6 * (size_t)npad_max + p];
+                ax[r] = ay[r] = az[r] = 0.0;
+            }
+        }
+        // next task (prefetch its source unit into the other stage)
+        int In = I, jn = j + 1;
+        if (jn >= TU) { In = I + 1; jn = rho * In; }
+        if (t + 1 < t1) issue_load(jn, stage ^ 1);
+
+        const int sJ = species_of_slot(L, S, j * C::BS);
+        const double nu = s_nu[sI * S + sJ];
+        const bool diag = j < rho * (I + 1);
+#pragma unroll
+        for (int r = 0; r < RT; ++r) wp[r] = w0[r] * nu;
+        for (int i = tid; i < 3 * C::BS; i += C::THREADS) s_acc[i] = 0.0;
+        mbar_wait(&s_bar[stage], (phase_bits >> stage) & 1u);
+        phase_bits ^= 1u << stage;
+        __syncthreads();
+
+        const double* sx = s_src + (size_t)stage * C::NCOMP * C::BS;
+        for (int ph = 0; ph < W; ++ph) {
+            const int base = ((wv + ph) % W) * C::SUB;
+            double bx[RS], by[RS], bz[RS];
+#pragma unroll
+            for (int s = 0; s < RS; ++s) bx[s] = by[s] = bz[s] = 0.0;
+#pragma unroll 1
+            for (int k = 0; k < 32; ++k) {
+                const int g = base + ((lane + k) & 31) * RS;
+                double qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS];
+                if (RS % 2 == 0) {
+#pragma unroll
+                    for (int s = 0; s < RS; s += 2) {
+                        const double2 a0 = *reinterpret_cast<const double2*>(sx + 0 * C::BS + g + s);
+                        const double2 a1 = *reinterpret_cast<const double2*>(sx + 1 * C::BS + g + s);
+                        const double2 a2 = *reinterpret_cast<const double2*>(sx + 2 * C::BS + g + s);
+                        const double2 a3 = *reinterpret_cast<const double2*>(sx + 3 * C::BS + g + s);
+                        const double2 a4 = *reinterpret_cast<const double2*>(sx + 4 * C::BS + g + s);
+                        const double2 a5 = *reinterpret_cast<const double2*>(sx + 5 * C::BS + g + s);
+                        const double2 a6 = *reinterpret_cast<const double2*>(sx + 6 * C::BS + g + s);
+                        qx[s] = a0.x; qx[s + 1] = a0.y; qy[s] = a1.x; qy[s + 1] = a1.y; qz[s] = a2.x; qz[s + 1] = a2.y;
+                        qw[s] = a3.x * nu; qw[s + 1] = a3.y * nu;
+                        hx[s] = a4.x; hx[s + 1] = a4.y; hy[s] = a5.x; hy[s + 1] = a5.y; hz[s] = a6.x; hz[s + 1] = a6.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int s = 0; s < RS; ++s) {
+                        qx[s] = sx[0 * C::BS + g + s]; qy[s] = sx[1 * C::BS + g + s]; qz[s] = sx[2 * C::BS + g + s];
+                        qw[s] = sx[3 * C::BS + g + s] * nu;
+                        hx[s] = sx[4 * C::BS + g + s]; hy[s] = sx[5 * C::BS + g + s]; hz[s] = sx[6 * C::BS + g + s];
+                    }
+                }
+                if (diag) {
+                    sym_step<false, RT, RS>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                } else {
+                    sym_step<true, RT, RS>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+#pragma unroll
+                    for (int s = 0; s < RS; ++s) {
+                        bx[s] = __shfl_sync(0xffffffffu, bx[s], (lane + 1) & 31);
+                        by[s] = __shfl_sync(0xffffffffu, by[s], (lane + 1) & 31);
+                        bz[s] = __shfl_sync(0xffffffffu, bz[s], (lane + 1) & 31);
+                    }
+                }
+            }
+            if (!diag) {
+                // after 32 rotations lane l again holds source group l of this sub-tile
+#pragma unroll
+                for (int s = 0; s < RS; ++s) {
+                    const int e = base + lane * RS + s;
+                    s_acc[e] += bx[s]; s_acc[C::BS + e] += by[s]; s_acc[2 * C::BS + e] += bz[s];
+                }
+            }
+            __syncthreads();
+        }
+        if (!diag) {
+            const double sc = -s_im[sJ];
+            for (int i = tid; i < 3 * C::BS; i += C::THREADS) {
+                const int d = i / C::BS, e = i - d * C::BS;
+                myslice[(size_t)d * npad_max + (size_t)j * C::BS + e] += sc * s_acc[i];
+            }
+        }
+        __syncthreads();
+        I = In; j = jn; stage ^= 1;
+    }
+    {
+        const double im = s_im[sI];
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
+            myslice[p] += ax[r] * im;
+            myslice[(size_t)npad_max + p] += ay[r] * im;
+            myslice[2 * (size_t)npad_max + p] += az[r] * im;
+        }
+    }
+}
+
+// Zero the per-CTA slices (skipped, like every kernel of an iteration, once the step is done).
+__global__ void zero_slices_kernel(const StepCtrl* __restrict__ ctrl, double2* __restrict__ p, size_t n2) {
+    if (ctrl && ctrl->done) return;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += stride) p[i] = make_double2(0.0, 0.0);
+}
+
+// {x,y,z,w,G} (packed SoA) -> structure-of-arrays source copy {x,y,z,w,gx,gy,gz}[npad_max], g = G/m.
+__global__ void build_soa_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
+                                 const double* __restrict__ x, const double* __restrict__ y,
+                                 const double* __restrict__ z, const double* __restrict__ w,
+                                 const double* __restrict__ Gx, const double* __restrict__ Gy,
+                                 const double* __restrict__ Gz, double* __restrict__ soa) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npad_max) return;
+    double v[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (p < L->npad) {
+        const double im = T->inv_mass[species_of_slot(L, T->S, p)];
+        v[0] = x[p]; v[1] = y[p]; v[2] = z[p]; v[3] = w[p];
+        v[4] = Gx[p] * im; v[5] = Gy[p] * im; v[6] = Gz[p] * im;
+    }
+#pragma unroll
+    for (int c = 0; c < 7; ++c) soa[(size_t)c * npad_max + p] = v[c];
+}
+
+}  // namespace landau

@@ -24,21 +24,34 @@ __global__ void step_begin_kernel(const DevTable* __restrict__ T, const DevLayou
                                   const double* __restrict__ Gx, const double* __restrict__ Gy,
                                   const double* __restrict__ Gz, double* __restrict__ xk,
                                   double* __restrict__ yk, double* __restrict__ zk,
-                                  double* __restrict__ rec) {
+                                  double* __restrict__ rec, double* __restrict__ soa) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p == 0) {
         ctrl->done = 0; ctrl->iterations = 0; ctrl->converged = 0; ctrl->ticket = 0u;
         ctrl->residual = __longlong_as_double(0x7ff0000000000000LL);
     }
-    if (p >= npad_max || p >= L->npad) return;
+    if (p >= npad_max) return;
+    if (p >= L->npad) {
+        if (soa)
+            for (int c = 0; c < 7; ++c) soa[(size_t)c * npad_max + p] = 0.0;
+        return;
+    }
     const double im = T->inv_mass[species_of_slot(L, T->S, p)];
     const double a = xn[p], b = yn[p], c = zn[p];
     xk[p] = a; yk[p] = b; zk[p] = c;
-    double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
-    o[0] = make_double2(a, b);
-    o[1] = make_double2(c, w[p]);
-    o[2] = make_double2(Gx[p] * im, Gy[p] * im);
-    o[3] = make_double2(Gz[p] * im, 0.0);
+    const double g0 = Gx[p] * im, g1 = Gy[p] * im, g2 = Gz[p] * im, ww = w[p];
+    if (rec) {
+        double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
+        o[0] = make_double2(a, b);
+        o[1] = make_double2(c, ww);
+        o[2] = make_double2(g0, g1);
+        o[3] = make_double2(g2, 0.0);
+    }
+    if (soa) {
+        soa[p] = a; soa[(size_t)npad_max + p] = b; soa[2 * (size_t)npad_max + p] = c;
+        soa[3 * (size_t)npad_max + p] = ww;
+        soa[4 * (size_t)npad_max + p] = g0; soa[5 * (size_t)npad_max + p] = g1; soa[6 * (size_t)npad_max + p] = g2;
+    }
 }
 
 // v^(k+1) = v^n + dt * (fixed-order sum of the partial fields); residual; next midpoint records.
@@ -48,7 +61,8 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
                    int max_iter, const double* __restrict__ vpart, const double* __restrict__ xn,
                    const double* __restrict__ yn, const double* __restrict__ zn,
                    const double* __restrict__ w, double* __restrict__ xk, double* __restrict__ yk,
-                   double* __restrict__ zk, double* __restrict__ rec, double* __restrict__ blockpart) {
+                   double* __restrict__ zk, double* __restrict__ rec, double* __restrict__ soa,
+                   double* __restrict__ blockpart) {
     if (ctrl->done) return;
     __shared__ double s_num[UPD_THREADS / 32], s_den[UPD_THREADS / 32];
     __shared__ int s_last;
@@ -69,9 +83,13 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         num = wm * (dx * dx + dy * dy + dz * dz);
         den = wm * (x1 * x1 + y1 * y1 + z1 * z1);
         xk[p] = x1; yk[p] = y1; zk[p] = z1;
-        double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
-        o[0] = make_double2(0.5 * (x0 + x1), 0.5 * (y0 + y1));      // Eq. (25)
-        reinterpret_cast<double*>(o + 1)[0] = 0.5 * (z0 + z1);
+        const double ux = 0.5 * (x0 + x1), uy = 0.5 * (y0 + y1), uz = 0.5 * (z0 + z1);   // Eq. (25)
+        if (rec) {
+            double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
+            o[0] = make_double2(ux, uy);
+            reinterpret_cast<double*>(o + 1)[0] = uz;
+        }
+        if (soa) { soa[p] = ux; soa[(size_t)npad_max + p] = uy; soa[2 * (size_t)npad_max + p] = uz; }
     }
     num = warp_sum(num); den = warp_sum(den);
     const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;

@@ -47,7 +47,8 @@ def assert_field_close(got, ref, sid, S, tol=TOL_FIELD, what="field"):
             assert rel_l2(got[m], ref[m]) <= tol, f"{what} species {s}: rel L2 {rel_l2(got[m], ref[m]):.3e}"
 
 
-KERNEL_VARIANTS = [dict(pair_kernel=1, entropy_kernel=1), dict(pair_kernel=0, entropy_kernel=0)]
+KERNEL_VARIANTS = [dict(pair_kernel=1, entropy_kernel=1), dict(pair_kernel=0, entropy_kernel=0),
+                   dict(pair_kernel=2, entropy_kernel=2)]
 
 
 # ------------------------------------------------------------------------------------ quadrature
@@ -72,6 +73,24 @@ def test_pair_field_matches_oracle(B, oracle_mod, variant, cfg, n, shuffled):
     ref = o.pair_field(wl.v, wl.w, wl.species_id, G)
     got = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
     assert_field_close(got, ref, wl.species_id, wl.n_species)
+
+
+@pytest.mark.parametrize("pair_kernel", [1, 2])
+def test_pair_field_full_size_sampled_rows(B, oracle_mod, pair_kernel):
+    """BASELINE config 4 at 3 x 2^14 markers in the launch configuration bench.py times: sampled
+    target rows against the oracle (each row is a full sum over all 49152 sources)."""
+    wl = W.make(4, n_per_species=1 << 14, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl, pair_kernel=pair_kernel)
+    rng = np.random.default_rng(21)
+    G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+    got = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    assert ("sym" if pair_kernel == 2 else "onesided") in g.last_kernels()
+    rows = np.concatenate([rng.choice(np.flatnonzero(wl.species_id == s), 200, replace=False) for s in range(3)])
+    ref = o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows)
+    assert_field_close(got[rows], ref, wl.species_id[rows], 3)
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    assert np.abs((wm * got).sum(axis=0)).max() <= 1e-13 * np.abs(wm * got).sum()          # Eq. 27
+    assert abs((wm * wl.v * got).sum()) <= 1e-13 * np.abs(wm * wl.v * got).sum()             # Eq. 29
 
 
 # ------------------------------------------------------------------------------------ pass 1
