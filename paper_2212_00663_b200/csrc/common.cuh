@@ -37,8 +37,10 @@ struct DevLayout {
     int off[LD_MAX_SPECIES + 1];      // first slot of species s; off[S] = npad (all multiples of pad)
     int npad;
     int err;                          // 0, or LANDAU_E* found by a kernel (validation, non-finite)
-    double center[LD_MAX_SPECIES][3]; // weighted mean velocity of species s (factorised pass 1)
-    double halfwidth[LD_MAX_SPECIES]; // max_p |v_p - center|_inf / sqrt(2 eps_s)
+    int used_fact;                    // 1 if the last pass 1 took the factorised kernel
+    int _r1;
+    double center[LD_MAX_SPECIES][3]; // bounding-box centre of species s (factorised pass 1)
+    double halfwidth[LD_MAX_SPECIES]; // max_p |v_p - center|_inf / sqrt(2 eps_s), written once per pass 1
 };
 
 // Device-side control block of the fixed-point loop.

@@ -15,6 +15,17 @@
 
 namespace landau {
 
+constexpr double FACT_EXP_LIMIT = 500.0;
+
+// Can the factorised kernel be used for this cloud?  (Same answer in every kernel of one pass: the
+// layout's half-widths are written once per pass by entropy_bounds_kernel.)
+__device__ __forceinline__ bool fact_usable(const DevTable* __restrict__ T, const DevLayout* __restrict__ L) {
+    const double kmax = fabs(T->knot[T->n_q - 1]);
+    bool ok = true;
+    for (int s = 0; s < T->S; ++s) ok = ok && (6.0 * kmax * L->halfwidth[s] <= FACT_EXP_LIMIT);
+    return ok;
+}
+
 constexpr int ENT_THREADS = 128;   // targets per block (one target per thread)
 constexpr int ENT_SRC_TILE = 64;   // sources staged in shared memory per tile
 
@@ -25,11 +36,12 @@ constexpr int ENT_SRC_TILE = 64;   // sources staged in shared memory per tile
 template <int NQ, int NI>
 __global__ void __launch_bounds__(ENT_THREADS)
 entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
-                       int nchunks, const double* __restrict__ x, const double* __restrict__ y,
-                       const double* __restrict__ z, const double* __restrict__ w,
-                       double* __restrict__ part) {
+                       int nchunks, int skip_if_fact, const double* __restrict__ x,
+                       const double* __restrict__ y, const double* __restrict__ z,
+                       const double* __restrict__ w, double* __restrict__ part) {
     const int slot0 = blockIdx.x * ENT_THREADS;
     if (slot0 >= L->npad) return;
+    if (skip_if_fact && fact_usable(T, L)) return;   // the factorised kernel does this pass
     const int S = T->S;
     const int s = species_of_slot(L, S, slot0);
     const double inv = T->inv_sqrt_2eps[s];
@@ -97,17 +109,21 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
             }
 }
 
-// Node sums -> G_p (unscaled: (1/w_p) dS_eps/dv_p) and s_p.  `shift` (optional) holds per-slot
-// log-space corrections used by the factorised kernel; NULL for the literal kernel.
+// Node sums -> G_p (unscaled: (1/w_p) dS_eps/dv_p) and s_p.  fact_mode: 0 = the node sums are the
+// literal kernel's; 1 = they are the factorised kernel's if fact_usable() (automatic choice), else the
+// literal kernel's; 2 = factorised forced (a cloud that is too wide raises LANDAU_ERANGE = -5).
 __global__ void __launch_bounds__(128)
 entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, int npad_max,
                         int nchunks, const int* __restrict__ perm, const double* __restrict__ part,
                         const double* __restrict__ px, const double* __restrict__ py,
-                        const double* __restrict__ pz, int factorised,
+                        const double* __restrict__ pz, int fact_mode,
                         double* __restrict__ Gx, double* __restrict__ Gy, double* __restrict__ Gz,
                         double* __restrict__ snode) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npad_max || p >= L->npad) return;
+    const bool factorised = fact_mode != 0 && fact_usable(T, L);
+    if (p == 0) L->used_fact = factorised ? 1 : 0;
+    if (fact_mode == 2 && !factorised) { if (p == 0) atomicMin(&L->err, -5); return; }
     if (perm[p] < 0) { Gx[p] = 0.0; Gy[p] = 0.0; Gz[p] = 0.0; snode[p] = 0.0; return; }
     const int S = T->S, nq = T->n_q;
     const int s = species_of_slot(L, S, p);

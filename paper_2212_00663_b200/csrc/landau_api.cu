@@ -15,6 +15,7 @@
 
 #include "common.cuh"
 #include "entropy.cuh"
+#include "entropy_fact.cuh"
 #include "moments.cuh"
 #include "pack.cuh"
 #include "pair.cuh"
@@ -246,10 +247,7 @@ int npad_upper(int64_t N, int S, int pad) {
 }
 
 
-// ---- optimised kernels (filled in below when available) -------------------------------------
-int entropy_fact_available(int nq) { (void)nq; return 0; }
-int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) { (void)c; (void)cl; (void)nchunks; return LANDAU_ECUDA; }
-
+// ---- optimised kernels -----------------------------------------------------------------------
 int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; return cl.sym; }
 int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts) {
     const int G = c->sm_count;
@@ -301,37 +299,66 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
 
 // ---- a1/a2: entropy gradient of a packed cloud ---------------------------------------------
 template <int NQ, int NI>
-void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks) {
+void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks, int skip_if_fact) {
     dim3 grid(cl.npad_max / ENT_THREADS, nchunks, NQ / NI);
     entropy_literal_kernel<NQ, NI><<<grid, ENT_THREADS, 0, c->stream>>>(
-        c->d_tab, cl.L(), cl.npad_max, nchunks, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->part.p);
+        c->d_tab, cl.L(), cl.npad_max, nchunks, skip_if_fact, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->part.p);
 }
+
+template <int NQ, int NI>
+int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) {
+    RC(ensure(c, c->facttab, sizeof(double) * FactCfg<NQ>::REC * (size_t)cl.npad_max));
+    entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
+        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p);
+    dim3 grid(cl.npad_max / FACT_THREADS, nchunks, NQ / NI);
+    entropy_fact_kernel<NQ, NI><<<grid, FACT_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
+                                                                      (const double*)c->facttab.p, (double*)c->part.p);
+    return 0;
+}
+
+// node groups (gridDim.z) each kernel splits the n_q^3 node sums into
+int literal_groups(int nq) { return nq <= 4 ? 1 : nq; }
+int fact_groups(int nq) { return nq <= 4 ? 1 : (nq == 6 ? 3 : nq); }
 
 int entropy(landau_ctx* c, Cloud& cl) {
     const int nq = c->n_q;
     const size_t M = (size_t)nq * nq * nq;
     const int ttiles = cl.npad_max / ENT_THREADS;
-    const int ig = nq <= 4 ? 1 : nq;
-    int nchunks = ceil_div(6 * c->sm_count, ttiles * ig);
-    nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / ENT_SRC_TILE)));
+    // 0 automatic (factorised when the cloud is narrow enough, decided on the device), 1 literal, 2 factorised
+    const int mode = c->entropy_kernel;
+    const int ig = mode == 1 ? literal_groups(nq) : std::min(literal_groups(nq), fact_groups(nq));
+    // enough blocks for >= ~20 waves of 2 resident blocks per SM, so that the last wave costs < 5 %
+    int nchunks = ceil_div(40 * c->sm_count, ttiles * ig);
+    nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / (c->S * 256))));   // >= 4 source tiles per chunk
     nchunks = std::min(nchunks, 64);
     while (nchunks > 1 && (size_t)nchunks * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) --nchunks;
     RC(ensure(c, c->part, (size_t)nchunks * M * cl.npad_max * sizeof(double)));
-    int use_fact = 0;
-    if (c->entropy_kernel == 2 || c->entropy_kernel == 0) use_fact = entropy_fact_available(nq);
     {
     ProfScope prof(c, 1);
-    if (use_fact) {
-        RC(launch_entropy_fact(c, cl, nchunks));
-    } else {
+    if (mode != 1) {
+        entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w());
         switch (nq) {
-            case 2: launch_entropy_literal<2, 2>(c, cl, nchunks); break;
-            case 3: launch_entropy_literal<3, 3>(c, cl, nchunks); break;
-            case 4: launch_entropy_literal<4, 4>(c, cl, nchunks); break;
-            case 5: launch_entropy_literal<5, 1>(c, cl, nchunks); break;
-            case 6: launch_entropy_literal<6, 1>(c, cl, nchunks); break;
-            case 7: launch_entropy_literal<7, 1>(c, cl, nchunks); break;
-            case 8: launch_entropy_literal<8, 1>(c, cl, nchunks); break;
+            case 2: RC((launch_entropy_fact<2, 2>(c, cl, nchunks))); break;
+            case 3: RC((launch_entropy_fact<3, 3>(c, cl, nchunks))); break;
+            case 4: RC((launch_entropy_fact<4, 4>(c, cl, nchunks))); break;
+            case 5: RC((launch_entropy_fact<5, 1>(c, cl, nchunks))); break;
+            case 6: RC((launch_entropy_fact<6, 2>(c, cl, nchunks))); break;
+            case 7: RC((launch_entropy_fact<7, 1>(c, cl, nchunks))); break;
+            case 8: RC((launch_entropy_fact<8, 1>(c, cl, nchunks))); break;
+            default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
+        }
+        c->launches += 3;
+    }
+    if (mode != 2) {
+        const int skip = mode == 0 ? 1 : 0;
+        switch (nq) {
+            case 2: launch_entropy_literal<2, 2>(c, cl, nchunks, skip); break;
+            case 3: launch_entropy_literal<3, 3>(c, cl, nchunks, skip); break;
+            case 4: launch_entropy_literal<4, 4>(c, cl, nchunks, skip); break;
+            case 5: launch_entropy_literal<5, 1>(c, cl, nchunks, skip); break;
+            case 6: launch_entropy_literal<6, 1>(c, cl, nchunks, skip); break;
+            case 7: launch_entropy_literal<7, 1>(c, cl, nchunks, skip); break;
+            case 8: launch_entropy_literal<8, 1>(c, cl, nchunks, skip); break;
             default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
         }
         c->launches += 1;
@@ -339,11 +366,9 @@ int entropy(landau_ctx* c, Cloud& cl) {
     }
     entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
-        use_fact, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
+        mode == 1 ? 0 : (mode == 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
     c->launches += 1;
     CU(cudaGetLastError());
-    c->k_entropy = use_fact ? "fact" : "literal";
-    snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     return 0;
 }
 
@@ -373,15 +398,19 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     return 0;
 }
 
-// Read the layout's error flag (one synchronisation).
+// Read the layout's error flag and which pass-1 kernel ran (one synchronisation).
 int finish(landau_ctx* c, Cloud& cl, const char* where) {
     int* h = (int*)c->h_pin;
-    CU(cudaMemcpyAsync(h, &cl.L()->err, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(h, &cl.L()->err, 2 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
+    c->k_entropy = h[1] ? "fact" : "literal";
+    snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
     if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
+    if (*h == LANDAU_ERANGE)
+        return fail(c, LANDAU_ERANGE, "%s: marker cloud too wide for the factorised entropy kernel (entropy_kernel = 2)", where);
     if (*h) return fail(c, *h, "%s: device-side error %d", where, *h);
     return 0;
 }

@@ -106,6 +106,51 @@ def test_entropy_grad_matches_oracle(B, oracle_mod, variant, cfg, n, n_q):
     np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
 
 
+def test_factorised_kernel_is_the_default_and_handles_drifting_clouds(B, oracle_mod):
+    """Automatic choice takes the factorised kernel on a paper-like cloud, also when the species
+    drift far from the origin (the padded dummies sit at v = 0: they must add exactly 0)."""
+    wl = W.make(0, n_per_species=200, shuffled=True)
+    drift = np.where(wl.species_id[:, None] == 0, np.array([[40.0, -25.0, 10.0]]), np.array([[-3.0, 2.0, 1.0]]))
+    v = wl.v + drift
+    g, o = make_pair(B, oracle_mod, wl)
+    Gref, Sref = o.entropy_grad(v, wl.w, wl.species_id, with_entropy=True)
+    Ggot, Sgot = g.entropy_grad(v, wl.w, wl.species_id, with_entropy=True)
+    assert "entropy=fact" in g.last_kernels()
+    assert_field_close(Ggot.cpu().numpy(), Gref, wl.species_id, wl.n_species, what="entropy gradient (drift)")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+
+
+def test_wide_cloud_takes_the_literal_kernel(B, oracle_mod):
+    """Reading N3: a cloud whose half-width (in mollifier units) would overflow the factorised
+    tables is evaluated by the literal kernel in automatic mode, and refused (-5) when the
+    factorised kernel is forced."""
+    rng = np.random.default_rng(5)
+    n = 150
+    v = 0.3 * rng.standard_normal((n, 3))
+    v[n // 2:, 0] += 400.0                          # two clusters 400/sqrt(2 eps) ~ 1265 widths apart
+    w = 1.0 + rng.random(n)
+    sid = np.zeros(n, dtype=np.int32)
+    mass, charge, eps = [1.0], [1.0], [0.05]
+    o = oracle_mod.LandauRef(mass, charge, eps)
+    Gref, Sref = o.entropy_grad(v, w, sid, with_entropy=True)
+    g = B.Landau(mass, charge, eps)
+    Ggot, Sgot = g.entropy_grad(v, w, sid, with_entropy=True)
+    assert "entropy=literal" in g.last_kernels()
+    assert_field_close(Ggot.cpu().numpy(), Gref, sid, 1, what="entropy gradient (wide)")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+    gf = B.Landau(mass, charge, eps, entropy_kernel=2)
+    with pytest.raises(B.LandauError) as e:
+        gf.entropy_grad(v, w, sid)
+    assert e.value.code == B.ERANGE
+    # just inside the limit the factorised kernel still agrees with the oracle (largest table entries)
+    v2 = 0.3 * rng.standard_normal((n, 3))
+    v2[n // 2:, 1] += 0.9 * 2.0 * (500.0 / (6.0 * 1.6506801238857844)) * np.sqrt(2 * 0.05)
+    Gref2, _ = o.entropy_grad(v2, w, sid, with_entropy=True)
+    Ggot2, _ = gf.entropy_grad(v2, w, sid, with_entropy=True)
+    assert "entropy=fact" in gf.last_kernels()
+    assert_field_close(Ggot2.cpu().numpy(), Gref2, sid, 1, what="entropy gradient (near limit)")
+
+
 # ------------------------------------------------------------------------------------ full field
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS)
 @pytest.mark.parametrize("cfg,n", [(0, 256), (2, 500), (4, 384)])
