@@ -66,8 +66,11 @@ typedef struct {
     void* stream;     /* cudaStream_t; NULL = default stream                                      */
     int pair_kernel;  /* 0 = automatic; 1 = one-sided tiled kernel; 2 = symmetric (action-reaction)
                          kernel.  For tests and per-kernel timing.                                */
-    int entropy_kernel; /* 0 = automatic; 1 = literal separable form (3 n_q exponentials per
-                         pair); 2 = factorised form (1 exponential per pair)                     */
+    int entropy_kernel; /* 0 = automatic (3 when the cloud is narrow enough, else 1); 1 = literal
+                         separable form (3 n_q exponentials per pair); 2 = factorised form (1
+                         exponential per pair) on the FP64 vector pipe; 3 = factorised form as an
+                         FP64 tensor contraction (DMMA).  2 and 3 return LANDAU_ERANGE when the
+                         cloud is too wide for the factorised form.                               */
     int device;       /* CUDA device ordinal; -1 = current device                                 */
 } landau_opts;
 

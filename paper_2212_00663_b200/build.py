@@ -52,7 +52,8 @@ def up_to_date() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and up_to_date():
         return LIB
-    cmd = [nvcc_path(), *NVCC_FLAGS, "-I", str(INCLUDE), "-o", str(LIB), *map(str, sources())]
+    extra = os.environ.get("LANDAU_NVCC_EXTRA", "").split()   # tuning knobs, e.g. -DLANDAU_SYM_RT=2
+    cmd = [nvcc_path(), *NVCC_FLAGS, *extra, "-I", str(INCLUDE), "-o", str(LIB), *map(str, sources())]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

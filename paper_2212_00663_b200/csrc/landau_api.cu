@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "entropy.cuh"
 #include "entropy_fact.cuh"
+#include "entropy_mma.cuh"
 #include "moments.cuh"
 #include "pack.cuh"
 #include "pair.cuh"
@@ -229,7 +230,16 @@ void gauss_hermite_gw(int n, double* knots, double* weights) {
 
 // The symmetric pair kernel (pair_sym.cuh) in its large configuration: 8 warps, 4 targets per
 // lane, 2 sources per lane and step: target tiles of 1024 slots, source units of 512.
-constexpr int SYM_W = 8, SYM_RT = 4, SYM_RS = 2;
+#ifndef LANDAU_SYM_W      // tuning knobs: -DLANDAU_SYM_W=.. -DLANDAU_SYM_RT=.. -DLANDAU_SYM_RS=.. (build.py: LANDAU_NVCC_EXTRA)
+#define LANDAU_SYM_W 8
+#endif
+#ifndef LANDAU_SYM_RT
+#define LANDAU_SYM_RT 4
+#endif
+#ifndef LANDAU_SYM_RS
+#define LANDAU_SYM_RS 2
+#endif
+constexpr int SYM_W = LANDAU_SYM_W, SYM_RT = LANDAU_SYM_RT, SYM_RS = LANDAU_SYM_RS;
 using SymL = SymCfg<SYM_W, SYM_RT, SYM_RS>;
 constexpr int64_t SYM_MIN_MARKERS = 16384;
 
@@ -316,17 +326,42 @@ int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) {
     return 0;
 }
 
+template <int NQ>
+int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks) {
+    using M = MmaCfg<NQ>;
+    RC(ensure(c, c->facttab, sizeof(double) * M::REC * (size_t)cl.npad_max));
+    entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
+        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p);
+    auto kern = entropy_mma_kernel<NQ>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)M::SMEM));
+        attr_done = true;
+    }
+    dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
+    kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
+                                                    (const double*)c->facttab.p, (double*)c->part.p);
+    return 0;
+}
+
 // node groups (gridDim.z) each kernel splits the n_q^3 node sums into
 int literal_groups(int nq) { return nq <= 4 ? 1 : nq; }
 int fact_groups(int nq) { return nq <= 4 ? 1 : (nq == 6 ? 3 : nq); }
+int mma_groups(int nq) {
+    switch (nq) { case 5: return MmaCfg<5>::GROUPS; case 6: return MmaCfg<6>::GROUPS; case 7: return MmaCfg<7>::GROUPS;
+                  case 8: return MmaCfg<8>::GROUPS; default: return 1; }
+}
 
 int entropy(landau_ctx* c, Cloud& cl) {
     const int nq = c->n_q;
     const size_t M = (size_t)nq * nq * nq;
     const int ttiles = cl.npad_max / ENT_THREADS;
-    // 0 automatic (factorised when the cloud is narrow enough, decided on the device), 1 literal, 2 factorised
+    // 0 automatic (DMMA contraction when the cloud is narrow enough, decided on the device, else literal),
+    // 1 literal, 2 factorised on the vector pipe, 3 factorised as a DMMA contraction
     const int mode = c->entropy_kernel;
-    const int ig = mode == 1 ? literal_groups(nq) : std::min(literal_groups(nq), fact_groups(nq));
+    const bool use_mma = mode == 0 || mode == 3;
+    const int ig = mode == 1 ? literal_groups(nq)
+                             : std::min(literal_groups(nq), use_mma ? mma_groups(nq) : fact_groups(nq));
     // enough blocks for >= ~20 waves of 2 resident blocks per SM, so that the last wave costs < 5 %
     int nchunks = ceil_div(40 * c->sm_count, ttiles * ig);
     nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / (c->S * 256))));   // >= 4 source tiles per chunk
@@ -337,7 +372,17 @@ int entropy(landau_ctx* c, Cloud& cl) {
     ProfScope prof(c, 1);
     if (mode != 1) {
         entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w());
-        switch (nq) {
+        if (use_mma) switch (nq) {
+            case 2: RC((launch_entropy_mma<2>(c, cl, nchunks))); break;
+            case 3: RC((launch_entropy_mma<3>(c, cl, nchunks))); break;
+            case 4: RC((launch_entropy_mma<4>(c, cl, nchunks))); break;
+            case 5: RC((launch_entropy_mma<5>(c, cl, nchunks))); break;
+            case 6: RC((launch_entropy_mma<6>(c, cl, nchunks))); break;
+            case 7: RC((launch_entropy_mma<7>(c, cl, nchunks))); break;
+            case 8: RC((launch_entropy_mma<8>(c, cl, nchunks))); break;
+            default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
+        }
+        else switch (nq) {
             case 2: RC((launch_entropy_fact<2, 2>(c, cl, nchunks))); break;
             case 3: RC((launch_entropy_fact<3, 3>(c, cl, nchunks))); break;
             case 4: RC((launch_entropy_fact<4, 4>(c, cl, nchunks))); break;
@@ -349,7 +394,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
         }
         c->launches += 3;
     }
-    if (mode != 2) {
+    if (mode != 2 && mode != 3) {
         const int skip = mode == 0 ? 1 : 0;
         switch (nq) {
             case 2: launch_entropy_literal<2, 2>(c, cl, nchunks, skip); break;
@@ -366,7 +411,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
     }
     entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
-        mode == 1 ? 0 : (mode == 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
+        mode == 1 ? 0 : (mode >= 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
     c->launches += 1;
     CU(cudaGetLastError());
     return 0;
@@ -405,12 +450,12 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
-    c->k_entropy = h[1] ? "fact" : "literal";
+    c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
     if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
     if (*h == LANDAU_ERANGE)
-        return fail(c, LANDAU_ERANGE, "%s: marker cloud too wide for the factorised entropy kernel (entropy_kernel = 2)", where);
+        return fail(c, LANDAU_ERANGE, "%s: marker cloud too wide for the factorised entropy kernel (entropy_kernel = 2 or 3)", where);
     if (*h) return fail(c, *h, "%s: device-side error %d", where, *h);
     return 0;
 }
@@ -520,7 +565,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (o.nu0 == 0.0) o.nu0 = 1.0;
     if (o.n_q < 2 || o.n_q > LD_MAX_NQ) return LANDAU_EINVAL;
     if (o.precision < 0 || o.precision > 1 || o.pair_kernel < 0 || o.pair_kernel > 2 || o.entropy_kernel < 0 ||
-        o.entropy_kernel > 2)
+        o.entropy_kernel > 3)
         return LANDAU_EINVAL;
     for (int s = 0; s < S; ++s)
         if (!(mass[s] > 0.0) || !(eps[s] > 0.0) || !isfinite(charge[s]) || !isfinite(mass[s]) || !isfinite(eps[s]))
@@ -554,6 +599,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     }
     for (int i = 0; i < S * S; ++i) t.nu[i] = c->nu[i];
     for (int i = 0; i < c->n_q; ++i) { t.knot[i] = c->knot[i]; t.gw[i] = c->gw[i]; }
+    for (int j = 0; j < 64; ++j) t.exp2_tab[j] = exp2((double)j / 64.0);
     if (cudaMalloc(&c->d_tab, sizeof(DevTable)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);

@@ -48,7 +48,7 @@ def assert_field_close(got, ref, sid, S, tol=TOL_FIELD, what="field"):
 
 
 KERNEL_VARIANTS = [dict(pair_kernel=1, entropy_kernel=1), dict(pair_kernel=0, entropy_kernel=0),
-                   dict(pair_kernel=2, entropy_kernel=2)]
+                   dict(pair_kernel=2, entropy_kernel=2), dict(pair_kernel=2, entropy_kernel=3)]
 
 
 # ------------------------------------------------------------------------------------ quadrature
@@ -96,7 +96,7 @@ def test_pair_field_full_size_sampled_rows(B, oracle_mod, pair_kernel):
 # ------------------------------------------------------------------------------------ pass 1
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS)
 @pytest.mark.parametrize("cfg,n,n_q", [(0, 256, 4), (0, 97, 4), (4, 200, 4), (0, 64, 2), (0, 64, 3), (0, 48, 5),
-                                       (0, 40, 6), (0, 33, 8), (3, 300, 4)])
+                                       (0, 40, 6), (0, 33, 8), (0, 70, 7), (3, 300, 4), (1, 1100, 4)])
 def test_entropy_grad_matches_oracle(B, oracle_mod, variant, cfg, n, n_q):
     wl = W.make(cfg, n_per_species=n, shuffled=True)
     g, o = make_pair(B, oracle_mod, wl, n_q=n_q, **variant)
@@ -115,7 +115,7 @@ def test_factorised_kernel_is_the_default_and_handles_drifting_clouds(B, oracle_
     g, o = make_pair(B, oracle_mod, wl)
     Gref, Sref = o.entropy_grad(v, wl.w, wl.species_id, with_entropy=True)
     Ggot, Sgot = g.entropy_grad(v, wl.w, wl.species_id, with_entropy=True)
-    assert "entropy=fact" in g.last_kernels()
+    assert "entropy=mma" in g.last_kernels()
     assert_field_close(Ggot.cpu().numpy(), Gref, wl.species_id, wl.n_species, what="entropy gradient (drift)")
     np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
 
@@ -138,17 +138,20 @@ def test_wide_cloud_takes_the_literal_kernel(B, oracle_mod):
     assert "entropy=literal" in g.last_kernels()
     assert_field_close(Ggot.cpu().numpy(), Gref, sid, 1, what="entropy gradient (wide)")
     np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
-    gf = B.Landau(mass, charge, eps, entropy_kernel=2)
-    with pytest.raises(B.LandauError) as e:
-        gf.entropy_grad(v, w, sid)
-    assert e.value.code == B.ERANGE
+    for forced in (2, 3):
+        gf = B.Landau(mass, charge, eps, entropy_kernel=forced)
+        with pytest.raises(B.LandauError) as e:
+            gf.entropy_grad(v, w, sid)
+        assert e.value.code == B.ERANGE
     # just inside the limit the factorised kernel still agrees with the oracle (largest table entries)
     v2 = 0.3 * rng.standard_normal((n, 3))
     v2[n // 2:, 1] += 0.9 * 2.0 * (500.0 / (6.0 * 1.6506801238857844)) * np.sqrt(2 * 0.05)
     Gref2, _ = o.entropy_grad(v2, w, sid, with_entropy=True)
-    Ggot2, _ = gf.entropy_grad(v2, w, sid, with_entropy=True)
-    assert "entropy=fact" in gf.last_kernels()
-    assert_field_close(Ggot2.cpu().numpy(), Gref2, sid, 1, what="entropy gradient (near limit)")
+    for forced, name in ((2, "fact"), (3, "mma")):
+        gf = B.Landau(mass, charge, eps, entropy_kernel=forced)
+        Ggot2, _ = gf.entropy_grad(v2, w, sid, with_entropy=True)
+        assert f"entropy={name}" in gf.last_kernels()
+        assert_field_close(Ggot2.cpu().numpy(), Gref2, sid, 1, what=f"entropy gradient (near limit, {name})")
 
 
 # ------------------------------------------------------------------------------------ full field
