@@ -116,22 +116,24 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
                      rec + ((size_t)src0 + (size_t)(t0 + k) * MMA_TILE) * REC, BYTES, &s_bar[k & 1]);
         }
     };
+    // product-table builder: lane = node (conflict-free: a warp reads <= NQ distinct factors of ONE record per
+    // load and writes 32 consecutive doubles of one row), the block's two warp pairs take alternate sources
+    const int be = tid & 63, bq = tid >> 6;
+    const int bnd = node0 + be;
+    const bool bvalid = be < NL && bnd < M;
+    const int oi = 4 + (bvalid ? bnd / (NQ * NQ) : 0), oj = 4 + NQ + (bvalid ? (bnd / NQ) % NQ : 0),
+              ol = 4 + 2 * NQ + (bvalid ? bnd % NQ : 0);
     auto build = [&](int k) {                                        // records of tile k -> product table k & 1
         mbar_wait(&s_bar[k & 1], (uint32_t)(k >> 1) & 1u);
-        const int q = tid >> 1, half = tid & 1;
-        const double* r = s_rec + (size_t)(k & 1) * MMA_TILE * REC + q * REC;
-        double* row = s_prod + ((size_t)(k & 1) * MMA_TILE + q) * MMA_ROW;
-        if (half == 0) {
-            *reinterpret_cast<double2*>(row + 64) = *reinterpret_cast<const double2*>(r);
-            *reinterpret_cast<double2*>(row + 66) = *reinterpret_cast<const double2*>(r + 2);
-        }
-#pragma unroll
-        for (int e = 0; e < NL / 2; ++e) {
-            const int local = half * (NL / 2) + e;
-            const int nd = node0 + local;
-            double v = 0.0;
-            if (nd < M) v = r[4 + nd / (NQ * NQ)] * r[4 + NQ + (nd / NQ) % NQ] * r[4 + 2 * NQ + nd % NQ];
-            row[local] = v;
+        const double* r = s_rec + (size_t)(k & 1) * MMA_TILE * REC + bq * REC;
+        double* row = s_prod + ((size_t)(k & 1) * MMA_TILE + bq) * MMA_ROW;
+#pragma unroll 8
+        for (int qi = 0; qi < MMA_TILE / 2; ++qi) {
+            const double v = r[oi] * r[oj] * r[ol];
+            if (be < NL) row[be] = bvalid ? v : 0.0;
+            if (be < 4) row[64 + be] = r[be];
+            r += 2 * REC;
+            row += 2 * MMA_ROW;
         }
     };
 
