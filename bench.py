@@ -189,6 +189,22 @@ def config_dict(args, wl, iters=None):
     return d
 
 
+def aggregate_over_ranks(times, pairs):
+    """Contract of the multi-rank line ("replicas only"): time = MAX over ranks, work = SUM
+    over ranks.  `times` / `pairs` are tensors on the backend's device (cuda for nccl, cpu for gloo); a
+    no-op without an initialised process group.  Covered on CPU by tests/test_bench_multirank.py (gloo)."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(pairs, op=dist.ReduceOp.SUM)
+    return times.tolist(), pairs.tolist()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/r1_pair_sym_v2_full.md: 475 MB + 401 MB), valid for that workload only
+NCU_TRAFFIC_BYTES = {("c4_2e16", "sym"): 876e6}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -277,11 +293,7 @@ def run_ours(args):
 
     times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
     pairs = torch.tensor([float(iters_total) * N * (N - 1), float(it_h) * N * (N - 1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-        dist.all_reduce(pairs, op=dist.ReduceOp.SUM)
-    t_dev_max, t_e2e_max = times.tolist()
-    pairs_dev, pairs_e2e = pairs.tolist()
+    (t_dev_max, t_e2e_max), (pairs_dev, pairs_e2e) = aggregate_over_ranks(times, pairs)
 
     if rank == 0:
         value = pairs_dev / t_dev_max
@@ -290,7 +302,10 @@ def run_ours(args):
         achieved = FLOPS_PER_PAIR * N * (N - 1) / pair_s / 1e12
         peak_meas = g.fp64_peak(5) / 1e12
         roofline = {"bound": "alu", "kernel": g.last_kernels(), "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12,
-                    "unit": "TFLOP/s", "frac": achieved / (FP64_PEAK_NOMINAL / 1e12), "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / (FP64_PEAK_NOMINAL / 1e12),
+                    "traffic": NCU_TRAFFIC_BYTES.get((args.workload, "sym" if "pair=sym" in g.last_kernels() else "")),
+                    "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                    "algorithmic_bytes": 56.0 * N + 24.0 * N,
                     "peak_source": "nominal FP64 FMA rate 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                    "MEASURED_PEAKS.json has no FP64 figure",
                     "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
