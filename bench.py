@@ -331,6 +331,26 @@ def run_ours(args):
                 "e2e": {"value": pairs_e2e / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e_max / args.steps},
                 "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        if args.workload.startswith("c4"):
+            # BASELINE config 4: "plus an FP32 field variant" -- pass 2 alone, FP32 arithmetic, vs the FP64 kernel
+            G = g.entropy_grad(v_d, w_d, s_d)
+            V64 = g.pair_field(v_d, w_d, s_d, G)
+            g32 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, precision=1)
+            V32 = g32.pair_field(v_d, w_d, s_d, G)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(3):
+                g32.pair_field(v_d, w_d, s_d, G)
+            e1.record()
+            torch.cuda.synchronize()
+            t32 = e0.elapsed_time(e1) * 1e-3 / 3
+            sid_t = s_d.long()
+            err = [float(torch.linalg.norm((V32 - V64)[sid_t == k]) / torch.linalg.norm(V64[sid_t == k]))
+                   for k in range(wl.n_species)]
+            line["fp32_field_variant"] = {"kernels": g32.last_kernels(), "pairs_per_s": N * (N - 1) / t32,
+                                          "ms_per_eval": 1e3 * t32, "includes": "pack + pair kernel + combine",
+                                          "rel_l2_vs_fp64_per_species": err}
+            del g32
         if not args.no_cpu_baseline and world == 1:
             _, info, _ = oracle_sample(wl, max(1, round(iters_total / args.steps)), args.cpu_seconds, args.workload)
             line["cpu_baseline"] = info

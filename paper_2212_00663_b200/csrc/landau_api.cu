@@ -429,6 +429,22 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
         RC(launch_pair_sym(c, cl, ctrl, nparts_out));
         return 0;
     }
+    if (c->precision == 1 && !ctrl) {                       // FP32 field variant (never inside the implicit step)
+        constexpr int RF = 4;
+        const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * RF);
+        const int stiles = cl.npad_max / PAIR_SRC_TILE;
+        int nchunks = std::max(1, std::min(stiles, ceil_div(8 * c->sm_count, ttiles)));
+        nchunks = std::min(nchunks, 32);
+        RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
+        dim3 grid(ttiles, nchunks);
+        pair_onesided_f32_kernel<RF><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
+                                                                        cl.recs(), (double*)c->vpart.p);
+        c->k_pair = "onesided_f32";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+        c->launches += 1;
+        *nparts_out = nchunks;
+        return 0;
+    }
     constexpr int R = 2;
     const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * R);
     const int stiles = cl.npad_max / PAIR_SRC_TILE;

@@ -106,6 +106,93 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
     }
 }
 
+// FP32 variant of the one-sided kernel (BASELINE config 4, "plus an FP32 field variant"; landau_opts.precision = 1,
+// field evaluation only, never the implicit step).  Same tiling; records are converted to FP32 while they are
+// staged into shared memory, every per-pair operation (differences included) is FP32 on the FMA pipe with
+// MUFU.RSQ + one Newton step, the per-tile sums (128 sources) are FP32, and tiles are accumulated in FP64.
+// A pair whose FP32 separation underflows (|z|^2 < 1e-30) contributes 0 (reading S5 in FP32).
+// Expected error vs the FP64 oracle: ~1e-6 relative L2 (tests/test_gpu_parity.py, bench.py report it).
+template <int R>
+__global__ void __launch_bounds__(PAIR_THREADS)
+pair_onesided_f32_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
+                         const double* __restrict__ rec, double* __restrict__ vpart) {
+    const int npad = L->npad;
+    const int slot0 = blockIdx.x * (PAIR_THREADS * R);
+    if (slot0 >= npad) return;
+    const int S = T->S;
+    __shared__ float4 sa[PAIR_SRC_TILE], sb[PAIR_SRC_TILE];
+    __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
+    for (int i = threadIdx.x; i < S * S; i += PAIR_THREADS) s_nu[i] = T->nu[i];
+
+    float px[R], py[R], pz[R], gx[R], gy[R], gz[R];
+    double tx[R], ty[R], tz[R];
+    int sp[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        int p = slot0 + r * PAIR_THREADS + threadIdx.x;
+        if (p >= npad) p = npad - 1;
+        const double2* rp = reinterpret_cast<const double2*>(rec + (size_t)p * 8);
+        const double2 a = rp[0], b = rp[1], c = rp[2], d = rp[3];
+        px[r] = (float)a.x; py[r] = (float)a.y; pz[r] = (float)b.x;
+        gx[r] = (float)c.x; gy[r] = (float)c.y; gz[r] = (float)d.x;
+        tx[r] = ty[r] = tz[r] = 0.0;
+        sp[r] = species_of_slot(L, S, p);
+    }
+    const int ntiles = npad / PAIR_SRC_TILE;
+    const int tpc = ceil_div(ntiles, nchunks);
+    const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
+    for (int t = t0; t < t1; ++t) {
+        __syncthreads();
+        {
+            const double2* src = reinterpret_cast<const double2*>(rec + ((size_t)t * PAIR_SRC_TILE + threadIdx.x) * 8);
+            const double2 a = src[0], b = src[1], c = src[2], d = src[3];
+            sa[threadIdx.x] = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+            sb[threadIdx.x] = make_float4((float)c.x, (float)c.y, (float)d.x, 0.f);
+        }
+        __syncthreads();
+        const int sbs = species_of_slot(L, S, t * PAIR_SRC_TILE);
+        float ax[R], ay[R], az[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) ax[r] = ay[r] = az[r] = 0.f;
+#pragma unroll 4
+        for (int j = 0; j < PAIR_SRC_TILE; ++j) {
+            const float4 a = sa[j], b = sb[j];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float zx = px[r] - a.x, zy = py[r] - a.y, zz = pz[r] - a.z;
+                const float cx = gx[r] - b.x, cy = gy[r] - b.y, cz = gz[r] - b.z;
+                const float r2 = fmaf(zz, zz, fmaf(zy, zy, zx * zx));
+                const float d = fmaf(zz, cz, fmaf(zy, cy, zx * cx));
+                float y = rsqrtf(fmaxf(r2, 1e-30f));
+                y = y * fmaf(-0.5f * r2 * y, y, 1.5f);            // one Newton step
+                y = r2 < 1e-30f ? 0.f : y;
+                const float h = d * (y * y);
+                const float wy = a.w * y;
+                ax[r] = fmaf(wy, fmaf(-zx, h, cx), ax[r]);
+                ay[r] = fmaf(wy, fmaf(-zy, h, cy), ay[r]);
+                az[r] = fmaf(wy, fmaf(-zz, h, cz), az[r]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double nu = s_nu[sp[r] * S + sbs];
+            tx[r] = fma(nu, (double)ax[r], tx[r]); ty[r] = fma(nu, (double)ay[r], ty[r]);
+            tz[r] = fma(nu, (double)az[r], tz[r]);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int p = slot0 + r * PAIR_THREADS + threadIdx.x;
+        if (p < npad) {
+            const double im = T->inv_mass[sp[r]];
+            double* o = vpart + (size_t)blockIdx.y * 3 * (size_t)npad_max + p;
+            o[0] = tx[r] * im;
+            o[(size_t)npad_max] = ty[r] * im;
+            o[2 * (size_t)npad_max] = tz[r] * im;
+        }
+    }
+}
+
 // {x,y,z,w,G} (packed SoA) -> source records with g = G/m_s.
 __global__ void build_rec_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                                  int npad_max, const double* __restrict__ x, const double* __restrict__ y,

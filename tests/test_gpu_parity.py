@@ -154,6 +154,27 @@ def test_wide_cloud_takes_the_literal_kernel(B, oracle_mod):
         assert_field_close(Ggot2.cpu().numpy(), Gref2, sid, 1, what=f"entropy gradient (near limit, {name})")
 
 
+def test_fp32_pair_field_variant(B, oracle_mod):
+    """BASELINE config 4's FP32 field variant (landau_opts.precision = 1): FP32 arithmetic inside the pairwise
+    sum only.  Tolerance 2e-5 relative L2 per species: 24-bit differences of O(1) velocities against pair
+    separations down to ~1e-3 of the thermal speed, summed over N sources with random signs."""
+    wl = W.make(4, n_per_species=1500, shuffled=True)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    G = o.entropy_grad(wl.v, wl.w, wl.species_id)
+    Vref = o.pair_field(wl.v, wl.w, wl.species_id, G)
+    g32 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, precision=1)
+    V32 = g32.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    assert "pair=onesided_f32" in g32.last_kernels()
+    assert_field_close(V32, Vref, wl.species_id, wl.n_species, tol=2e-5, what="FP32 pair field")
+    assert rel_l2(V32, Vref) > 1e-9, "the FP32 variant must really compute in FP32"
+    # the whole field through the FP32 variant (pass 1 stays FP64), and the step ignores the flag
+    Vf = g32.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(Vf, Vref, wl.species_id, wl.n_species, tol=2e-5, what="FP32 field")
+    g32.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = g32.step(1e-3, 1e-12, 50)
+    assert rc == 0 and conv and "f32" not in g32.last_kernels()
+
+
 # ------------------------------------------------------------------------------------ full field
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS)
 @pytest.mark.parametrize("cfg,n", [(0, 256), (2, 500), (4, 384)])
