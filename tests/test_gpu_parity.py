@@ -375,3 +375,16 @@ def test_eval_field_does_not_touch_held_markers(B):
     other = W.make(0, n_per_species=333, seed=9, shuffled=True)
     g.eval_field(other.v, other.w, other.species_id)
     np.testing.assert_array_equal(g.get_markers().cpu().numpy(), wl.v)
+
+
+def test_history_runner_reduced_config2(B):
+    """paper_2212_00663_b200.histories on a reduced config 2: conservation per step, anisotropy decays,
+    S_eps does not decrease (north_star: multi-step runs are compared by moment / temperature histories)."""
+    from paper_2212_00663_b200 import histories
+    wl, H, summary = histories.run_history(2, n_per_species=768, steps=25)
+    assert summary["steps_not_converged"] == 0
+    assert summary["energy_drift_rel_per_step_max"] <= TOL_DRIFT and summary["momentum_drift_rel_max"] <= TOL_DRIFT
+    an = summary["anisotropy"]
+    assert 0 < an["last"] < an["first"] and an["fitted_rate"] < 0
+    assert summary["S_eps_monotone"]
+    assert H["T"].shape == (26, 2) and H["kurt"].shape == (26, 2, 3)
