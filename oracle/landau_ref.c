@@ -422,6 +422,85 @@ int landau_ref_step(landau_ref_ctx* c, double dt, double tol, int max_iter, land
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O4b  Discrete-gradient step, Eqs. (46)-(49), SURVEY.md NEXT-1.
+ *   Gamma(K, p, q): the discrete gradient of the quadratic K is its midpoint gradient,
+ *       (1/(m_s w_p)) dK/dv_p = (v_p^n + v_p^{n+1})/2 = u_p, so Q is evaluated at u_p - u_q as in Eq. (24).
+ *   Gamma(S_eps, p, q): the paper leaves the discrete gradient open ("many existing options"); reading
+ *   DG1 takes Gonzalez' midpoint discrete gradient (the paper's ref. [39]) in the Euclidean
+ *   inner product of all 3N velocity components:
+ *       dbar S/dv_p = w_p G_p(u) + lambda (v_p^{n+1} - v_p^n),
+ *       lambda = [ S(v^{n+1}) - S(v^n) - sum_p w_p G_p(u).(v_p^{n+1} - v_p^n) ] / sum_p |v_p^{n+1} - v_p^n|^2
+ *   (lambda = 0 when v^{n+1} = v^n), which satisfies Eq. (48) identically; S = sum_s S_eps,s.
+ *   The step solves  v^{n+1} = v^n + dt * O3(u; Gbar),  Gbar_p = (1/w_p) dbar S/dv_p,  by the Jacobi
+ *   fixed point of O4 with Gbar re-evaluated from (v^n, v^(k)) in every iteration.
+ * ------------------------------------------------------------------------------------------ */
+int landau_ref_step_dg(landau_ref_ctx* c, double dt, double tol, int max_iter, landau_ref_step_info* info) {
+    if (!c || !c->v || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0)) return -1;
+    const int64_t N = c->N;
+    const size_t B3 = sizeof(double) * 3 * (size_t)N;
+    double* G = (double*)malloc(B3);
+    double* Gb = (double*)malloc(B3);
+    double* vk = (double*)malloc(B3);
+    double* u = (double*)malloc(B3);
+    double* V = (double*)malloc(B3);
+    double Ss[64];
+    if (!G || !Gb || !vk || !u || !V || c->S > 64) { free(G); free(Gb); free(vk); free(u); free(V); return -2; }
+    int rc = landau_ref_entropy_grad(c, N, c->v, c->w, c->sid, G, Ss);
+    long double S0 = 0.0L;
+    for (int s = 0; s < c->S; ++s) S0 += Ss[s];
+    int iters = 0, converged = 0;
+    double res = INFINITY;
+    if (rc == 0) {
+        memcpy(vk, c->v, B3);
+        for (int k = 0; k < max_iter; ++k) {
+            for (int64_t i = 0; i < 3 * N; ++i) u[i] = 0.5 * (c->v[i] + vk[i]);
+            long double lambda = 0.0L;
+            if (k > 0) {
+                rc = landau_ref_entropy_grad(c, N, u, c->w, c->sid, G, NULL);          /* G(u)      */
+                if (rc) break;
+                rc = landau_ref_entropy_grad(c, N, vk, c->w, c->sid, Gb, Ss);           /* S(v^(k))  */
+                if (rc) break;
+                long double Sk = 0.0L, lin = 0.0L, dv2 = 0.0L;
+                for (int s = 0; s < c->S; ++s) Sk += Ss[s];
+                for (int64_t p = 0; p < N; ++p)
+                    for (int d = 0; d < 3; ++d) {
+                        const long double dv = (long double)vk[3 * p + d] - c->v[3 * p + d];
+                        lin += (long double)c->w[p] * G[3 * p + d] * dv;
+                        dv2 += dv * dv;
+                    }
+                if (dv2 > 0.0L) lambda = (Sk - S0 - lin) / dv2;
+            }
+            for (int64_t p = 0; p < N; ++p)
+                for (int d = 0; d < 3; ++d)
+                    Gb[3 * p + d] = (double)(G[3 * p + d]
+                                             + lambda * ((long double)vk[3 * p + d] - c->v[3 * p + d]) / c->w[p]);
+            rc = landau_ref_pair_field(c, N, u, c->w, c->sid, Gb, V);
+            if (rc) break;
+            long double num = 0.0L, den = 0.0L;
+            for (int64_t p = 0; p < N; ++p) {
+                const long double wm = (long double)c->w[p] * c->mass[c->sid[p]];
+                for (int d = 0; d < 3; ++d) {
+                    const double vn = c->v[3 * p + d] + dt * V[3 * p + d];
+                    const long double diff = (long double)vn - vk[3 * p + d];
+                    num += wm * diff * diff;
+                    den += wm * (long double)vn * vn;
+                    vk[3 * p + d] = vn;
+                }
+            }
+            res = (double)sqrtl(num / den);
+            iters = k + 1;
+            if (!isfinite(res)) { rc = -4; break; }
+            if (res <= tol) { converged = 1; break; }
+        }
+    }
+    if (rc == 0) memcpy(c->v, vk, B3);
+    free(G); free(Gb); free(vk); free(u); free(V);
+    if (info) { info->iterations = iters; info->residual = res; info->converged = converged; }
+    if (rc) return rc;
+    return converged ? 0 : 1;
+}
+
+/* ------------------------------------------------------------------------------------------
  * O5  Moments (PAPER.md:151 Eq. 26, :162 Eq. 28, :191-193 Eq. 33, :118 Eq. 20):
  *   n_s = sum w_p,  P_s = m_s sum w_p v_p,  K_s = (m_s/2) sum w_p |v_p|^2,  S_eps,s as in O2.
  * ------------------------------------------------------------------------------------------ */

@@ -66,6 +66,10 @@ int landau_ref_get_markers(landau_ref_ctx* ctx, double* v_out);
 /* O4: one step of Eq. (24)-(25) by Jacobi fixed-point iteration. */
 int landau_ref_step(landau_ref_ctx* ctx, double dt, double tol, int max_iter,
                     landau_ref_step_info* info);
+/* O4b: one step of the discrete-gradient scheme, Eqs. (46)-(49), with Gonzalez' midpoint discrete
+ * gradient of S_eps (reading DG1); same fixed point, residual and status conventions as O4. */
+int landau_ref_step_dg(landau_ref_ctx* ctx, double dt, double tol, int max_iter,
+                       landau_ref_step_info* info);
 /* O5: n_s, P_s (S x 3), K_s, S_eps,s of the held markers; any output may be NULL. */
 int landau_ref_moments(landau_ref_ctx* ctx, double* n, double* P, double* K, double* S_eps);
 /* stress: S x 6 = m_s sum w v_i v_j in order xx,yy,zz,xy,xz,yz; m4: S x 3 = sum w (v_i-u_i)^4 */

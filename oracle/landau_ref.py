@@ -60,6 +60,7 @@ def _load():
     lib.landau_ref_set_markers.argtypes = [vp, C.c_int64, dp, dp, ip]
     lib.landau_ref_get_markers.argtypes = [vp, dp]
     lib.landau_ref_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
+    lib.landau_ref_step_dg.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_ref_moments.argtypes = [vp, dp, dp, dp, dp]
     lib.landau_ref_moments_ext.argtypes = [vp, dp, dp]
     _lib = lib
@@ -209,6 +210,14 @@ class LandauRef:
         rc = self._lib.landau_ref_step(self._h, float(dt), float(tol), int(max_iter), C.byref(info))
         if rc < 0:
             raise OracleError(rc, "step")
+        return rc, int(info.iterations), float(info.residual), bool(info.converged)
+
+    def step_dg(self, dt, tol=1e-12, max_iter=50):
+        """Discrete-gradient step, Eqs. (46)-(49) with Gonzalez' discrete gradient of S_eps (reading DG1)."""
+        info = StepInfo()
+        rc = self._lib.landau_ref_step_dg(self._h, float(dt), float(tol), int(max_iter), C.byref(info))
+        if rc < 0:
+            raise OracleError(rc, "step_dg")
         return rc, int(info.iterations), float(info.residual), bool(info.converged)
 
     def moments(self, with_entropy: bool = True):
