@@ -126,6 +126,14 @@ int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_ste
 int landau_run(landau_ctx* ctx, int n_steps, double dt, double tol, int max_iter,
                landau_step_info* info);
 
+/* one step of the discrete-gradient scheme, Eqs. (46)-(49), which adds
+ * guaranteed entropy monotonicity (Eq. 49) to the conservation laws of Eq. (24).  Q is taken at the
+ * midpoint (the discrete gradient of the quadratic K); the entropy gradient is Gonzalez' midpoint discrete
+ * gradient  dbar S/dv_p = w_p G_p(u) + lambda (v_p^{n+1} - v_p^n)  (reading DG1).  Same Jacobi fixed
+ * point, residual, status and info conventions as landau_step; every iteration costs two pass-1 and one
+ * pass-2 evaluations and the loop is driven from the host (three small read-backs per iteration). */
+int landau_step_dg(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
+
 /* Moments of the held markers, HOST outputs, any may be NULL:
  * n[S] = sum w (Eq. 33), P[S x 3] = m_s sum w v (Eq. 26), K[S] = (m_s/2) sum w |v|^2 (Eq. 28),
  * S_eps[S] = regularised entropy (Eq. 20; costs one pass 1). */

@@ -22,6 +22,7 @@
 #include "pair.cuh"
 #include "pair_sym.cuh"
 #include "step.cuh"
+#include "step_dg.cuh"
 
 using namespace landau;
 
@@ -76,6 +77,7 @@ struct landau_ctx {
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
+    Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
     // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
     bool prof_on = false;
@@ -640,7 +642,8 @@ void landau_destroy(landau_ctx* c) {
         release(cl->lay); release(cl->xyzw); release(cl->perm); release(cl->G); release(cl->rec); release(cl->soa);
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
-                   &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab})
+                   &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
+                   &c->dg_Gk, &c->dg_part})
         release(*b);
     delete c;
 }
@@ -815,6 +818,100 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
 
 int landau_step(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {
     return landau_run(c, 1, dt, tol, max_iter, info);
+}
+
+// NEXT-1: one discrete-gradient step (Eqs. 46-49; step_dg.cuh).  Host-driven loop: every iteration reads the
+// entropy sums, the lambda partials and the residual back (three small synchronisations against two pass-1 and
+// one pass-2 evaluations of work).
+int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {
+    if (!c) return LANDAU_EINVAL;
+    Cloud& cl = c->state;
+    if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step_dg: no markers held (landau_set_markers first)");
+    if (max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
+        return fail(c, LANDAU_EINVAL, "step_dg: need max_iter >= 1, dt > 0, tol >= 0");
+    const int npm = cl.npad_max;
+    const size_t B4 = sizeof(double) * 4 * (size_t)npm;
+    RC(ensure(c, c->vk, B4));
+    RC(ensure(c, c->dg_u, B4));
+    RC(ensure(c, c->dg_Gu, B4));
+    RC(ensure(c, c->dg_Gk, B4));
+    RC(ensure(c, c->records, sizeof(StepRecord)));
+    const int nub = ceil_div(npm, UPD_THREADS), ndb = ceil_div(npm, DG_THREADS);
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(2 * nub, 4096)));
+    RC(ensure(c, c->dg_part, sizeof(double) * 2 * (size_t)ndb));
+    double* xk = (double*)c->vk.p;
+    double* yk = xk + npm;
+    double* zk = yk + npm;
+    cudaStream_t st = c->stream;
+    // cloud-shaped views that share the state's layout and permutation
+    Cloud U = cl;  U.xyzw = c->dg_u;  U.G = c->dg_Gu;        // midpoint u, G(u)
+    Cloud VK = cl; VK.xyzw = c->vk;   VK.G = c->dg_Gk;       // iterate v^(k), its entropy integrand
+    const double PI = 3.14159265358979323846;
+    double* hs = (double*)c->h_pin + 64;
+    auto total_entropy = [&](Cloud& q, double* S_out) -> int {
+        RC(species_sums(c, q, true, false, hs));
+        double S = 0.0;
+        for (int s = 0; s < c->S; ++s) S += -hs[s * MOM_OUT + 11] / (PI * sqrt(PI));
+        *S_out = S;
+        return 0;
+    };
+    CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
+    CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
+    c->prof_step = 0; c->prof_iter = 0;
+    RC(entropy(c, cl));                                       // G(v^n), entropy integrand at v^n
+    double S0 = 0.0;
+    RC(total_entropy(cl, &S0));
+    step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
+                                                           cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
+                                                           cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
+    CU(cudaMemcpyAsync(xk + 3 * (size_t)npm, cl.w(), sizeof(double) * (size_t)npm, cudaMemcpyDeviceToDevice, st));
+    c->launches += 1;
+    StepCtrl* hc = (StepCtrl*)c->h_pin;
+    std::vector<double> hp(2 * (size_t)ndb);
+    for (int k = 0; k < max_iter; ++k) {
+        int nparts = 0;
+        c->prof_iter = k;
+        if (k > 0) {
+            dg_midpoint_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), npm, cl.x(), cl.y(), cl.z(), cl.w(), xk, yk,
+                                                                    zk, U.x());
+            RC(entropy(c, U));
+            RC(entropy(c, VK));
+            double Sk = 0.0;
+            RC(total_entropy(VK, &Sk));
+            dg_lambda_partial_kernel<<<ndb, DG_THREADS, 0, st>>>(cl.L(), npm, cl.x(), cl.y(), cl.z(), cl.w(), xk, yk, zk,
+                                                                 U.Gx(), U.Gy(), U.Gz(), (double*)c->dg_part.p);
+            CU(cudaMemcpyAsync(hp.data(), c->dg_part.p, sizeof(double) * 2 * (size_t)ndb, cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            double lin = 0.0, dv2 = 0.0;
+            for (int b = 0; b < ndb; ++b) { lin += hp[2 * b]; dv2 += hp[2 * b + 1]; }
+            const double lambda = dv2 > 0.0 ? (Sk - S0 - lin) / dv2 : 0.0;
+            dg_build_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), npm, lambda, U.x(), cl.x(), cl.y(),
+                                                                 cl.z(), xk, yk, zk, U.Gx(), U.Gy(), U.Gz(),
+                                                                 cl.sym ? nullptr : cl.recs(),
+                                                                 cl.sym ? cl.soas() : nullptr);
+            c->launches += 3;
+        }
+        RC(pair(c, cl, c->d_ctrl, &nparts));
+        step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
+                                                         (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                         xk, yk, zk, cl.sym ? nullptr : cl.recs(),
+                                                         cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p);
+        c->launches += 1;
+        CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (hc->done) break;
+    }
+    step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk, zk,
+                                                            (StepRecord*)c->records.p, c->d_cursor);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    const int iterations = hc->iterations, converged = hc->converged, cerr = hc->err;
+    const double residual = hc->residual;
+    int rc = finish(c, cl, "step_dg");
+    if (rc < 0) return rc;
+    if (cerr) return fail(c, cerr, "step_dg: non-finite residual");
+    if (info) { info->iterations = iterations; info->residual = residual; info->converged = converged; }
+    return converged ? LANDAU_OK : LANDAU_NOT_CONVERGED;
 }
 
 int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps) {
