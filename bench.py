@@ -68,6 +68,9 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the oracle sample")
     ap.add_argument("--pair-kernel", type=int, default=0)
     ap.add_argument("--entropy-kernel", type=int, default=0)
+    ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi",
+                    help="fixed-point solver of Eq. (24): the paper's Jacobi iteration (default) or Anderson (NEXT-4)")
+    ap.add_argument("--anderson-depth", type=int, default=3)
     return ap.parse_args()
 
 
@@ -183,7 +186,9 @@ def config_dict(args, wl, iters=None):
          "step": "set_markers + landau_step (pass 1, fixed-point iterations of pass 2) + moments(S_eps) + get_markers",
          "l2": "inputs re-packed every step; pass-2 working set is L2-resident by design (56 B/marker); "
                "compute-bound path, cache state does not change the timing",
-         "parallelism": "replicas only" if args.gpus > 1 else "single GPU"}
+         "parallelism": "replicas only" if args.gpus > 1 else "single GPU",
+         "solver": "jacobi (paper)" if getattr(args, "solver", "jacobi") == "jacobi"
+                   else f"anderson depth {args.anderson_depth}"}
     if iters is not None:
         d["iterations_per_step"] = iters
     return d
@@ -224,6 +229,8 @@ def run_ours(args):
     N = wl.n_markers
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, pair_kernel=args.pair_kernel,
                  entropy_kernel=args.entropy_kernel)
+    if args.solver == "anderson":
+        g.set_solver(1, args.anderson_depth)
     dev = torch.device("cuda", local)
     v_d = torch.tensor(wl.v, device=dev); w_d = torch.tensor(wl.w, device=dev)
     s_d = torch.tensor(wl.species_id, device=dev)

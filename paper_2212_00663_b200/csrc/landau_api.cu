@@ -23,6 +23,7 @@
 #include "pair_sym.cuh"
 #include "step.cuh"
 #include "step_dg.cuh"
+#include "step_anderson.cuh"
 
 using namespace landau;
 
@@ -77,6 +78,9 @@ struct landau_ctx {
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
+    int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
+    AndersonCtrl* d_aa = nullptr;
+    Buf aa_hist;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
     // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
@@ -621,6 +625,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (cudaMalloc(&c->d_tab, sizeof(DevTable)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_aa, sizeof(AndersonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMallocHost(&c->h_pin, PIN_BYTES) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMemcpy(c->d_tab, &t, sizeof(t), cudaMemcpyHostToDevice) != cudaSuccess) return bail(LANDAU_ECUDA);
@@ -636,6 +641,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_tab) cudaFree(c->d_tab);
     if (c->d_ctrl) cudaFree(c->d_ctrl);
     if (c->d_cursor) cudaFree(c->d_cursor);
+    if (c->d_aa) cudaFree(c->d_aa);
     if (c->d_momout) cudaFree(c->d_momout);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     for (Cloud* cl : {&c->tmp, &c->state}) {
@@ -643,7 +649,7 @@ void landau_destroy(landau_ctx* c) {
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
-                   &c->dg_Gk, &c->dg_part})
+                   &c->dg_Gk, &c->dg_part, &c->aa_hist})
         release(*b);
     delete c;
 }
@@ -764,7 +770,8 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     RC(ensure(c, c->vk, sizeof(double) * 3 * (size_t)npm));
     RC(ensure(c, c->records, sizeof(StepRecord) * (size_t)n_steps));
     const int nub = ceil_div(npm, UPD_THREADS);
-    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(2 * nub, 4096)));
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(AA_NRED * nub, 4096)));
+    if (c->solver == 1) RC(ensure(c, c->aa_hist, sizeof(double) * (2 * (size_t)c->aa_depth + 2) * 3 * (size_t)npm));
     double* xk = (double*)c->vk.p;
     double* yk = xk + npm;
     double* zk = yk + npm;
@@ -778,6 +785,35 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
                                                                cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
                                                                cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
         c->launches += 1;
+        if (c->solver == 1) {
+            // NEXT-4: Anderson-accelerated fixed point (step_anderson.cuh); commits g(x_k) of the last evaluation
+            double* dF = (double*)c->aa_hist.p;
+            double* dG = dF + (size_t)c->aa_depth * 3 * npm;
+            double* fprev = dG + (size_t)c->aa_depth * 3 * npm;
+            double* gcur = fprev + 3 * (size_t)npm;
+            AndersonCtrl h_aa;
+            memset(&h_aa, 0, sizeof(h_aa));
+            h_aa.m = c->aa_depth;
+            CU(cudaMemcpyAsync(c->d_aa, &h_aa, sizeof(int) * 2, cudaMemcpyHostToDevice, st));
+            for (int k = 0; k < max_iter; ++k) {
+                int nparts = 0;
+                c->prof_iter = k;
+                RC(pair(c, cl, c->d_ctrl, &nparts));
+                anderson_update_kernel<<<nub, UPD_THREADS, 0, st>>>(
+                    c->d_tab, cl.L(), c->d_ctrl, c->d_aa, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p,
+                    cl.x(), cl.y(), cl.z(), cl.w(), xk, yk, zk, dF, dG, fprev, gcur, (double*)c->blockpart.p);
+                anderson_mix_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_aa, npm, cl.x(), cl.y(),
+                                                                         cl.z(), gcur, dG, xk, yk, zk,
+                                                                         cl.sym ? nullptr : cl.recs(),
+                                                                         cl.sym ? cl.soas() : nullptr);
+                c->launches += 2;
+            }
+            step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), gcur,
+                                                                    gcur + npm, gcur + 2 * (size_t)npm,
+                                                                    (StepRecord*)c->records.p, c->d_cursor);
+            c->launches += 1;
+            continue;
+        }
         for (int k = 0; k < max_iter; ++k) {
             int nparts = 0;
             c->prof_iter = k;
@@ -814,6 +850,16 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
         if (!h[n].converged) any_unconverged = 1;
     }
     return any_unconverged ? LANDAU_NOT_CONVERGED : LANDAU_OK;
+}
+
+int landau_set_solver(landau_ctx* c, int solver, int depth) {
+    if (!c) return LANDAU_EINVAL;
+    if (solver < 0 || solver > 1) return fail(c, LANDAU_EINVAL, "set_solver: solver must be 0 (Jacobi) or 1 (Anderson)");
+    if (solver == 1 && (depth < 1 || depth > AA_MAXM))
+        return fail(c, LANDAU_EINVAL, "set_solver: Anderson depth must be 1..%d", AA_MAXM);
+    c->solver = solver;
+    if (solver == 1) c->aa_depth = depth;
+    return 0;
 }
 
 int landau_step(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {

@@ -419,3 +419,53 @@ def test_dg_step_matches_oracle_and_conserves(B, oracle_mod, cfg, n, dt, tol, st
     assert abs(m1["K"].sum() - m0["K"].sum()) <= TOL_DRIFT * m0["K"].sum()
     assert np.all(np.diff(S_hist) >= -1e-13 * abs(S_hist[0]))
     np.testing.assert_allclose(m1["S_eps"], o.moments()["S_eps"], rtol=1e-10, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------ NEXT-4: Anderson solver
+@pytest.mark.parametrize("cfg,n,dt", [(0, 256, 0.01), (4, 384, 1e-3), (1, 1024, 0.02), (3, 9000, 0.01)])
+@pytest.mark.parametrize("depth", [1, 3, 5])
+def test_anderson_solver_reaches_the_same_step(B, oracle_mod, cfg, n, dt, depth):
+    """landau_set_solver(1, depth): the converged step solves the same Eq. (24) (unique fixed point, reading N4),
+    so it must agree with the oracle's plain Jacobi step to ~tol, conserve momentum and energy to 1e-12, and need
+    no more iterations than the Jacobi loop of the CUDA path."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    gj = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g.set_solver(1, depth)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    gj.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(dt, 1e-12, 60)
+    rcj, itj, resj, convj = gj.step(dt, 1e-12, 60)
+    assert rc == 0 and conv and rcj == 0 and convj
+    assert it <= itj, (it, itj)
+    v1 = g.get_markers().cpu().numpy()
+    if n <= 1024:
+        o.set_markers(wl.v, wl.w, wl.species_id)
+        rco, ito, reso, convo = o.step(dt, 1e-12, 60)
+        assert rco == 0 and convo
+        ref = o.get_markers()
+    else:
+        ref = gj.get_markers().cpu().numpy()
+    assert_field_close(v1, ref, wl.species_id, wl.n_species, tol=1e-11, what="Anderson state")
+    assert_field_close(v1 - wl.v, ref - wl.v, wl.species_id, wl.n_species, tol=1e-8, what="Anderson displacement")
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= TOL_DRIFT * m0["K"].sum()
+
+
+def test_anderson_momentum_conserved_when_not_converged(B):
+    wl = W.make(4, n_per_species=300, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g.set_solver(1, 3)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(1e-3, 1e-14, 3)
+    assert rc == 1 and not conv and it == 3
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    with pytest.raises(B.LandauError):
+        g.set_solver(1, 9)
+    g.set_solver(0)
