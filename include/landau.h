@@ -123,7 +123,7 @@ int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_ste
 
 /* how landau_step / landau_run solve Eq. (24).  solver 0 (default) = the paper's plain
  * Jacobi fixed-point iteration; solver 1 = the same fixed point with Anderson acceleration of the given
- * depth (1..5, 3 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the
+ * depth (1..10, 3 to 5 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the
  * stopping rule, status codes and conservation properties are unchanged; only the iterates between v^n and
  * the converged v^{n+1} differ.  Still device driven (no host synchronisation inside a step). */
 int landau_set_solver(landau_ctx* ctx, int solver, int depth);

@@ -238,7 +238,7 @@ class Landau:
         return rc, int(info.iterations), float(info.residual), bool(info.converged)
 
     def set_solver(self, solver: int = 0, depth: int = 3):
-        """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..5 (NEXT-4)."""
+        """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..10 (NEXT-4)."""
         self._check(self._lib.landau_set_solver(self._h, int(solver), int(depth)), "landau_set_solver")
 
     def step_dg(self, dt, tol=1e-12, max_iter=50):

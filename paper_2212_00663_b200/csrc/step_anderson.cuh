@@ -20,7 +20,7 @@
 
 namespace landau {
 
-constexpr int AA_MAXM = 5;
+constexpr int AA_MAXM = 10;
 constexpr int AA_NRED = 2 + 2 * AA_MAXM;    // num, den, b_j, a_j
 
 struct AndersonCtrl {
@@ -30,21 +30,22 @@ struct AndersonCtrl {
     double gamma[AA_MAXM];
 };
 
-// Solve the nc x nc system (Gaussian elimination with partial pivoting); returns false when it is numerically
-// singular relative to its diagonal.
+// Solve the nc x nc normal equations after scaling the columns to unit norm (Gaussian elimination with partial
+// pivoting); returns false when the scaled Gram matrix is numerically singular (nearly dependent columns).
 __device__ inline bool aa_solve(int nc, const double (*G)[AA_MAXM], const double* b, double* x) {
-    double A[AA_MAXM][AA_MAXM + 1];
-    double dmax = 0.0;
+    double A[AA_MAXM][AA_MAXM + 1], sc[AA_MAXM];
     for (int i = 0; i < nc; ++i) {
-        for (int j = 0; j < nc; ++j) A[i][j] = G[i][j];
-        A[i][nc] = b[i];
-        dmax = fmax(dmax, fabs(G[i][i]));
+        if (!(G[i][i] > 0.0) || !isfinite(G[i][i])) return false;
+        sc[i] = 1.0 / sqrt(G[i][i]);
     }
-    if (!(dmax > 0.0)) return false;
+    for (int i = 0; i < nc; ++i) {
+        for (int j = 0; j < nc; ++j) A[i][j] = G[i][j] * sc[i] * sc[j];
+        A[i][nc] = b[i] * sc[i];
+    }
     for (int c = 0; c < nc; ++c) {
         int piv = c;
         for (int r = c + 1; r < nc; ++r) if (fabs(A[r][c]) > fabs(A[piv][c])) piv = r;
-        if (!(fabs(A[piv][c]) > 1e-13 * dmax)) return false;
+        if (!(fabs(A[piv][c]) > 1e-10)) return false;
         if (piv != c) for (int j = c; j <= nc; ++j) { const double t = A[c][j]; A[c][j] = A[piv][j]; A[piv][j] = t; }
         for (int r = c + 1; r < nc; ++r) {
             const double f = A[r][c] / A[c][c];
@@ -56,7 +57,10 @@ __device__ inline bool aa_solve(int nc, const double (*G)[AA_MAXM], const double
         for (int j = c + 1; j < nc; ++j) s -= A[c][j] * x[j];
         x[c] = s / A[c][c];
     }
-    for (int c = 0; c < nc; ++c) if (!isfinite(x[c])) return false;
+    for (int c = 0; c < nc; ++c) {
+        x[c] *= sc[c];
+        if (!isfinite(x[c])) return false;
+    }
     return true;
 }
 
@@ -156,15 +160,24 @@ anderson_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
         if (!isfinite(res)) { ctrl->err = -4; ctrl->done = 1; }
         else if (res <= tol) { ctrl->converged = 1; ctrl->done = 1; }
         else if (it >= max_iter) ctrl->done = 1;
-        double gam[AA_MAXM] = {0, 0, 0, 0, 0};
+        double gam[AA_MAXM];
+        for (int j = 0; j < AA_MAXM; ++j) gam[j] = 0.0;
         if (nc > 0) {
             for (int j = 0; j < nc; ++j) { aa->gram[slot_new][j] = s_tot[2 + AA_MAXM + j]; aa->gram[j][slot_new] = s_tot[2 + AA_MAXM + j]; }
-            double rhs[AA_MAXM];
-            for (int j = 0; j < nc; ++j) rhs[j] = s_tot[2 + j];
-            if (!aa_solve(nc, aa->gram, rhs, gam)) {
-                for (int j = 0; j < AA_MAXM; ++j) gam[j] = 0.0;          // fall back to the newest column alone
-                const double d = aa->gram[slot_new][slot_new];
-                if (d > 0.0 && isfinite(rhs[slot_new] / d)) gam[slot_new] = rhs[slot_new] / d;
+            // least squares over the nu most recent columns, nu = nc, nc-1, ..., 1: the first window whose
+            // Gram matrix is numerically regular wins (old, nearly dependent columns are dropped first)
+            for (int nu = nc; nu >= 1; --nu) {
+                int slots[AA_MAXM];
+                double Gs[AA_MAXM][AA_MAXM], rhs[AA_MAXM], sol[AA_MAXM];
+                for (int a = 0; a < nu; ++a) slots[a] = ((slot_new - a) % m + m) % m;
+                for (int a = 0; a < nu; ++a) {
+                    rhs[a] = s_tot[2 + slots[a]];
+                    for (int b2 = 0; b2 < nu; ++b2) Gs[a][b2] = aa->gram[slots[a]][slots[b2]];
+                }
+                if (aa_solve(nu, Gs, rhs, sol)) {
+                    for (int a = 0; a < nu; ++a) gam[slots[a]] = sol[a];
+                    break;
+                }
             }
         }
         for (int j = 0; j < AA_MAXM; ++j) aa->gamma[j] = gam[j];

@@ -467,5 +467,5 @@ def test_anderson_momentum_conserved_when_not_converged(B):
     wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
     assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
     with pytest.raises(B.LandauError):
-        g.set_solver(1, 9)
+        g.set_solver(1, 11)
     g.set_solver(0)
