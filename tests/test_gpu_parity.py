@@ -93,6 +93,26 @@ def test_pair_field_full_size_sampled_rows(B, oracle_mod, pair_kernel):
     assert abs((wm * wl.v * got).sum()) <= 1e-13 * np.abs(wm * wl.v * got).sum()             # Eq. 29
 
 
+@pytest.mark.parametrize("nps,entropy_kernel", [(1 << 14, 3), (1 << 14, 2), (1 << 16, 3)])
+def test_entropy_grad_full_size_sampled_rows(B, oracle_mod, nps, entropy_kernel):
+    """Pass 1 at BASELINE config 4 sizes (up to the bench default 3 x 2^16) in the launch configuration
+    bench.py times: sampled target rows against the oracle (each row = 64 node sums over all same-species
+    sources), plus a property that holds at any size: G is invariant under a common translation of the
+    cloud (SURVEY.md O2 pin), which moves every marker relative to the factorisation centre and the origin."""
+    wl = W.make(4, n_per_species=nps, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl, entropy_kernel=entropy_kernel)
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert ("entropy=mma" if entropy_kernel == 3 else "entropy=fact") in g.last_kernels()
+    rng = np.random.default_rng(22)
+    rows = np.sort(np.concatenate([rng.choice(np.flatnonzero(wl.species_id == s), 24, replace=False)
+                                   for s in range(3)])).astype(np.int64)
+    ref = o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows)
+    assert_field_close(G[rows], ref, wl.species_id[rows], 3, what="entropy gradient (full size)")
+    shift = np.array([0.37, -1.9, 0.81])
+    G2 = g.entropy_grad(wl.v + shift, wl.w, wl.species_id).cpu().numpy()
+    assert_field_close(G2, G, wl.species_id, 3, tol=1e-9, what="entropy gradient (translated cloud)")
+
+
 # ------------------------------------------------------------------------------------ pass 1
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS)
 @pytest.mark.parametrize("cfg,n,n_q", [(0, 256, 4), (0, 97, 4), (4, 200, 4), (0, 64, 2), (0, 64, 3), (0, 48, 5),
