@@ -121,6 +121,13 @@ int landau_get_markers_host(landau_ctx* ctx, double* v_out /* host */);
  * Returns 0, or 1 if not converged (state still advanced; reading S8). */
 int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
 
+/* velocity-space dimension.  3 (default), or 2 = the paper's own 2-V setting (PAPER.md:110,
+ * 180): markers must be given with v_z = 0; the z-component of the entropy gradient, which cancels
+ * analytically by the antisymmetry of the Gauss-Hermite knots, is then stored as an exact zero, so that
+ * v_z = 0 is preserved exactly by every field evaluation and step (in 3-V arithmetic a round-off-sized G_z
+ * would seed the physical relaxation into v_z).  x/y results equal the 2-V Eqs. (22)-(24) (reading D1). */
+int landau_set_dimension(landau_ctx* ctx, int dim);
+
 /* how landau_step / landau_run solve Eq. (24).  solver 0 (default) = the paper's plain
  * Jacobi fixed-point iteration; solver 1 = the same fixed point with Anderson acceleration of the given
  * depth (1..10, 3 to 5 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the

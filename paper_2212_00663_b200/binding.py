@@ -24,7 +24,7 @@ EINVAL, ENOMEM, ECUDA, ENONFINITE, ERANGE = -1, -2, -3, -4, -5
 SYMBOLS = [
     "landau_default_opts", "landau_create", "landau_destroy", "landau_eval_field",
     "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
-    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver",
+    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_last_error",
@@ -80,6 +80,7 @@ def load(build_if_missing: bool = True):
     lib.landau_get_markers_host.argtypes = [vp, dp]
     lib.landau_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_set_solver.argtypes = [vp, C.c_int, C.c_int]
+    lib.landau_set_dimension.argtypes = [vp, C.c_int]
     lib.landau_step_dg.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_run.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_moments.argtypes = [vp, hd, hd, hd, hd]
@@ -240,6 +241,10 @@ class Landau:
     def set_solver(self, solver: int = 0, depth: int = 3):
         """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..10 (NEXT-4)."""
         self._check(self._lib.landau_set_solver(self._h, int(solver), int(depth)), "landau_set_solver")
+
+    def set_dimension(self, dim: int = 3):
+        """3 (default) or 2 = the paper's 2-V setting: v_z = 0 is preserved exactly (NEXT-2)."""
+        self._check(self._lib.landau_set_dimension(self._h, int(dim)), "landau_set_dimension")
 
     def step_dg(self, dt, tol=1e-12, max_iter=50):
         """Discrete-gradient step, Eqs. (46)-(49).  Returns as step()."""

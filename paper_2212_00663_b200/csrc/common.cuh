@@ -21,7 +21,7 @@ struct DevTable {
     int S;
     int n_q;
     int pad;                          // padding granularity of the packed layout (slots)
-    int _r0;
+    int dim;                          // 3 (default) or 2: 2-V mode, v_z = 0 is kept exactly (landau_set_dimension)
     double mass[LD_MAX_SPECIES];
     double inv_mass[LD_MAX_SPECIES];
     double eps[LD_MAX_SPECIES];

@@ -158,7 +158,9 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
     const double pref = -sqrt(2.0 / eps) / (PI * sqrt(PI));
     gx *= pref; gy *= pref; gz *= pref;
     if (!(isfinite(gx) && isfinite(gy) && isfinite(gz) && isfinite(sn))) atomicMin(&L->err, -4);
-    Gx[p] = gx; Gy[p] = gy; Gz[p] = gz; snode[p] = sn;
+    // 2-V mode (NEXT-2): with v_z = 0 the z-sum cancels analytically (knots are antisymmetric); storing an exact
+    // zero keeps the v_z = 0 manifold invariant (g_z = 0 => every pair term has u_z = 0 exactly)
+    Gx[p] = gx; Gy[p] = gy; Gz[p] = (T->dim == 2) ? 0.0 : gz; snode[p] = sn;
 }
 
 }  // namespace landau

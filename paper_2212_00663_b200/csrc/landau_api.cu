@@ -78,6 +78,7 @@ struct landau_ctx {
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
+    int dim = 3;                          // landau_set_dimension
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
     AndersonCtrl* d_aa = nullptr;
     Buf aa_hist;
@@ -614,7 +615,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     DevTable t;
     memset(&t, 0, sizeof(t));
-    t.S = S; t.n_q = c->n_q; t.pad = 128;
+    t.S = S; t.n_q = c->n_q; t.pad = 128; t.dim = 3;
     for (int s = 0; s < S; ++s) {
         t.mass[s] = mass[s]; t.inv_mass[s] = 1.0 / mass[s]; t.eps[s] = eps[s];
         t.inv_sqrt_2eps[s] = 1.0 / sqrt(2.0 * eps[s]);
@@ -850,6 +851,15 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
         if (!h[n].converged) any_unconverged = 1;
     }
     return any_unconverged ? LANDAU_NOT_CONVERGED : LANDAU_OK;
+}
+
+int landau_set_dimension(landau_ctx* c, int dim) {
+    if (!c) return LANDAU_EINVAL;
+    if (dim != 2 && dim != 3) return fail(c, LANDAU_EINVAL, "set_dimension: dim must be 2 or 3");
+    c->dim = dim;
+    CU(cudaMemcpyAsync(&c->d_tab->dim, &c->dim, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return 0;
 }
 
 int landau_set_solver(landau_ctx* c, int solver, int depth) {

@@ -1,0 +1,149 @@
+"""the paper's own numerical tests 3.1-3.3 on the CUDA path.
+
+    python -m paper_2212_00663_b200.paper_tests --test 3 [--n-grid 32] [--steps 100000] [--out DIR]
+
+The paper's tests are 2-V; they run here through the 3-V kernels with v_z = 0, which is exactly the paper's
+2-V scheme (reading D1; pinned in tests/test_oracle_quadrature_and_entropy.py).  Initial data,
+mollifier rule and time step are the paper's (workloads.paper_test: grid-initialised Maxwellians, Eqs. 34-35,
+eps_s = 1.2 (L_s/N)^1.98, dt = 1e-8 s); the marker count per species is not stated in the paper (n_grid^2 here).
+Steps run in chunks of `landau_run` (device-driven fixed point, one host sync per chunk); moments are sampled
+between chunks.  Output: DIR/paper_test<k>.csv (time in seconds, temperatures in eV, flows in m/s) and
+DIR/paper_test<k>.json with the numbers the paper prints next to its figures:
+
+  test 1 (Fig. 1)  temperature shift of species 1 vs Eq. (38), Delta T = m |u_1 - u_2|^2 / 8 (2-V);
+  test 2 (Fig. 2)  e-folding time of the electron flow vs the printed tau_r = 5.2e-6 s;
+  test 3 (Fig. 3)  isotropisation times tau_e, tau_i from the decay of T^x - T^y (Eqs. 42-43: rate 2/tau) vs
+                   Eq. (41) in its 2-V form and the printed 5.2e-6 s / 1.7e-4 s; thermalisation time from the decay
+                   of T_e - T_i vs Eqs. (44)-(45) and the printed 1.6e-3 s.
+Nothing here touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+from pathlib import Path
+
+import numpy as np
+
+from . import analytic as A
+from . import binding as B
+from . import workloads as W
+
+
+def _sample_plan(n_steps: int):
+    """Chunk lengths: every 10 steps for the first 3000 steps (electron time scale), then every 200."""
+    plan, done = [], 0
+    while done < n_steps:
+        c = 10 if done < 3000 else 200
+        c = min(c, n_steps - done)
+        plan.append(c)
+        done += c
+    return plan
+
+
+def run(test: int, n_grid: int = 32, steps=None, solver: int = 0, depth: int = 3, verbose: bool = False):
+    wl = W.paper_test(test, n_grid, n_steps=steps)
+    t0, v0, T0 = wl.notes["t0_seconds"], wl.notes["v0_m_per_s"], wl.notes["T0_eV"]
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g.set_dimension(2)
+    if solver:
+        g.set_solver(solver, depth)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    rows, iters, notconv = [], [], 0
+
+    def sample(step):
+        m = g.moments(with_entropy=True)
+        stress, _ = g.moments_ext()
+        tm = A.temperatures_from_moments(wl.mass, m["n"], m["P"], m["K"], stress)
+        rows.append(dict(t=step * wl.dt * t0, K=m["K"].copy(), P=m["P"].copy(), S=m["S_eps"].copy(),
+                         Tx=tm["T_axis"][:, 0] * T0, Ty=tm["T_axis"][:, 1] * T0, Tz=tm["T_axis"][:, 2] * T0,
+                         ux=tm["u"][:, 0] * v0, uy=tm["u"][:, 1] * v0))
+
+    wall0 = time.time()
+    sample(0)
+    done = 0
+    for c in _sample_plan(wl.n_steps):
+        rc, infos = g.run(c, wl.dt, wl.tol, wl.max_iter)
+        iters += [i[0] for i in infos]
+        notconv += sum(0 if i[2] else 1 for i in infos)
+        done += c
+        sample(done)
+        if verbose and done % 10000 == 0:
+            print(f"  step {done}/{wl.n_steps}  Tx {rows[-1]['Tx']}  Ty {rows[-1]['Ty']}", flush=True)
+    wall = time.time() - wall0
+    H = {k: np.array([r[k] for r in rows]) for k in rows[0]}
+    t = H["t"]
+    K = H["K"].sum(axis=1)
+    Pt = H["P"].sum(axis=1)
+    wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
+    T2 = 0.5 * (H["Tx"] + H["Ty"])                                  # 2-V species temperature
+    out = dict(test=test, name=wl.name, n_grid=n_grid, n_markers=wl.n_markers, steps=wl.n_steps,
+               dt_seconds=wl.dt * t0, t_end_seconds=float(t[-1]), t0_seconds=t0, eps=wl.eps.tolist(),
+               solver="jacobi" if not solver else f"anderson depth {depth}", wall_s=wall,
+               steps_per_s=wl.n_steps / wall, iterations_mean=float(np.mean(iters)), iterations_max=int(np.max(iters)),
+               steps_not_converged=int(notconv), energy_error_rel_max=float(np.abs(K - K[0]).max() / K[0]),
+               momentum_error_rel_max=float(np.abs(Pt - Pt[0]).max() / wm_abs),
+               Tz_max_eV=float(np.abs(H["Tz"]).max()), S_eps_first_last=[float(H["S"][0].sum()), float(H["S"][-1].sum())],
+               T_first_eV=T2[0].tolist(), T_last_eV=T2[-1].tolist())
+    coupling = A.coupling_from_nu(1.0)                              # nu = q^4 = 1 in normalised units
+    if test == 1:
+        du = np.array([H["ux"][0, 0] - H["ux"][0, 1], H["uy"][0, 0] - H["uy"][0, 1]]) / v0
+        out["fig1"] = dict(dT1_eV=float(T2[-1, 0] - T2[0, 0]), dT1_eq38_eV=float(T0 * (du ** 2).sum() / 8.0),
+                           printed_eV=125.0, u1_last_mps=[float(H["ux"][-1, 0]), float(H["uy"][-1, 0])],
+                           u_midpoint_eq37_mps=[float(0.5 * H["ux"][0].sum()), float(0.5 * H["uy"][0].sum())],
+                           K1_last_over_eq36=float(H["K"][-1, 0] / (0.5 * H["K"][0].sum())))
+    if test == 2:
+        du = H["ux"][:, 0] - H["ux"][:, 1]
+        sel = du > 0.05 * du[0]
+        out["fig2"] = dict(tau_r_fit_s=float(-1.0 / A.fit_exponential_rate(t[sel], du[sel])), printed_s=5.2e-6,
+                           ue_x_first_last=[float(H["ux"][0, 0]), float(H["ux"][-1, 0])])
+    if test == 3:
+        res = {}
+        for s, nm, printed in ((0, "e", 5.2e-6), (1, "i", 1.7e-4)):
+            gap = H["Tx"][:, s] - H["Ty"][:, s]
+            below = np.flatnonzero(gap <= 0.2 * gap[0])             # fit down to 20 % of the initial anisotropy
+            end = int(below[0]) if below.size else len(gap)
+            sel = np.arange(len(gap)) < max(end, 3)
+            rate = A.fit_exponential_rate(t[sel], gap[sel])
+            ana = A.isotropisation_rate_2v(wl.mass[s], 1.0, H["Tx"][0, s] / T0, H["Ty"][0, s] / T0, coupling) / t0
+            res[f"tau_{nm}_fit_s"] = float(-2.0 / rate)
+            res[f"tau_{nm}_eq41_2v_s"] = float(1.0 / ana)
+            res[f"tau_{nm}_printed_s"] = printed
+        gapT = T2[:, 0] - T2[:, 1]
+        late = t > 0.3 * t[-1]
+        rate = A.fit_exponential_rate(t[late], gapT[late])
+        ana = -A.temperature_gap_rate(wl.mass[0], wl.mass[1], 1.0, 1.0, T2[0, 0] / T0, T2[0, 1] / T0, coupling) / t0
+        res.update(tau_thermal_fit_s=float(-1.0 / rate), tau_gap_eq44_45_s=float(1.0 / ana), tau_thermal_printed_s=1.6e-3,
+                   Te_minus_Ti_first_last_eV=[float(gapT[0]), float(gapT[-1])])
+        out["fig3"] = res
+    return wl, H, out
+
+
+def write(outdir: Path, test: int, H, out, tag=""):
+    outdir.mkdir(parents=True, exist_ok=True)
+    S = H["Tx"].shape[1]
+    hdr = ["t_s", "K_total", "S_eps_total"] + [f"{q}_{s}" for q in ("Tx_eV", "Ty_eV", "ux_mps", "uy_mps", "K") for s in range(S)]
+    tab = np.column_stack([H["t"], H["K"].sum(axis=1), H["S"].sum(axis=1), H["Tx"], H["Ty"], H["ux"], H["uy"], H["K"]])
+    np.savetxt(outdir / f"paper_test{test}{tag}.csv", tab, delimiter=",", header=",".join(hdr), comments="")
+    (outdir / f"paper_test{test}{tag}.json").write_text(json.dumps(out, indent=1))
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--test", type=int, required=True, choices=[1, 2, 3])
+    ap.add_argument("--n-grid", type=int, default=32)
+    ap.add_argument("--steps", type=int, default=None, help="default: t_max/dt = 1e5 (PAPER.md:210-214)")
+    ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi")
+    ap.add_argument("--anderson-depth", type=int, default=3)
+    ap.add_argument("--out", default="gpurun_out")
+    ap.add_argument("--tag", default="")
+    args = ap.parse_args()
+    wl, H, out = run(args.test, args.n_grid, args.steps, 1 if args.solver == "anderson" else 0, args.anderson_depth,
+                     verbose=True)
+    write(Path(args.out), args.test, H, out, args.tag)
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

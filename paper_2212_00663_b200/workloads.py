@@ -228,3 +228,56 @@ def random_cloud(n_per_species, mass, charge, temperature, seed, drift=None,
                        w_raw=wr, T=float(temperature[k])))
     return _assemble("random_cloud", sp, rng, shuffled, dt=0.01, n_steps=1, seed=seed,
                      eps_rule=eps_rule)
+
+
+# ---------------------------------------------------------------------------------------------------
+# the paper's own 2-V tests, run through the 3-V path with
+# v_z = 0 (then the 3-V scheme IS the paper's 2-V scheme, reading D1).  Markers sit on an N x N mesh
+# of cell centres in [-L_s, L_s]^2, L_s = 5 v_t,s, with weights w_p = (2L/N)^2 f_s(v_p) of the (anisotropic,
+# drifting) Maxwellian of Eq. (34), normalised to n_s (Eq. 35); eps_s = 1.2 (L_s/N)^1.98 evaluated in SI
+# (PAPER.md:208).  Computation is in normalised units: velocity v0 = sqrt(T0/m_e), mass m_e, density n0,
+# time t0 = m_e^2 v0^3 (8 pi eps0^2)/(e^4 lnLambda n0), in which nu_ss' = q_s^2 q_s'^2 (reading U1) and k_B T0 = 1.
+E_CHARGE = 1.602176634e-19
+M_E_KG = 9.1093837015e-31
+EPS0 = 8.8541878128e-12
+PAPER_TESTS = {
+    # name, T0 [eV], lnLambda, species: (mass/m_e, charge, Tx/T0, Ty/T0, ux/v0, uy/v0)
+    1: ("E1_electron_positron", 1000.0, 16.0, [(1.0, -1.0, 1.0, 1.0, -1.0, 0.125), (1.0, +1.0, 1.0, 1.0, 0.0, -0.125)]),
+    2: ("E2_ei_velocity_relaxation", 400.0, 15.0, [(1.0, -1.0, 1.0, 1.0, 0.5, 0.0), (200.0, +1.0, 1.0, 1.0, 0.0, 0.0)]),
+    3: ("E3_eD_isotropisation", 400.0, 14.6, [(1.0, -1.0, 1.0, 0.75, 0.0, 0.0),
+                                              (3670.48, +1.0, 0.625, 0.5, 0.0, 0.0)]),
+}
+
+
+def paper_time_unit(T0_eV: float, lnLambda: float, n0: float = 1e20) -> float:
+    """Seconds per normalised time unit: t0 = m_e^2 v0^3 (8 pi eps0^2)/(e^4 lnLambda n0), v0 = sqrt(T0/m_e)."""
+    v0 = np.sqrt(T0_eV * E_CHARGE / M_E_KG)
+    return float(M_E_KG ** 2 * v0 ** 3 * 8.0 * np.pi * EPS0 ** 2 / (E_CHARGE ** 4 * lnLambda * n0))
+
+
+def paper_test(test: int, n_grid: int = 32, dt_seconds: float = 1e-8, n_steps: Optional[int] = None) -> Workload:
+    """One of the paper's tests 3.1-3.3 (E1-E3 of SURVEY.md section 2.4) as a Workload (deterministic: no rng)."""
+    name, T0, lnL, species = PAPER_TESTS[test]
+    v0 = np.sqrt(T0 * E_CHARGE / M_E_KG)
+    t0 = paper_time_unit(T0, lnL)
+    mass, charge, eps, vs, ws, ids = [], [], [], [], [], []
+    for k, (m, q, Tx, Ty, ux, uy) in enumerate(species):
+        vt = np.sqrt(0.5 * (Tx + Ty) / m)                        # thermal speed of the mean temperature, units of v0
+        L = 5.0 * vt
+        c = -L + (np.arange(n_grid) + 0.5) * (2.0 * L / n_grid)  # cell centres
+        X, Y = np.meshgrid(c, c, indexing="ij")
+        f = np.exp(-m * (X - ux) ** 2 / (2.0 * Tx) - m * (Y - uy) ** 2 / (2.0 * Ty))   # Eq. (34) up to its constant
+        w = (f / f.sum()).ravel()                                 # Eq. (35), normalised to n_s = 1
+        keep = w > 1e-300
+        v = np.stack([X.ravel()[keep], Y.ravel()[keep], np.zeros(int(keep.sum()))], axis=1)
+        w = w[keep] / w[keep].sum()
+        eps_si = 1.2 * (L * v0 / n_grid) ** 1.98                  # PAPER.md:208, in (m/s)^1.98 read as (m/s)^2
+        mass.append(m); charge.append(q); eps.append(eps_si / v0 ** 2)
+        vs.append(v); ws.append(w); ids.append(np.full(w.shape[0], k, dtype=np.int32))
+    dt = dt_seconds / t0
+    return Workload(name=name, mass=np.array(mass), charge=np.array(charge), density=np.ones(len(species)),
+                    eps=np.array(eps), v=np.ascontiguousarray(np.concatenate(vs)), w=np.concatenate(ws),
+                    species_id=np.concatenate(ids), dt=float(dt),
+                    n_steps=int(n_steps if n_steps is not None else round(1e-3 / dt_seconds)), tol=1e-12, max_iter=30,
+                    notes={"t0_seconds": t0, "v0_m_per_s": float(v0), "T0_eV": T0, "lnLambda": lnL, "n_grid": n_grid,
+                           "two_v": True, "species": species})

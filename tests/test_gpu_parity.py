@@ -489,3 +489,39 @@ def test_anderson_momentum_conserved_when_not_converged(B):
     with pytest.raises(B.LandauError):
         g.set_solver(1, 11)
     g.set_solver(0)
+
+
+# ------------------------------------------------------------------------------------ NEXT-2: the paper's 2-V setting
+def test_two_v_mode_keeps_vz_zero_and_matches_oracle(B, oracle_mod):
+    """landau_set_dimension(2) on the paper's test 3.3 initial data (grid-initialised anisotropic Maxwellians,
+    Eqs. 34-35, v_z = 0): v_z stays exactly 0 over many steps (in 3-V arithmetic a round-off G_z seeds the
+    physical relaxation into v_z), x/y agree with the oracle run on the same v_z = 0 data (reading D1), and the
+    conservation laws hold."""
+    wl = W.paper_test(3, n_grid=12)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_dimension(2)
+    V = g.eval_field(wl.v, wl.w, wl.species_id).cpu().numpy()
+    Vref = o.eval_field(wl.v, wl.w, wl.species_id)
+    assert np.all(V[:, 2] == 0.0) and np.abs(Vref[:, 2]).max() <= 1e-12 * np.abs(Vref).max()
+    assert_field_close(V[:, :2], Vref[:, :2], wl.species_id, wl.n_species, what="2-V field")
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, infos = g.run(40, wl.dt, 1e-12, 30)
+    assert rc == 0 and max(i[0] for i in infos) <= 10            # "5 to 10 iterations" (PAPER.md:210)
+    for _ in range(3):
+        assert o.step(wl.dt, 1e-12, 30)[0] == 0
+    v40 = g.get_markers().cpu().numpy()
+    assert np.all(v40[:, 2] == 0.0)
+    g3 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g3.set_dimension(2)
+    g3.set_markers(wl.v, wl.w, wl.species_id)
+    g3.run(3, wl.dt, 1e-12, 30)
+    assert_field_close(g3.get_markers().cpu().numpy()[:, :2], o.get_markers()[:, :2], wl.species_id, wl.n_species,
+                       tol=1e-11, what="2-V state after 3 steps")
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= 1e-11 * m0["K"].sum()
+    with pytest.raises(B.LandauError):
+        g.set_dimension(4)
