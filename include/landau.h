@@ -148,6 +148,28 @@ int landau_run(landau_ctx* ctx, int n_steps, double dt, double tol, int max_iter
  * pass-2 evaluations and the loop is driven from the host (three small read-backs per iteration). */
 int landau_step_dg(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
 
+/* many spatial collision cells in one call.  The bracket couples only markers of the same
+ * cell; a PIC code has thousands of small cells.  Markers of cell k are rows
+ * cell_offset[k] .. cell_offset[k+1]-1 of v / w / species_id (DEVICE arrays, any species order inside a cell;
+ * cell_offset is a HOST array of n_cells + 1 entries).  Every cell is advanced by n_steps steps of Eq. (24)
+ * (same Jacobi fixed point, residual, tolerance and readings as landau_step) by ONE kernel launch: one
+ * persistent thread block per cell with the cell's state in shared memory.  v_out (DEVICE, same layout, may
+ * alias v) receives the new velocities in caller order.  Limits: <= 1024 markers per cell, n_q <= 4.
+ * info (HOST, n_cells entries, may be NULL): per-cell status (0 ok, 1 = some step hit max_iter, < 0 = the
+ * cell was rejected and copied through unchanged: -1 invalid markers, -4 non-finite, -5 too wide for the
+ * factorised pass 1), iterations summed over the steps, the largest per-step count, and the last residual.
+ * Returns 0, 1 (some cell did not converge) or the most negative cell status. */
+typedef struct {
+    int status;
+    int iterations;
+    int max_iterations;
+    int steps_not_converged;
+    double residual;
+} landau_cell_info;
+int landau_cells_run(landau_ctx* ctx, int n_cells, const int64_t* cell_offset, const double* v, const double* w,
+                     const int32_t* species_id, double* v_out, int n_steps, double dt, double tol, int max_iter,
+                     landau_cell_info* info);
+
 /* Moments of the held markers, HOST outputs, any may be NULL:
  * n[S] = sum w (Eq. 33), P[S x 3] = m_s sum w v (Eq. 26), K[S] = (m_s/2) sum w |v|^2 (Eq. 28),
  * S_eps[S] = regularised entropy (Eq. 20; costs one pass 1). */

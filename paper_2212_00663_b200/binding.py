@@ -24,7 +24,7 @@ EINVAL, ENOMEM, ECUDA, ENONFINITE, ERANGE = -1, -2, -3, -4, -5
 SYMBOLS = [
     "landau_default_opts", "landau_create", "landau_destroy", "landau_eval_field",
     "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
-    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension",
+    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_cells_run",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_last_error",
@@ -36,6 +36,11 @@ class Opts(C.Structure):
     _fields_ = [("n_q", C.c_int), ("nu0", C.c_double), ("nu", C.POINTER(C.c_double)),
                 ("precision", C.c_int), ("stream", C.c_void_p), ("pair_kernel", C.c_int),
                 ("entropy_kernel", C.c_int), ("device", C.c_int)]
+
+
+class CellInfo(C.Structure):
+    _fields_ = [("status", C.c_int), ("iterations", C.c_int), ("max_iterations", C.c_int),
+                ("steps_not_converged", C.c_int), ("residual", C.c_double)]
 
 
 class StepInfo(C.Structure):
@@ -81,6 +86,8 @@ def load(build_if_missing: bool = True):
     lib.landau_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_set_solver.argtypes = [vp, C.c_int, C.c_int]
     lib.landau_set_dimension.argtypes = [vp, C.c_int]
+    lib.landau_cells_run.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                     C.POINTER(CellInfo)]
     lib.landau_step_dg.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_run.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
     lib.landau_moments.argtypes = [vp, hd, hd, hd, hd]
@@ -241,6 +248,26 @@ class Landau:
     def set_solver(self, solver: int = 0, depth: int = 3):
         """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..10 (NEXT-4)."""
         self._check(self._lib.landau_set_solver(self._h, int(solver), int(depth)), "landau_set_solver")
+
+    def cells_run(self, cell_offset, v, w, sid, n_steps, dt, tol=1e-12, max_iter=50, out=None, strict=True):
+        """Many collision cells in one launch (NEXT-3).  cell_offset: host int64 [n_cells + 1]; v, w, sid: the
+        markers of all cells (device tensors or arrays).  Returns (status, v_out tensor, info record array with
+        fields status / iterations / max_iterations / steps_not_converged / residual).  strict=False returns a
+        negative status (some cell was rejected and copied through) instead of raising; see info["status"]."""
+        off = np.ascontiguousarray(cell_offset, dtype=np.int64)
+        n_cells = int(off.shape[0] - 1)
+        v, w, sid, N = self._dev_in(v, w, sid)
+        if out is None:
+            out = self._torch.empty((N, 3), dtype=self._torch.float64, device=self._dev)
+        infos = (CellInfo * n_cells)()
+        rc = self._check(self._lib.landau_cells_run(self._h, n_cells, off.ctypes.data, v.data_ptr(), w.data_ptr(),
+                                                    sid.data_ptr(), out.data_ptr(), int(n_steps), float(dt),
+                                                    float(tol), int(max_iter), infos),
+                         "landau_cells_run", allow=(0, 1) if strict else (0, 1, EINVAL, ENONFINITE, ERANGE))
+        info = np.array([(i.status, i.iterations, i.max_iterations, i.steps_not_converged, i.residual) for i in infos],
+                        dtype=[("status", "i4"), ("iterations", "i4"), ("max_iterations", "i4"),
+                               ("steps_not_converged", "i4"), ("residual", "f8")])
+        return rc, out, info
 
     def set_dimension(self, dim: int = 3):
         """3 (default) or 2 = the paper's 2-V setting: v_z = 0 is preserved exactly (NEXT-2)."""

@@ -1,0 +1,329 @@
+// cells.cuh -- SURVEY.md section 8(f) NEXT-3: many spatial collision cells in one launch.
+//
+// The paper's bracket couples only markers of the same collision cell (indicator 1(p, p-bar)) and
+// "an efficient parallelization per each collision cell is elementary"; its tests use one cell
+// (PAPER.md:110).  A PIC code calls the operator with thousands of small cells (10^2..10^3 markers each), a
+// regime in which the large-N path of this library is bound by launch latency.  This kernel is the B200 answer
+// for that regime: ONE persistent CTA per cell, the cell's whole state resident in shared memory, and the
+// complete algorithm of Algorithm 1 for n_steps time steps inside a single launch:
+//   load + stable bucketing by species  ->  per step { pass 1 (Eq. 22, factorised form of entropy_fact.cuh)
+//   -> Jacobi fixed point of Eq. (24) with pass 2 (Eq. 23) per iteration, residual by a block reduction }
+//   -> write back in caller order.
+// No global-memory traffic, no kernel launch and no host synchronisation inside a step.  Cells are dealt to the
+// CTAs through an atomic counter (cells are independent, so results do not depend on the assignment).
+// Limits: markers per cell <= CELLS_CAP (shared memory), n_q <= 4; a cell that is too wide for the factorised
+// pass 1 (reading N3) reports LANDAU_ERANGE and is left unchanged.  Arithmetic, stopping rule and readings are
+// those of the single-cell path (S4, S5, S7, S8); tests compare every cell with the oracle.
+#pragma once
+#include "common.cuh"
+#include "entropy.cuh"
+#include "entropy_mma.cuh"   // exp_neg_tab
+#include "pair.cuh"          // pair_accumulate
+
+namespace landau {
+
+constexpr int CELLS_THREADS = 256;
+constexpr int CELLS_CAP = 1024;                 // markers per cell (all species)
+constexpr int CELLS_ROUNDS = CELLS_CAP / CELLS_THREADS;
+
+struct CellRecord {          // mirrors landau_cell_info (host struct) field by field
+    int status;              // 0 ok, 1 some step did not converge, < 0 error (cell left unchanged)
+    int iterations;          // fixed-point iterations, summed over the steps
+    int max_iterations;      // most iterations any step took
+    int steps_not_converged;
+    double residual;         // residual of the last step
+};
+
+template <int NQ>
+struct CellsCfg {
+    // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / ux uy uz (pass 2)
+    static constexpr int DPM = 10 + 3 * NQ;
+    static size_t smem(int cap) {
+        return sizeof(double) * ((size_t)DPM * cap + 64 + 32) + sizeof(int) * (size_t)cap;
+    }
+};
+
+// Fixed-order block sum of two values (warp shuffles, then warp 0 adds the warp totals in index order).
+__device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_red) {
+    a = warp_sum(a); b = warp_sum(b);
+    const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) { s_red[2 * wv] = a; s_red[2 * wv + 1] = b; }
+    __syncthreads();
+    double x = 0.0, y = 0.0;
+    for (int k = 0; k < CELLS_THREADS / 32; ++k) { x += s_red[2 * k]; y += s_red[2 * k + 1]; }
+    a = x; b = y;
+}
+
+template <int NQ>
+__global__ void __launch_bounds__(CELLS_THREADS, 1)
+cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const long long* __restrict__ cell_off,
+                 const double* __restrict__ v, const double* __restrict__ w, const int32_t* __restrict__ sid,
+                 double* __restrict__ v_out, int n_steps, double dt, double tol, int max_iter,
+                 int* __restrict__ next_cell, CellRecord* __restrict__ records) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* xn = reinterpret_cast<double*>(smem_raw);
+    double* yn = xn + cap; double* zn = yn + cap; double* ww = zn + cap;
+    double* Gx = ww + cap; double* Gy = Gx + cap; double* Gz = Gy + cap;
+    double* xk = Gz + cap; double* yk = xk + cap; double* zk = yk + cap;
+    double* tab = zk + cap;                               // [cap][3 NQ] in pass 1; ux uy uz in pass 2
+    double* ux = tab; double* uy = ux + cap; double* uz = uy + cap;
+    double* s_e2 = tab + (size_t)3 * NQ * cap;            // [64]
+    double* s_red = s_e2 + 64;                            // [32]
+    int* idx = reinterpret_cast<int*>(s_red + 32);        // [cap] caller index (within the cell) of slot p
+    __shared__ int s_off[LD_MAX_SPECIES + 1];
+    __shared__ int s_wcnt[CELLS_THREADS / 32];
+    __shared__ int s_cell, s_status;
+    __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
+
+    const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+    const int S = T->S;
+    if (tid < 64) s_e2[tid] = T->exp2_tab[tid];
+    for (int i = tid; i < S * S; i += CELLS_THREADS) s_nu[i] = T->nu[i];
+    double kn[NQ], ga[NQ];
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) { kn[i] = T->knot[i]; ga[i] = T->gw[i]; }
+    const double kmax = fabs(kn[NQ - 1]);
+    const double PI = 3.14159265358979323846;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) { s_cell = atomicAdd(next_cell, 1); s_status = 0; }
+        __syncthreads();
+        const int cell = s_cell;
+        if (cell >= n_cells) return;
+        const long long g0 = cell_off[cell];
+        const int n = (int)(cell_off[cell + 1] - g0);
+        CellRecord rec;
+        rec.status = 0; rec.iterations = 0; rec.max_iterations = 0; rec.steps_not_converged = 0; rec.residual = 0.0;
+        auto pass_through = [&]() {                                    // failed cell: output = input
+            if (v_out != v && n > 0)
+                for (long long i = tid; i < 3LL * n; i += CELLS_THREADS) v_out[3 * g0 + i] = v[3 * g0 + i];
+        };
+        if (n < 1 || n > cap) {
+            pass_through();
+            if (tid == 0) { rec.status = n == 0 ? 0 : -1; records[cell] = rec; }
+            continue;
+        }
+        // ---- load + stable bucketing by species (caller order preserved inside a species)
+        int base = 0;
+        for (int s = 0; s < S; ++s) {
+            if (tid == 0) s_off[s] = base;
+            for (int c0 = 0; c0 < n; c0 += CELLS_THREADS) {
+                const int i = c0 + tid;
+                int si = -2;
+                if (i < n) { si = sid[g0 + i]; if (si < 0 || si >= S) { si = -2; s_status = -1; } }
+                const bool mine = si == s;
+                const unsigned m = __ballot_sync(0xffffffffu, mine);
+                if (lane == 0) s_wcnt[wv] = __popc(m);
+                __syncthreads();
+                int before = 0, total = 0;
+                for (int k = 0; k < CELLS_THREADS / 32; ++k) { if (k < wv) before += s_wcnt[k]; total += s_wcnt[k]; }
+                if (mine) {
+                    const int p = base + before + __popc(m & ((1u << lane) - 1u));
+                    const double a = v[3 * (g0 + i)], b = v[3 * (g0 + i) + 1], c = v[3 * (g0 + i) + 2], wi = w[g0 + i];
+                    if (!(isfinite(a) && isfinite(b) && isfinite(c) && isfinite(wi))) s_status = -4;
+                    else if (!(wi > 0.0)) s_status = -1;
+                    xn[p] = a; yn[p] = b; zn[p] = c; ww[p] = wi; idx[p] = i;
+                }
+                base += total;
+                __syncthreads();
+            }
+        }
+        if (tid == 0) for (int s = S; s <= LD_MAX_SPECIES; ++s) s_off[s] = base;
+        __syncthreads();
+        if (s_status != 0 || base != n) {
+            pass_through();
+            if (tid == 0) { rec.status = s_status != 0 ? s_status : -1; records[cell] = rec; }
+            continue;
+        }
+        for (int step = 0; step < n_steps && s_status == 0; ++step) {
+            // ---- pass 1 (Eq. 22, factorised): G_p for every species, sources = same species of this cell
+            for (int s = 0; s < S; ++s) {
+                const int o0 = s_off[s], o1 = s_off[s + 1];
+                if (o0 == o1) continue;
+                const double eps = T->eps[s], inv = T->inv_sqrt_2eps[s];
+                // bounding box -> centre and half-width in mollifier units
+                double lo[3] = {1.7976931348623157e308, 1.7976931348623157e308, 1.7976931348623157e308};
+                double hi[3] = {-1.7976931348623157e308, -1.7976931348623157e308, -1.7976931348623157e308};
+                for (int p = o0 + tid; p < o1; p += CELLS_THREADS) {
+                    lo[0] = fmin(lo[0], xn[p]); hi[0] = fmax(hi[0], xn[p]);
+                    lo[1] = fmin(lo[1], yn[p]); hi[1] = fmax(hi[1], yn[p]);
+                    lo[2] = fmin(lo[2], zn[p]); hi[2] = fmax(hi[2], zn[p]);
+                }
+                double cen[3], hw = 0.0;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+                        hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+                    }
+                    __syncthreads();
+                    if (lane == 0) { s_red[2 * wv] = lo[d]; s_red[2 * wv + 1] = hi[d]; }
+                    __syncthreads();
+                    double a = s_red[0], b = s_red[1];
+                    for (int k = 1; k < CELLS_THREADS / 32; ++k) { a = fmin(a, s_red[2 * k]); b = fmax(b, s_red[2 * k + 1]); }
+                    cen[d] = 0.5 * a + 0.5 * b;
+                    hw = fmax(hw, 0.5 * b - 0.5 * a);
+                }
+                if (!(6.0 * kmax * hw * inv <= FACT_EXP_LIMIT)) { if (tid == 0) s_status = -5; break; }
+                // scaled coordinates (alias of xk..zk) and the per-marker exponential tables
+                for (int p = o0 + tid; p < o1; p += CELLS_THREADS) {
+                    const double a = (xn[p] - cen[0]) * inv, b = (yn[p] - cen[1]) * inv, c = (zn[p] - cen[2]) * inv;
+                    xk[p] = a; yk[p] = b; zk[p] = c;
+                    double* t = tab + (size_t)p * 3 * NQ;
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const double k2 = 2.0 * kn[i];
+                        t[i] = exp(k2 * a); t[NQ + i] = exp(k2 * b); t[2 * NQ + i] = exp(k2 * c);
+                    }
+                }
+                __syncthreads();
+                const double lognorm = -1.5 * log(2.0 * PI * eps);
+                const double pref = -sqrt(2.0 / eps) / (PI * sqrt(PI));
+                for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
+                    const int pt = r0 + tid;
+                    const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
+                    const double px = xk[p], py = yk[p], pz = zk[p];
+                    double acc[NQ][NQ][NQ];
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i)
+#pragma unroll
+                        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+                            for (int l = 0; l < NQ; ++l) acc[i][j][l] = 0.0;
+#pragma unroll 2
+                    for (int q = o0; q < o1; ++q) {
+                        const double dx = px - xk[q], dy = py - yk[q], dz = pz - zk[q];
+                        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                        const double c = ww[q] * exp_neg_tab(r2, s_e2);
+                        const double* t = tab + (size_t)q * 3 * NQ;
+                        double ty[NQ], tz[NQ];
+#pragma unroll
+                        for (int j = 0; j < NQ; ++j) { ty[j] = t[NQ + j]; tz[j] = t[2 * NQ + j]; }
+#pragma unroll
+                        for (int i = 0; i < NQ; ++i) {
+                            const double cx = c * t[i];
+#pragma unroll
+                            for (int j = 0; j < NQ; ++j) {
+                                const double cxy = cx * ty[j];
+#pragma unroll
+                                for (int l = 0; l < NQ; ++l) acc[i][j][l] = fma(cxy, tz[l], acc[i][j][l]);
+                            }
+                        }
+                    }
+                    double gx = 0.0, gy = 0.0, gz = 0.0;
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i)
+#pragma unroll
+                        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+                            for (int l = 0; l < NQ; ++l) {
+                                const double lnrho = lognorm + log(acc[i][j][l])
+                                                     - ((kn[i] * kn[i] + kn[j] * kn[j] + kn[l] * kn[l])
+                                                        + 2.0 * (kn[i] * px + kn[j] * py + kn[l] * pz));
+                                const double t = ga[i] * ga[j] * ga[l] * (1.0 + lnrho);
+                                gx = fma(t, kn[i], gx); gy = fma(t, kn[j], gy); gz = fma(t, kn[l], gz);
+                            }
+                    gx *= pref; gy *= pref; gz *= pref;
+                    if (pt < o1) {
+                        if (!(isfinite(gx) && isfinite(gy) && isfinite(gz))) s_status = -4;
+                        Gx[p] = gx; Gy[p] = gy; Gz[p] = (T->dim == 2) ? 0.0 : gz;
+                    }
+                }
+                __syncthreads();
+            }
+            __syncthreads();
+            if (s_status != 0) break;
+            // ---- Eq. (24): Jacobi fixed point, G^n frozen (g = G/m in place), v^(0) = v^n
+            int sp[CELLS_ROUNDS];
+            double im[CELLS_ROUNDS], wm[CELLS_ROUNDS];
+#pragma unroll
+            for (int r = 0; r < CELLS_ROUNDS; ++r) {
+                const int p = r * CELLS_THREADS + tid;
+                sp[r] = 0; im[r] = 0.0; wm[r] = 0.0;
+                if (p < n) {
+                    int s = 0;
+                    for (int t = 1; t < S; ++t) s += (p >= s_off[t]) ? 1 : 0;
+                    sp[r] = s; im[r] = T->inv_mass[s]; wm[r] = ww[p] * T->mass[s];
+                    Gx[p] *= im[r]; Gy[p] *= im[r]; Gz[p] *= im[r];
+                    xk[p] = xn[p]; yk[p] = yn[p]; zk[p] = zn[p];
+                    ux[p] = xn[p]; uy[p] = yn[p]; uz[p] = zn[p];
+                }
+            }
+            __syncthreads();
+            int it = 0, conv = 0;
+            double res = 0.0;
+            while (it < max_iter) {
+                double nx[CELLS_ROUNDS], ny[CELLS_ROUNDS], nz[CELLS_ROUNDS];
+                double num = 0.0, den = 0.0;
+#pragma unroll
+                for (int r = 0; r < CELLS_ROUNDS; ++r) {
+                    const int p = r * CELLS_THREADS + tid;
+                    nx[r] = ny[r] = nz[r] = 0.0;
+                    if (r * CELLS_THREADS < n) {                       // uniform: this round has targets
+                        const int pc = min(p, n - 1);
+                        const double px = ux[pc], py = uy[pc], pz = uz[pc];
+                        const double hx = Gx[pc], hy = Gy[pc], hz = Gz[pc];
+                        double tx = 0.0, ty = 0.0, tz = 0.0;
+                        for (int sb = 0; sb < S; ++sb) {
+                            const int q0 = s_off[sb], q1 = s_off[sb + 1];
+                            double ax = 0.0, ay = 0.0, az = 0.0;
+#pragma unroll 4
+                            for (int q = q0; q < q1; ++q)
+                                pair_accumulate(px - ux[q], py - uy[q], pz - uz[q], hx - Gx[q], hy - Gy[q], hz - Gz[q],
+                                                ww[q], ax, ay, az);
+                            const double nu = s_nu[sp[r] * S + sb];
+                            tx = fma(nu, ax, tx); ty = fma(nu, ay, ty); tz = fma(nu, az, tz);
+                        }
+                        if (p < n) {
+                            const double a = fma(dt, tx * im[r], xn[p]), b = fma(dt, ty * im[r], yn[p]),
+                                         c = fma(dt, tz * im[r], zn[p]);
+                            const double dx = a - xk[p], dy = b - yk[p], dz = c - zk[p];
+                            num += wm[r] * (dx * dx + dy * dy + dz * dz);
+                            den += wm[r] * (a * a + b * b + c * c);
+                            nx[r] = a; ny[r] = b; nz[r] = c;
+                        }
+                    }
+                }
+                cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
+#pragma unroll
+                for (int r = 0; r < CELLS_ROUNDS; ++r) {
+                    const int p = r * CELLS_THREADS + tid;
+                    if (p < n) {
+                        xk[p] = nx[r]; yk[p] = ny[r]; zk[p] = nz[r];
+                        ux[p] = 0.5 * (xn[p] + nx[r]); uy[p] = 0.5 * (yn[p] + ny[r]); uz[p] = 0.5 * (zn[p] + nz[r]);
+                    }
+                }
+                __syncthreads();
+                res = sqrt(num / den);
+                ++it;
+                if (!isfinite(res)) { if (tid == 0) s_status = -4; break; }
+                if (res <= tol) { conv = 1; break; }
+            }
+            __syncthreads();
+            if (s_status != 0) break;
+            // commit (also when not converged, reading S8)
+            for (int p = tid; p < n; p += CELLS_THREADS) { xn[p] = xk[p]; yn[p] = yk[p]; zn[p] = zk[p]; }
+            rec.iterations += it;
+            rec.max_iterations = max(rec.max_iterations, it);
+            rec.steps_not_converged += conv ? 0 : 1;
+            rec.residual = res;
+            __syncthreads();
+        }
+        __syncthreads();
+        if (s_status != 0) {                                           // error: the cell is left unchanged
+            pass_through();
+            if (tid == 0) { rec.status = s_status; records[cell] = rec; }
+            continue;
+        }
+        for (int p = tid; p < n; p += CELLS_THREADS) {
+            double* o = v_out + 3 * (g0 + idx[p]);
+            o[0] = xn[p]; o[1] = yn[p]; o[2] = zn[p];
+        }
+        if (tid == 0) { rec.status = rec.steps_not_converged ? 1 : 0; records[cell] = rec; }
+    }
+}
+
+}  // namespace landau

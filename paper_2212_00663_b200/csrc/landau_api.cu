@@ -24,6 +24,7 @@
 #include "step.cuh"
 #include "step_dg.cuh"
 #include "step_anderson.cuh"
+#include "cells.cuh"
 
 using namespace landau;
 
@@ -82,6 +83,7 @@ struct landau_ctx {
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
     AndersonCtrl* d_aa = nullptr;
     Buf aa_hist;
+    Buf cells_off, cells_rec;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
     // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
@@ -561,6 +563,29 @@ __global__ void fp64_peak_kernel(double* out, int iters, double a, double b) {
 }  // namespace
 
 // =============================================================================================
+namespace {
+// NEXT-3: many collision cells, one persistent CTA per cell, whole run in one launch (cells.cuh).
+template <int NQ>
+int launch_cells(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
+                 double* v_out, int n_steps, double dt, double tol, int max_iter) {
+    auto kern = cells_run_kernel<NQ>;
+    const size_t smem = CellsCfg<NQ>::smem(cap);
+    static size_t attr_set = 0;
+    if (smem > attr_set) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = smem;
+    }
+    int* counter = (int*)((char*)c->cells_off.p + sizeof(long long) * ((size_t)n_cells + 1));
+    const int grid = std::min(n_cells, c->sm_count);
+    kern<<<grid, CELLS_THREADS, smem, c->stream>>>(c->d_tab, n_cells, cap, (const long long*)c->cells_off.p, v, w, sid,
+                                                   v_out, n_steps, dt, tol, max_iter, counter,
+                                                   (CellRecord*)c->cells_rec.p);
+    c->launches += 1;
+    return 0;
+}
+
+}  // namespace
+
 extern "C" {
 
 void landau_default_opts(landau_opts* o) {
@@ -650,7 +675,7 @@ void landau_destroy(landau_ctx* c) {
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
-                   &c->dg_Gk, &c->dg_part, &c->aa_hist})
+                   &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec})
         release(*b);
     delete c;
 }
@@ -968,6 +993,55 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     if (cerr) return fail(c, cerr, "step_dg: non-finite residual");
     if (info) { info->iterations = iterations; info->residual = residual; info->converged = converged; }
     return converged ? LANDAU_OK : LANDAU_NOT_CONVERGED;
+}
+
+int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, const double* v, const double* w,
+                     const int32_t* sid, double* v_out, int n_steps, double dt, double tol, int max_iter,
+                     landau_cell_info* info) {
+    if (!c) return LANDAU_EINVAL;
+    if (n_cells < 1 || !cell_offset || !v || !w || !sid || !v_out)
+        return fail(c, LANDAU_EINVAL, "cells_run: NULL array or n_cells < 1");
+    if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
+        return fail(c, LANDAU_EINVAL, "cells_run: need n_steps >= 1, max_iter >= 1, dt > 0, tol >= 0");
+    if (c->n_q > 4) return fail(c, LANDAU_EINVAL, "cells_run: n_q <= 4 only (n_q = %d)", c->n_q);
+    int cap = 0;
+    for (int k = 0; k < n_cells; ++k) {
+        const int64_t nk = cell_offset[k + 1] - cell_offset[k];
+        if (nk < 0) return fail(c, LANDAU_EINVAL, "cells_run: cell_offset must be non-decreasing");
+        if (nk > CELLS_CAP)
+            return fail(c, LANDAU_EINVAL, "cells_run: cell %d has %lld markers, limit %d per cell", k, (long long)nk, CELLS_CAP);
+        cap = std::max(cap, (int)nk);
+    }
+    cap = std::max(32, (cap + 1) & ~1);
+    cudaStream_t st = c->stream;
+    RC(ensure(c, c->cells_off, sizeof(long long) * ((size_t)n_cells + 1) + 64));
+    RC(ensure(c, c->cells_rec, sizeof(CellRecord) * (size_t)n_cells));
+    static_assert(sizeof(long long) == sizeof(int64_t), "offset type");
+    CU(cudaMemcpyAsync(c->cells_off.p, cell_offset, sizeof(int64_t) * ((size_t)n_cells + 1), cudaMemcpyHostToDevice, st));
+    CU(cudaMemsetAsync((char*)c->cells_off.p + sizeof(long long) * ((size_t)n_cells + 1), 0, sizeof(int), st));
+    switch (c->n_q) {
+        case 2: RC((launch_cells<2>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        case 3: RC((launch_cells<3>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        default: RC((launch_cells<4>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+    }
+    CU(cudaGetLastError());
+    std::vector<CellRecord> h(n_cells);
+    CU(cudaMemcpyAsync(h.data(), c->cells_rec.p, sizeof(CellRecord) * (size_t)n_cells, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    snprintf(c->kernels, sizeof(c->kernels), "cells=fused");
+    int worst = 0, any_unconv = 0;
+    for (int k = 0; k < n_cells; ++k) {
+        if (info) {
+            info[k].status = h[k].status; info[k].iterations = h[k].iterations;
+            info[k].max_iterations = h[k].max_iterations; info[k].steps_not_converged = h[k].steps_not_converged;
+            info[k].residual = h[k].residual;
+        }
+        worst = std::min(worst, h[k].status);
+        if (h[k].status == 1) any_unconv = 1;
+    }
+    if (worst < 0) return fail(c, worst, "cells_run: at least one cell failed (status %d); see landau_cell_info.status", worst);
+    return any_unconv ? LANDAU_NOT_CONVERGED : LANDAU_OK;
 }
 
 int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps) {

@@ -525,3 +525,81 @@ def test_two_v_mode_keeps_vz_zero_and_matches_oracle(B, oracle_mod):
     assert abs(m1["K"].sum() - m0["K"].sum()) <= 1e-11 * m0["K"].sum()
     with pytest.raises(B.LandauError):
         g.set_dimension(4)
+
+
+# ------------------------------------------------------------------------------------ NEXT-3: many collision cells
+def _make_cells(rng_seed=5):
+    """A ragged batch: cells of different sizes, species mixes and orders, one empty cell."""
+    parts, off = [], [0]
+    for k, (cfg, n) in enumerate([(0, 40), (0, 150), (4, 60), (0, 7), (4, 333), (0, 500), (0, 1)]):
+        wl = W.make(cfg, n_per_species=n, seed=100 + k, shuffled=True)
+        parts.append(wl)
+        off.append(off[-1] + wl.n_markers)
+        if k == 2:
+            off.append(off[-1])                                  # an empty cell
+            parts.append(None)
+    return parts, np.array(off, dtype=np.int64)
+
+
+def test_cells_run_matches_oracle_per_cell(B, oracle_mod):
+    """landau_cells_run: every cell of a ragged batch advanced by 2 steps of Eq. (24) in ONE launch must equal the
+    oracle run on that cell alone (the cells share the species table of config 4: e, D+, C6+)."""
+    parts, off = _make_cells()
+    ref4 = W.make(4, n_per_species=8)
+    mass, charge = ref4.mass, ref4.charge
+    eps = np.array([0.05, 0.05 / 3671.0, 0.05 / 22032.0])
+    # config-0 cells use species ids 0 (e) and 1 (here: D+ slot) of the shared table; rescale their ion velocities
+    vs, ws, ss = [], [], []
+    for wl in parts:
+        if wl is None:
+            continue
+        v = wl.v.copy()
+        if wl.n_species == 2:
+            v[wl.species_id == 1] *= np.sqrt(1836.0 / 3671.0)
+        vs.append(v); ws.append(wl.w); ss.append(wl.species_id)
+    v, w, sid = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss)
+    g = B.Landau(mass, charge, eps)
+    dt, n_steps = 1e-3, 2
+    rc, vout, info = g.cells_run(off, v, w, sid, n_steps, dt, 1e-12, 60)
+    vout = vout.cpu().numpy()
+    assert rc == 0 and "cells" in g.last_kernels()
+    o = oracle_mod.LandauRef(mass, charge, eps)
+    for k in range(len(off) - 1):
+        a, b = off[k], off[k + 1]
+        if a == b:
+            assert info["status"][k] == 0 and info["iterations"][k] == 0
+            continue
+        o.set_markers(v[a:b], w[a:b], sid[a:b])
+        its = 0
+        for _ in range(n_steps):
+            rco, ito, reso, convo = o.step(dt, 1e-12, 60)
+            assert rco == 0
+            its += ito
+        ref = o.get_markers()
+        assert info["status"][k] == 0 and abs(int(info["iterations"][k]) - its) <= 2
+        if b - a > 1:
+            assert rel_l2(vout[a:b] - v[a:b], ref - v[a:b]) <= 1e-8, k
+        assert rel_l2(vout[a:b], ref) <= 1e-11, k
+        wm = (w[a:b] * mass[sid[a:b]])[:, None]
+        assert np.abs((wm * (vout[a:b] - v[a:b])).sum(0)).max() <= TOL_DRIFT * np.abs(wm * v[a:b]).sum()
+        K0, K1 = 0.5 * (wm * v[a:b] ** 2).sum(), 0.5 * (wm * vout[a:b] ** 2).sum()
+        assert abs(K1 - K0) <= TOL_DRIFT * K0
+
+
+def test_cells_run_rejects_bad_cells_and_passes_them_through(B):
+    wl = W.make(0, n_per_species=50, shuffled=True)
+    v = np.concatenate([wl.v, wl.v, wl.v]); w = np.concatenate([wl.w, wl.w, wl.w]).copy()
+    sid = np.concatenate([wl.species_id] * 3)
+    off = np.array([0, 100, 200, 300], dtype=np.int64)
+    w[130] = -1.0                                                # cell 1 is invalid
+    v[205] = 400.0                                               # cell 2 is too wide for the factorised pass 1
+    g = B.Landau(wl.mass, wl.charge, wl.eps)
+    rc, vout, info = g.cells_run(off, v, w, sid, 1, wl.dt, 1e-12, 50, strict=False)
+    vout = vout.cpu().numpy()
+    assert rc == B.ERANGE and list(info["status"]) == [0, B.EINVAL, B.ERANGE]
+    assert np.array_equal(vout[100:300], v[100:300]) and not np.array_equal(vout[:100], v[:100])
+    with pytest.raises(B.LandauError):
+        g.cells_run(off, v, w, sid, 1, wl.dt)
+    with pytest.raises(B.LandauError):                           # more than 1024 markers in a cell
+        big = W.make(0, n_per_species=600)
+        g.cells_run(np.array([0, 1200]), big.v, big.w, big.species_id, 1, 0.01)
