@@ -42,6 +42,7 @@ struct Cloud {
     int npad_max = 0;
     int pad = 0;
     Buf lay, xyzw, perm, G, rec, soa;
+    bool G_valid = false;   // G / snode hold pass 1 of the CURRENT x, y, z (lets a step reuse the pass 1 of landau_moments)
     int sym = 0;   // 1: the symmetric pair kernel's layout (pad = its target tile) and SoA source copy
     DevLayout* L() const { return (DevLayout*)lay.p; }
     double* x() const { return (double*)xyzw.p; }
@@ -293,7 +294,7 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
     const int S = c->S;
     const int pad = choose_pad(c, N);
     const int npm = npad_upper(N, S, pad);
-    cl.N = N; cl.npad_max = npm; cl.pad = pad; cl.sym = want_sym(c, N);
+    cl.N = N; cl.npad_max = npm; cl.pad = pad; cl.sym = want_sym(c, N); cl.G_valid = false;
     if (cl.sym) RC(ensure(c, cl.soa, sizeof(double) * 7 * (size_t)npm));
     RC(ensure(c, cl.lay, sizeof(DevLayout)));
     RC(ensure(c, cl.xyzw, sizeof(double) * 4 * (size_t)npm));
@@ -423,6 +424,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
         mode == 1 ? 0 : (mode >= 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
     c->launches += 1;
     CU(cudaGetLastError());
+    cl.G_valid = true;
     return 0;
 }
 
@@ -477,6 +479,7 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
     c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+    if (*h) cl.G_valid = false;
     if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
     if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
     if (*h == LANDAU_ERANGE)
@@ -806,7 +809,8 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
     for (int n = 0; n < n_steps; ++n) {
         c->prof_step = n; c->prof_iter = 0;
-        RC(entropy(c, cl));
+        if (!cl.G_valid) RC(entropy(c, cl));     // a preceding landau_moments(S_eps) already evaluated pass 1 here
+        cl.G_valid = false;                      // the step moves the markers
         step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
                                                                cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
                                                                cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
@@ -882,6 +886,7 @@ int landau_set_dimension(landau_ctx* c, int dim) {
     if (!c) return LANDAU_EINVAL;
     if (dim != 2 && dim != 3) return fail(c, LANDAU_EINVAL, "set_dimension: dim must be 2 or 3");
     c->dim = dim;
+    c->state.G_valid = false; c->tmp.G_valid = false;
     CU(cudaMemcpyAsync(&c->d_tab->dim, &c->dim, sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return 0;
@@ -939,7 +944,8 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
     c->prof_step = 0; c->prof_iter = 0;
-    RC(entropy(c, cl));                                       // G(v^n), entropy integrand at v^n
+    if (!cl.G_valid) RC(entropy(c, cl));                      // G(v^n), entropy integrand at v^n
+    cl.G_valid = false;
     double S0 = 0.0;
     RC(total_entropy(cl, &S0));
     step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
@@ -1048,7 +1054,7 @@ int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps
     if (!c) return LANDAU_EINVAL;
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "moments: no markers held");
-    if (S_eps) RC(entropy(c, cl));
+    if (S_eps && !cl.G_valid) RC(entropy(c, cl));
     double* h = (double*)c->h_pin + 64;
     RC(species_sums(c, cl, S_eps != nullptr, false, h));
     const double PI = 3.14159265358979323846;

@@ -603,3 +603,25 @@ def test_cells_run_rejects_bad_cells_and_passes_them_through(B):
     with pytest.raises(B.LandauError):                           # more than 1024 markers in a cell
         big = W.make(0, n_per_species=600)
         g.cells_run(np.array([0, 1200]), big.v, big.w, big.species_id, 1, 0.01)
+
+
+def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
+    """landau_moments(S_eps) evaluates pass 1 at the current state; the next landau_step starts from exactly that
+    state and reuses it (one pass 1 per step instead of two in history runs).  Results must be identical to a run
+    that never asks for the entropy."""
+    wl = W.make(0, n_per_species=200, shuffled=True)
+    ga = B.Landau(wl.mass, wl.charge, wl.eps)
+    gb = B.Landau(wl.mass, wl.charge, wl.eps)
+    ga.set_markers(wl.v, wl.w, wl.species_id)
+    gb.set_markers(wl.v, wl.w, wl.species_id)
+    for _ in range(3):
+        ga.moments(with_entropy=True)
+        l0 = ga.launch_count()
+        ra = ga.step(wl.dt, wl.tol, wl.max_iter)
+        la = ga.launch_count() - l0
+        l0 = gb.launch_count()
+        rb = gb.step(wl.dt, wl.tol, wl.max_iter)
+        lb = gb.launch_count() - l0
+        assert ra == rb and la < lb
+    assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+    np.testing.assert_array_equal(ga.moments()["S_eps"], gb.moments()["S_eps"])
