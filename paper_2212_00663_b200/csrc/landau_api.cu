@@ -84,10 +84,11 @@ struct landau_ctx {
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
     AndersonCtrl* d_aa = nullptr;
     Buf aa_hist;
-    Buf cells_off, cells_rec;
+    Buf cells_off, cells_rec, soa32;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
     // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
+    bool entropy_ran = false;             // a pass 1 ran since the last finish() (for landau_last_kernels)
     bool prof_on = false;
     bool in_run = false;
     struct ProfEv { cudaEvent_t e0, e1; int kind; int step; int iter; };
@@ -254,7 +255,7 @@ using SymL = SymCfg<SYM_W, SYM_RT, SYM_RS>;
 constexpr int64_t SYM_MIN_MARKERS = 16384;
 
 int want_sym(const landau_ctx* c, int64_t N) {
-    if (c->pair_kernel == 1 || c->precision == 1) return 0;
+    if (c->pair_kernel == 1) return 0;
     if (c->pair_kernel == 2) return 1;
     return N >= SYM_MIN_MARKERS;
 }
@@ -425,6 +426,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
     c->launches += 1;
     CU(cudaGetLastError());
     cl.G_valid = true;
+    c->entropy_ran = true;
     return 0;
 }
 
@@ -436,11 +438,34 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     ProfScope prof(c, 0);
     c->k_pair = use_sym ? "sym" : "onesided";
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
-    if (use_sym) {
+    const bool fp32_field = c->precision == 1 && !ctrl;     // FP32 variant: field evaluation only
+    if (use_sym && !fp32_field) {
         RC(launch_pair_sym(c, cl, ctrl, nparts_out));
         return 0;
     }
-    if (c->precision == 1 && !ctrl) {                       // FP32 field variant (never inside the implicit step)
+    if (c->precision == 1 && !ctrl && cl.sym) {             // FP32 field variant, symmetric kernel in FP32
+        using SymF = SymCfg<SYM_W, SYM_RT, SYM_RS, float>;
+        const int G = c->sm_count;
+        const size_t n = (size_t)G * 3 * cl.npad_max, n7 = 7 * (size_t)cl.npad_max;
+        RC(ensure(c, c->vpart, sizeof(double) * n));
+        RC(ensure(c, c->soa32, sizeof(float) * n7));
+        auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, float>;
+        static bool attr_done = false;
+        if (!attr_done) {
+            CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SymF::SMEM));
+            attr_done = true;
+        }
+        soa_to_f32_kernel<<<c->sm_count * 4, 256, 0, c->stream>>>(n7, cl.soas(), (float*)c->soa32.p);
+        zero_slices_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(nullptr, (double2*)c->vpart.p, n / 2);
+        kern<<<G, SymF::THREADS, SymF::SMEM, c->stream>>>(c->d_tab, cl.L(), nullptr, cl.npad_max,
+                                                          (const float*)c->soa32.p, (double*)c->vpart.p);
+        c->k_pair = "sym_f32";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+        c->launches += 3;
+        *nparts_out = G;
+        return 0;
+    }
+    if (c->precision == 1 && !ctrl) {                       // FP32 field variant below the symmetric kernel's size
         constexpr int RF = 4;
         const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * RF);
         const int stiles = cl.npad_max / PAIR_SRC_TILE;
@@ -477,7 +502,11 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
-    c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
+    if (c->entropy_ran)
+        c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
+    else if (!c->in_run)
+        c->k_entropy = "-";
+    c->entropy_ran = false;
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (*h) cl.G_valid = false;
     if (*h == LANDAU_EINVAL) return fail(c, LANDAU_EINVAL, "%s: species_id out of range or weight <= 0", where);
@@ -678,7 +707,7 @@ void landau_destroy(landau_ctx* c) {
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
-                   &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec})
+                   &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32})
         release(*b);
     delete c;
 }

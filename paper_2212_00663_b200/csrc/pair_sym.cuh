@@ -59,14 +59,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     }
 }
 
-template <int W, int RT, int RS>
+template <int W, int RT, int RS, typename F = double>
 struct SymCfg {
     static constexpr int THREADS = W * 32;
     static constexpr int BT = W * 32 * RT;   // targets per tile (registers)
     static constexpr int BS = W * 32 * RS;   // sources per unit (shared memory)
     static constexpr int SUB = 32 * RS;      // sources per warp and phase
     static constexpr int NCOMP = 7;          // x y z w gx gy gz
-    static constexpr size_t SMEM = sizeof(double) * (2 * NCOMP * BS + 3 * BS) + 64;
+    static constexpr size_t SMEM = sizeof(F) * (2 * NCOMP * BS + 3 * BS) + 64;
     static_assert(BT % BS == 0, "target tile must be a whole number of source units");
 };
 
@@ -75,45 +75,59 @@ __device__ __host__ inline long long sym_tasks_before(int I, int TU, int rho) {
     return (long long)I * TU - (long long)rho * I * (I - 1) / 2;
 }
 
-template <bool SYM, int RT, int RS>
-__device__ __forceinline__ void sym_step(const double (&px)[RT], const double (&py)[RT], const double (&pz)[RT],
-                                         const double (&gx)[RT], const double (&gy)[RT], const double (&gz)[RT],
-                                         const double (&wp)[RT], double (&ax)[RT], double (&ay)[RT],
-                                         double (&az)[RT], const double (&qx)[RS], const double (&qy)[RS],
-                                         const double (&qz)[RS], const double (&hx)[RS], const double (&hy)[RS],
-                                         const double (&hz)[RS], const double (&wq)[RS], double (&bx)[RS],
-                                         double (&by)[RS], double (&bz)[RS]) {
+// FP32 flavour of rsqrt_or_zero (FP32 field variant of BASELINE config 4): MUFU.RSQ + one Newton step;
+// a separation that underflows in FP32 contributes 0 (reading S5 in FP32).
+__device__ __forceinline__ float rsqrt_or_zero(float x) {
+    float y = rsqrtf(fmaxf(x, 1e-30f));
+    y = y * fmaf(-0.5f * x * y, y, 1.5f);
+    return x < 1e-30f ? 0.f : y;
+}
+__device__ __forceinline__ float sym_fma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double sym_fma(double a, double b, double c) { return fma(a, b, c); }
+template <typename F> struct SymVec2;
+template <> struct SymVec2<double> { using type = double2; };
+template <> struct SymVec2<float> { using type = float2; };
+
+template <bool SYM, int RT, int RS, typename F>
+__device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], const F (&pz)[RT],
+                                         const F (&gx)[RT], const F (&gy)[RT], const F (&gz)[RT],
+                                         const F (&wp)[RT], F (&ax)[RT], F (&ay)[RT],
+                                         F (&az)[RT], const F (&qx)[RS], const F (&qy)[RS],
+                                         const F (&qz)[RS], const F (&hx)[RS], const F (&hy)[RS],
+                                         const F (&hz)[RS], const F (&wq)[RS], F (&bx)[RS],
+                                         F (&by)[RS], F (&bz)[RS]) {
 #pragma unroll
     for (int s = 0; s < RS; ++s) {
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const double zx = px[r] - qx[s], zy = py[r] - qy[s], zz = pz[r] - qz[s];
-            const double cx = gx[r] - hx[s], cy = gy[r] - hy[s], cz = gz[r] - hz[s];
-            const double r2 = fma(zz, zz, fma(zy, zy, zx * zx));
-            const double d = fma(zz, cz, fma(zy, cy, zx * cx));
-            const double yv = rsqrt_or_zero(r2);
-            const double h = d * (yv * yv);
-            const double ux = fma(-zx, h, cx), uy = fma(-zy, h, cy), uz = fma(-zz, h, cz);
-            const double a = wq[s] * yv;
-            ax[r] = fma(a, ux, ax[r]); ay[r] = fma(a, uy, ay[r]); az[r] = fma(a, uz, az[r]);
+            const F zx = px[r] - qx[s], zy = py[r] - qy[s], zz = pz[r] - qz[s];
+            const F cx = gx[r] - hx[s], cy = gy[r] - hy[s], cz = gz[r] - hz[s];
+            const F r2 = sym_fma(zz, zz, sym_fma(zy, zy, zx * zx));
+            const F d = sym_fma(zz, cz, sym_fma(zy, cy, zx * cx));
+            const F yv = rsqrt_or_zero(r2);
+            const F h = d * (yv * yv);
+            const F ux = sym_fma(-zx, h, cx), uy = sym_fma(-zy, h, cy), uz = sym_fma(-zz, h, cz);
+            const F a = wq[s] * yv;
+            ax[r] = sym_fma(a, ux, ax[r]); ay[r] = sym_fma(a, uy, ay[r]); az[r] = sym_fma(a, uz, az[r]);
             if (SYM) {
-                const double b = wp[r] * yv;
-                bx[s] = fma(b, ux, bx[s]); by[s] = fma(b, uy, by[s]); bz[s] = fma(b, uz, bz[s]);
+                const F b = wp[r] * yv;
+                bx[s] = sym_fma(b, ux, bx[s]); by[s] = sym_fma(b, uy, by[s]); bz[s] = sym_fma(b, uz, bz[s]);
             }
         }
     }
 }
 
-template <int W, int RT, int RS>
+template <int W, int RT, int RS, typename F = double>
 __global__ void __launch_bounds__(W * 32, 1)
 pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
-                const StepCtrl* __restrict__ ctrl, int npad_max, const double* __restrict__ soa,
+                const StepCtrl* __restrict__ ctrl, int npad_max, const F* __restrict__ soa,
                 double* __restrict__ vpart) {
-    using C = SymCfg<W, RT, RS>;
+    using C = SymCfg<W, RT, RS, F>;
+    using F2 = typename SymVec2<F>::type;
     if (ctrl && ctrl->done) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* s_src = reinterpret_cast<double*>(smem_raw);              // [2][NCOMP][BS]
-    double* s_acc = s_src + 2 * C::NCOMP * C::BS;                     // [3][BS]
+    F* s_src = reinterpret_cast<F*>(smem_raw);                        // [2][NCOMP][BS]
+    F* s_acc = s_src + 2 * C::NCOMP * C::BS;                          // [3][BS]
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_acc + 3 * C::BS); // [2]
     __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
     __shared__ double s_im[LD_MAX_SPECIES];
@@ -144,17 +158,17 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     auto issue_load = [&](int unit, int stage) {
         if (tid == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_expect_tx(&s_bar[stage], C::NCOMP * C::BS * (uint32_t)sizeof(double));
+            mbar_expect_tx(&s_bar[stage], C::NCOMP * C::BS * (uint32_t)sizeof(F));
 #pragma unroll
             for (int c = 0; c < C::NCOMP; ++c)
                 bulk_g2s(s_src + ((size_t)stage * C::NCOMP + c) * C::BS,
-                         soa + (size_t)c * npad_max + (size_t)unit * C::BS, C::BS * (uint32_t)sizeof(double),
+                         soa + (size_t)c * npad_max + (size_t)unit * C::BS, C::BS * (uint32_t)sizeof(F),
                          &s_bar[stage]);
         }
     };
 
     double* myslice = vpart + (size_t)blockIdx.x * 3 * (size_t)npad_max;
-    double px[RT], py[RT], pz[RT], gx[RT], gy[RT], gz[RT], w0[RT], wp[RT], ax[RT], ay[RT], az[RT];
+    F px[RT], py[RT], pz[RT], gx[RT], gy[RT], gz[RT], w0[RT], wp[RT], ax[RT], ay[RT], az[RT];
     int curI = -1, sI = 0;
     uint32_t phase_bits = 0;   // bit s = parity to wait for on stage s
     int stage = 0;
@@ -167,9 +181,9 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 #pragma unroll
                 for (int r = 0; r < RT; ++r) {
                     const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
-                    myslice[p] += ax[r] * im;
-                    myslice[(size_t)npad_max + p] += ay[r] * im;
-                    myslice[2 * (size_t)npad_max + p] += az[r] * im;
+                    myslice[p] += (double)ax[r] * im;
+                    myslice[(size_t)npad_max + p] += (double)ay[r] * im;
+                    myslice[2 * (size_t)npad_max + p] += (double)az[r] * im;
                 }
             }
             curI = I;
@@ -181,7 +195,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 w0[r] = soa[3 * (size_t)npad_max + p];
                 gx[r] = soa[4 * (size_t)npad_max + p]; gy[r] = soa[5 * (size_t)npad_max + p];
                 gz[r] = soa[6 * (size_t)npad_max + p];
-                ax[r] = ay[r] = az[r] = 0.0;
+                ax[r] = ay[r] = az[r] = F(0);
             }
         }
         // next task (prefetch its source unit into the other stage)
@@ -190,35 +204,35 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         if (t + 1 < t1) issue_load(jn, stage ^ 1);
 
         const int sJ = species_of_slot(L, S, j * C::BS);
-        const double nu = s_nu[sI * S + sJ];
+        const F nu = (F)s_nu[sI * S + sJ];
         const bool diag = j < rho * (I + 1);
 #pragma unroll
         for (int r = 0; r < RT; ++r) wp[r] = w0[r] * nu;
-        for (int i = tid; i < 3 * C::BS; i += C::THREADS) s_acc[i] = 0.0;
+        for (int i = tid; i < 3 * C::BS; i += C::THREADS) s_acc[i] = F(0);
         mbar_wait(&s_bar[stage], (phase_bits >> stage) & 1u);
         phase_bits ^= 1u << stage;
         __syncthreads();
 
-        const double* sx = s_src + (size_t)stage * C::NCOMP * C::BS;
+        const F* sx = s_src + (size_t)stage * C::NCOMP * C::BS;
         for (int ph = 0; ph < W; ++ph) {
             const int base = ((wv + ph) % W) * C::SUB;
-            double bx[RS], by[RS], bz[RS];
+            F bx[RS], by[RS], bz[RS];
 #pragma unroll
-            for (int s = 0; s < RS; ++s) bx[s] = by[s] = bz[s] = 0.0;
+            for (int s = 0; s < RS; ++s) bx[s] = by[s] = bz[s] = F(0);
 #pragma unroll 1
             for (int k = 0; k < 32; ++k) {
                 const int g = base + ((lane + k) & 31) * RS;
-                double qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS];
+                F qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS];
                 if (RS % 2 == 0) {
 #pragma unroll
                     for (int s = 0; s < RS; s += 2) {
-                        const double2 a0 = *reinterpret_cast<const double2*>(sx + 0 * C::BS + g + s);
-                        const double2 a1 = *reinterpret_cast<const double2*>(sx + 1 * C::BS + g + s);
-                        const double2 a2 = *reinterpret_cast<const double2*>(sx + 2 * C::BS + g + s);
-                        const double2 a3 = *reinterpret_cast<const double2*>(sx + 3 * C::BS + g + s);
-                        const double2 a4 = *reinterpret_cast<const double2*>(sx + 4 * C::BS + g + s);
-                        const double2 a5 = *reinterpret_cast<const double2*>(sx + 5 * C::BS + g + s);
-                        const double2 a6 = *reinterpret_cast<const double2*>(sx + 6 * C::BS + g + s);
+                        const F2 a0 = *reinterpret_cast<const F2*>(sx + 0 * C::BS + g + s);
+                        const F2 a1 = *reinterpret_cast<const F2*>(sx + 1 * C::BS + g + s);
+                        const F2 a2 = *reinterpret_cast<const F2*>(sx + 2 * C::BS + g + s);
+                        const F2 a3 = *reinterpret_cast<const F2*>(sx + 3 * C::BS + g + s);
+                        const F2 a4 = *reinterpret_cast<const F2*>(sx + 4 * C::BS + g + s);
+                        const F2 a5 = *reinterpret_cast<const F2*>(sx + 5 * C::BS + g + s);
+                        const F2 a6 = *reinterpret_cast<const F2*>(sx + 6 * C::BS + g + s);
                         qx[s] = a0.x; qx[s + 1] = a0.y; qy[s] = a1.x; qy[s + 1] = a1.y; qz[s] = a2.x; qz[s + 1] = a2.y;
                         qw[s] = a3.x * nu; qw[s + 1] = a3.y * nu;
                         hx[s] = a4.x; hx[s + 1] = a4.y; hy[s] = a5.x; hy[s + 1] = a5.y; hz[s] = a6.x; hz[s + 1] = a6.y;
@@ -232,9 +246,9 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                     }
                 }
                 if (diag) {
-                    sym_step<false, RT, RS>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<false, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                 } else {
-                    sym_step<true, RT, RS>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<true, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
 #pragma unroll
                     for (int s = 0; s < RS; ++s) {
                         bx[s] = __shfl_sync(0xffffffffu, bx[s], (lane + 1) & 31);
@@ -257,7 +271,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
             const double sc = -s_im[sJ];
             for (int i = tid; i < 3 * C::BS; i += C::THREADS) {
                 const int d = i / C::BS, e = i - d * C::BS;
-                myslice[(size_t)d * npad_max + (size_t)j * C::BS + e] += sc * s_acc[i];
+                myslice[(size_t)d * npad_max + (size_t)j * C::BS + e] += sc * (double)s_acc[i];
             }
         }
         __syncthreads();
@@ -268,9 +282,9 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
             const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
-            myslice[p] += ax[r] * im;
-            myslice[(size_t)npad_max + p] += ay[r] * im;
-            myslice[2 * (size_t)npad_max + p] += az[r] * im;
+            myslice[p] += (double)ax[r] * im;
+            myslice[(size_t)npad_max + p] += (double)ay[r] * im;
+            myslice[2 * (size_t)npad_max + p] += (double)az[r] * im;
         }
     }
 }
@@ -298,6 +312,12 @@ __global__ void build_soa_kernel(const DevTable* __restrict__ T, const DevLayout
     }
 #pragma unroll
     for (int c = 0; c < 7; ++c) soa[(size_t)c * npad_max + p] = v[c];
+}
+
+// FP64 SoA source copy -> FP32 (FP32 field variant).
+__global__ void soa_to_f32_kernel(size_t n, const double* __restrict__ a, float* __restrict__ b) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) b[i] = (float)a[i];
 }
 
 }  // namespace landau

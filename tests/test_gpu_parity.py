@@ -193,6 +193,17 @@ def test_fp32_pair_field_variant(B, oracle_mod):
     g32.set_markers(wl.v, wl.w, wl.species_id)
     rc, it, res, conv = g32.step(1e-3, 1e-12, 50)
     assert rc == 0 and conv and "f32" not in g32.last_kernels()
+    # at >= 16384 markers the FP32 variant is the symmetric (action-reaction) kernel in FP32
+    wl = W.make(4, n_per_species=6000, shuffled=True)
+    rng = np.random.default_rng(3)
+    G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+    g64 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g32 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, precision=1)
+    V64 = g64.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    V32 = g32.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    assert "pair=sym_f32" in g32.last_kernels() and "pair=sym " in g64.last_kernels() + " "
+    assert_field_close(V32, V64, wl.species_id, wl.n_species, tol=2e-5, what="FP32 symmetric pair field")
+    assert rel_l2(V32, V64) > 1e-9
 
 
 # ------------------------------------------------------------------------------------ full field
