@@ -338,6 +338,24 @@ def run_ours(args):
                 "e2e": {"value": pairs_e2e / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e_max / args.steps},
                 "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        if args.solver == "jacobi":
+            # SURVEY.md NEXT-4, reported beside the headline (which stays the paper's Jacobi iteration): the same
+            # step with the Anderson-accelerated fixed point, device-resident inputs, after both timed regions
+            g.set_solver(1, args.anderson_depth)
+            step_device()
+            torch.cuda.synchronize()
+            e0.record()
+            it_aa, conv_aa = 0, True
+            for _ in range(2):
+                it, conv, _m, _v = step_device()
+                it_aa += it; conv_aa &= bool(conv)
+            e1.record()
+            torch.cuda.synchronize()
+            t_aa = e0.elapsed_time(e1) * 1e-3 / 2
+            line["anderson_solver"] = {"depth": args.anderson_depth, "ms_per_step": 1e3 * t_aa, "steps_per_s": 1.0 / t_aa,
+                                       "iterations_per_step": it_aa / 2, "all_converged": conv_aa,
+                                       "pairs_per_s": (it_aa / 2) * N * (N - 1) / t_aa}
+            g.set_solver(0)
         if args.workload.startswith("c4"):
             # BASELINE config 4: "plus an FP32 field variant" -- pass 2 alone, FP32 arithmetic, vs the FP64 kernel
             G = g.entropy_grad(v_d, w_d, s_d)
