@@ -271,7 +271,12 @@ def run_ours(args):
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
-    g.profile_enable(True)
+    # per-kernel CUDA events ride in the timed region, except for clouds small enough for the CUDA-graph step
+    # (landau_set_step_graph, <= 65536 slots): graph replays cannot carry per-kernel events, so those workloads
+    # get their kernel times from extra profiled steps after the timed region
+    prof_in_timed = N > 60000
+    if prof_in_timed:
+        g.profile_enable(True)
     l0 = g.launch_count()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     iters_total, all_conv = 0, True
@@ -282,10 +287,22 @@ def run_ours(args):
     e1.record()
     barrier()
     t_dev = e0.elapsed_time(e1) * 1e-3
-    prof = g.profile_read()
-    g.profile_enable(False)
+    t_prof = t_dev
+    if prof_in_timed:
+        prof = g.profile_read()
+        g.profile_enable(False)
     launches = g.launch_count() - l0
     clocks = sampler.stop()
+    if not prof_in_timed:
+        g.profile_enable(True)
+        e0.record()
+        for _ in range(2):
+            step_device()
+        e1.record()
+        torch.cuda.synchronize()
+        t_prof = e0.elapsed_time(e1) * 1e-3
+        prof = g.profile_read()
+        g.profile_enable(False)
     # ---- end-to-end timed region (host buffers)
     step_host()
     barrier()
@@ -319,11 +336,13 @@ def run_ours(args):
                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": float(N) * (N - 1),
                     "avg_launch_ms": pair_s * 1e3, "launches_timed": prof["pair_launches"],
                     "pair_kernel_pairs_per_s": N * (N - 1) / pair_s,
-                    "pair_share_of_step": prof["pair_ms"] * 1e-3 / t_dev,
+                    "pair_share_of_step": prof["pair_ms"] * 1e-3 / t_prof,
+                    "kernel_times_from": "the timed region" if prof_in_timed else
+                                         "2 extra profiled steps (the timed region replays CUDA-graph steps)",
                     "entropy_kernel_ms": prof["entropy_ms"] / max(prof["entropy_launches"], 1),
                     "entropy_same_species_pairs_per_s": float((wl.counts().astype(float) ** 2).sum()) /
                                                         (prof["entropy_ms"] * 1e-3 / max(prof["entropy_launches"], 1)),
-                    "entropy_share_of_step": prof["entropy_ms"] * 1e-3 / t_dev}
+                    "entropy_share_of_step": prof["entropy_ms"] * 1e-3 / t_prof}
         h2d = int(v_h.numel() * 8 + w_h.numel() * 8 + s_h.numel() * 4)
         d2h = int(out_h.numel() * 8 + 4 * 8 * wl.n_species)
         K0 = float(m0["K"].sum()); K1 = float(m1["K"].sum())

@@ -128,6 +128,16 @@ int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_ste
  * would seed the physical relaxation into v_z).  x/y results equal the 2-V Eqs. (22)-(24) (reading D1). */
 int landau_set_dimension(landau_ctx* ctx, int dim);
 
+/* How landau_step / landau_run issue a step whose cost is launch latency (small clouds).  mode 1 (default,
+ * automatic): clouds of <= 65536 padded slots replay the whole step as ONE CUDA graph whose fixed-point body is a
+ * conditional WHILE node kept alive from the device (cudaGraphSetConditional in the update kernel) -- no launch
+ * per iteration, no pre-enqueued iterations that exit at once.  mode 0: always the plain launch sequence
+ * (max_iter iterations enqueued up front, early exit on the device flag).  mode 2: graph at any size.  Same
+ * kernels and bit-identical results either way; the graph is captured after the first ordinary step, is reused
+ * while shapes and parameters stay the same, and is not used while landau_profile_enable is on or with the
+ * Anderson solver. */
+int landau_set_step_graph(landau_ctx* ctx, int mode);
+
 /* how landau_step / landau_run solve Eq. (24).  solver 0 (default) = the paper's plain
  * Jacobi fixed-point iteration; solver 1 = the same fixed point with Anderson acceleration of the given
  * depth (1..10, 3 to 5 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the

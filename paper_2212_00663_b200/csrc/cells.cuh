@@ -61,7 +61,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                  const double* __restrict__ v, const double* __restrict__ w, const int32_t* __restrict__ sid,
                  double* __restrict__ v_out, int n_steps, double dt, double tol, int max_iter,
                  int* __restrict__ next_cell, CellRecord* __restrict__ records) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     double* xn = reinterpret_cast<double*>(smem_raw);
     double* yn = xn + cap; double* zn = yn + cap; double* ww = zn + cap;
     double* Gx = ww + cap; double* Gy = Gx + cap; double* Gz = Gy + cap;

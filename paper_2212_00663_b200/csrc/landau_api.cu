@@ -85,6 +85,15 @@ struct landau_ctx {
     AndersonCtrl* d_aa = nullptr;
     Buf aa_hist;
     Buf cells_off, cells_rec, soa32;
+    // CUDA-graph form of a whole step for launch-bound (small) clouds, landau_set_step_graph
+    int graph_mode = 1;                   // 0 off, 1 automatic (npad <= 65536 slots), 2 always
+    unsigned long long alloc_gen = 0;
+    cudaStream_t body_stream = nullptr, cap_stream = nullptr;
+    struct StepGraph {
+        cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
+        unsigned long long gen = 0; int64_t N = 0; int npm = 0, max_iter = 0, fixed_nodes = 0, body_nodes = 0;
+        double dt = 0.0, tol = 0.0; int ek = 0, pk = 0; bool failed = false;
+    } sg;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
     // optional per-kernel timing (landau_profile_*): CUDA events around the two all-pairs kernels
@@ -101,6 +110,7 @@ struct landau_ctx {
     char kernels[128];
     const char* k_pair = "-";
     const char* k_entropy = "-";
+    const char* k_step = "-";
 };
 
 namespace {
@@ -135,6 +145,7 @@ int ensure(landau_ctx* c, Buf& b, size_t bytes) {
     if (bytes <= b.cap) return 0;
     if (b.p) CU(cudaFree(b.p));
     b.p = nullptr; b.cap = 0;
+    ++c->alloc_gen;                       // invalidates a cached step graph (kernel arguments are baked in)
     size_t want = bytes + bytes / 8 + 256;
     CU(cudaMalloc(&b.p, want));
     b.cap = want;
@@ -504,8 +515,6 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
     if (c->entropy_ran)
         c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
-    else if (!c->in_run)
-        c->k_entropy = "-";
     c->entropy_ran = false;
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (*h) cl.G_valid = false;
@@ -595,6 +604,130 @@ __global__ void fp64_peak_kernel(double* out, int iters, double a, double b) {
 }  // namespace
 
 // =============================================================================================
+namespace {
+// ---- a4 for launch-bound clouds: one step as a CUDA graph with a conditional WHILE node ----------------------
+// Nodes: step_begin, WHILE { (zero_slices,) pair, step_update -> cudaGraphSetConditional }, commit.  Pass 1 stays
+// outside (ordinary launches just before the graph) so that a pass 1 already done by landau_moments is reused.
+// Built by stream capture of the very launch sequence landau_run issues otherwise, after one ordinary step has
+// sized every buffer (nothing may be allocated during capture).  Returns 0 and leaves sg.exec == nullptr with
+// sg.failed set if the capture is refused; the ordinary launch sequence is then used (same kernels, same results).
+void destroy_step_graph(landau_ctx* c) {
+    if (c->sg.exec) cudaGraphExecDestroy(c->sg.exec);
+    if (c->sg.graph) cudaGraphDestroy(c->sg.graph);
+    c->sg.exec = nullptr; c->sg.graph = nullptr;
+}
+
+bool step_graph_matches(const landau_ctx* c, const Cloud& cl, double dt, double tol, int max_iter) {
+    const auto& g = c->sg;
+    return g.exec && g.gen == c->alloc_gen && g.N == cl.N && g.npm == cl.npad_max && g.dt == dt && g.tol == tol &&
+           g.max_iter == max_iter && g.ek == c->entropy_kernel && g.pk == c->pair_kernel;
+}
+
+int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_iter) {
+    destroy_step_graph(c);
+    if ((!c->body_stream && cudaStreamCreateWithFlags(&c->body_stream, cudaStreamNonBlocking) != cudaSuccess) ||
+        (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess)) {
+        c->sg.failed = true; cudaGetLastError(); return 0;
+    }
+    const int npm = cl.npad_max;
+    const int nub = ceil_div(npm, UPD_THREADS);
+    double* xk = (double*)c->vk.p;
+    double* yk = xk + npm;
+    double* zk = yk + npm;
+    // capture on a private stream (the context's stream may be the legacy default stream, which cannot be captured)
+    cudaStream_t user_stream = c->stream;
+    cudaStream_t st = c->cap_stream;
+    c->stream = st;
+    const unsigned long long gen0 = c->alloc_gen;
+    const int64_t launches0 = c->launches;
+    const bool g_valid0 = cl.G_valid, ran0 = c->entropy_ran;
+    const char* stage = "begin capture";
+    cudaError_t ce = cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed);
+    bool ok = ce == cudaSuccess;
+    cudaGraph_t graph = nullptr;
+    int fixed = 0, body_nodes = 0;
+    if (ok) {
+        if (ok) {
+            step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
+                                                                   cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
+                                                                   cl.sym ? nullptr : cl.recs(),
+                                                                   cl.sym ? cl.soas() : nullptr);
+            c->launches += 1;
+        }
+        cudaStreamCaptureStatus status;
+        cudaGraph_t g = nullptr;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t ndeps = 0;
+        cudaGraphConditionalHandle handle = 0;
+        cudaGraphNode_t cond_node = nullptr;
+        cudaGraphNodeParams params = {cudaGraphNodeTypeConditional};
+#define SG_TRY(what, call) if (ok) { ce = (call); if (ce != cudaSuccess) { ok = false; stage = what; } }
+        SG_TRY("capture info", cudaStreamGetCaptureInfo(st, &status, nullptr, &g, &deps, &ndeps));
+        if (ok && status != cudaStreamCaptureStatusActive) { ok = false; stage = "capture not active"; }
+        SG_TRY("conditional handle", cudaGraphConditionalHandleCreate(&handle, g, 1, cudaGraphCondAssignDefault));
+        if (ok) {
+            params.type = cudaGraphNodeTypeConditional;
+            params.conditional.handle = handle;
+            params.conditional.type = cudaGraphCondTypeWhile;
+            params.conditional.size = 1;
+            SG_TRY("conditional node", cudaGraphAddNode(&cond_node, g, deps, ndeps, &params));
+        }
+        fixed = (int)(c->launches - launches0);
+        if (ok) {
+            cudaGraph_t body = params.conditional.phGraph_out[0];
+            SG_TRY("body capture", cudaStreamBeginCaptureToGraph(c->body_stream, body, nullptr, nullptr, 0,
+                                                                 cudaStreamCaptureModeRelaxed));
+            if (ok) {
+                const int64_t l1 = c->launches;
+                c->stream = c->body_stream;
+                int nparts = 0;
+                ok = pair(c, cl, c->d_ctrl, &nparts) == 0;
+                if (ok) {
+                    step_update_kernel<<<nub, UPD_THREADS, 0, c->body_stream>>>(
+                        c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p, cl.x(),
+                        cl.y(), cl.z(), cl.w(), xk, yk, zk, cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr,
+                        (double*)c->blockpart.p, handle);
+                    c->launches += 1;
+                }
+                c->stream = st;
+                body_nodes = (int)(c->launches - l1);
+                cudaGraph_t tmp = nullptr;
+                ce = cudaStreamEndCapture(c->body_stream, &tmp);
+                if (ce != cudaSuccess && ok) { ok = false; stage = "end body capture"; }
+            }
+        }
+        SG_TRY("update dependencies", cudaStreamUpdateCaptureDependencies(st, &cond_node, 1, cudaStreamSetCaptureDependencies));
+        if (ok) {
+            step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,
+                                                                    zk, (StepRecord*)c->records.p, c->d_cursor);
+            fixed += 1;
+        }
+        ce = cudaStreamEndCapture(st, &graph);
+        if ((ce != cudaSuccess || !graph) && ok) { ok = false; stage = "end capture"; }
+    }
+    c->stream = user_stream;
+    c->launches = launches0;                    // nothing was launched: capture only records
+    cl.G_valid = g_valid0; c->entropy_ran = ran0;
+    cudaGraphExec_t exec = nullptr;
+    if (ok && c->alloc_gen != gen0) { ok = false; stage = "a buffer was reallocated during capture"; }
+    SG_TRY("instantiate", cudaGraphInstantiate(&exec, graph, 0));
+#undef SG_TRY
+    if (!ok) {
+        cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+        c->sg.failed = true;
+        snprintf(c->err, sizeof(c->err), "step graph not built (%s: %s); using the plain launch sequence", stage,
+                 cudaGetErrorString(ce));
+        return 0;
+    }
+    auto& g = c->sg;
+    g.graph = graph; g.exec = exec; g.gen = c->alloc_gen; g.N = cl.N; g.npm = npm; g.dt = dt; g.tol = tol;
+    g.max_iter = max_iter; g.ek = c->entropy_kernel; g.pk = c->pair_kernel; g.fixed_nodes = fixed; g.body_nodes = body_nodes;
+    return 0;
+}
+}  // namespace
+
 namespace {
 // NEXT-3: many collision cells, one persistent CTA per cell, whole run in one launch (cells.cuh).
 template <int NQ>
@@ -700,6 +833,9 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_ctrl) cudaFree(c->d_ctrl);
     if (c->d_cursor) cudaFree(c->d_cursor);
     if (c->d_aa) cudaFree(c->d_aa);
+    destroy_step_graph(c);
+    if (c->body_stream) cudaStreamDestroy(c->body_stream);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->d_momout) cudaFree(c->d_momout);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     for (Cloud* cl : {&c->tmp, &c->state}) {
@@ -742,6 +878,7 @@ int landau_pair_field(landau_ctx* c, int64_t N, const double* v, const double* w
     if (!c) return LANDAU_EINVAL;
     if (!G_in || !out) return fail(c, LANDAU_EINVAL, "pair_field: NULL array");
     Cloud& cl = c->tmp;
+    c->k_entropy = "-";                       // the entropy gradient is supplied: no pass 1 in this call
     RC(pack(c, cl, N, v, w, sid));
     gather3_kernel<<<ceil_div(cl.npad_max, 256), 256, 0, c->stream>>>(cl.npad_max, cl.L(), cl.prm(), G_in, cl.Gx(),
                                                                       cl.Gy(), cl.Gz());
@@ -836,8 +973,19 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     cudaStream_t st = c->stream;
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
+    const bool graph_ok = c->graph_mode != 0 && !c->sg.failed && !c->prof_on && c->solver == 0 &&
+                          (c->graph_mode == 2 || npm <= 65536);
+    std::vector<char> via_graph(n_steps, 0);
     for (int n = 0; n < n_steps; ++n) {
         c->prof_step = n; c->prof_iter = 0;
+        if (graph_ok && step_graph_matches(c, cl, dt, tol, max_iter)) {
+            if (!cl.G_valid) RC(entropy(c, cl));
+            CU(cudaGraphLaunch(c->sg.exec, st));
+            c->launches += c->sg.fixed_nodes;
+            via_graph[n] = 1;
+            cl.G_valid = false;
+            continue;
+        }
         if (!cl.G_valid) RC(entropy(c, cl));     // a preceding landau_moments(S_eps) already evaluated pass 1 here
         cl.G_valid = false;                      // the step moves the markers
         step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
@@ -880,12 +1028,14 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
             step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                              (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
                                                              cl.w(), xk, yk, zk, cl.sym ? nullptr : cl.recs(),
-                                                             cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p);
+                                                             cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p, 0);
             c->launches += 1;
         }
         step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,
                                                                 zk, (StepRecord*)c->records.p, c->d_cursor);
         c->launches += 1;
+        // every buffer now has its size: capture the same sequence as a graph for the steps that follow
+        if (graph_ok && !step_graph_matches(c, cl, dt, tol, max_iter)) RC(build_step_graph(c, cl, dt, tol, max_iter));
     }
     CU(cudaGetLastError());
     // one synchronisation: records + error flags
@@ -903,8 +1053,11 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
         for (int n = 0; n < n_steps; ++n) its[n] = h[n].iterations;
         prof_resolve(c, its.data(), n_steps);
     }
+    c->k_step = via_graph[n_steps - 1] ? "graph" : "launch";
+    snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s step=%s", c->k_pair, c->k_entropy, c->k_step);
     int any_unconverged = 0;
     for (int n = 0; n < n_steps; ++n) {
+        if (via_graph[n]) c->launches += (int64_t)h[n].iterations * c->sg.body_nodes;   // WHILE body launches
         if (info) { info[n].iterations = h[n].iterations; info[n].residual = h[n].residual; info[n].converged = h[n].converged; }
         if (!h[n].converged) any_unconverged = 1;
     }
@@ -918,6 +1071,14 @@ int landau_set_dimension(landau_ctx* c, int dim) {
     c->state.G_valid = false; c->tmp.G_valid = false;
     CU(cudaMemcpyAsync(&c->d_tab->dim, &c->dim, sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+int landau_set_step_graph(landau_ctx* c, int mode) {
+    if (!c) return LANDAU_EINVAL;
+    if (mode < 0 || mode > 2) return fail(c, LANDAU_EINVAL, "set_step_graph: mode must be 0 (off), 1 (automatic) or 2 (always)");
+    c->graph_mode = mode;
+    c->sg.failed = false;
     return 0;
 }
 
@@ -1011,7 +1172,7 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
         step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                          (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
                                                          xk, yk, zk, cl.sym ? nullptr : cl.recs(),
-                                                         cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p);
+                                                         cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p, 0);
         c->launches += 1;
         CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));

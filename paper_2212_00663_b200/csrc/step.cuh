@@ -5,9 +5,11 @@
 //   v^(0) = v^n;  u = (v^n + v^(k))/2;  V = pass2(u; G^n);  v^(k+1) = v^n + dt V
 //   r_k = sqrt( sum w m |v^(k+1) - v^(k)|^2 / sum w m |v^(k+1)|^2 ),  stop at r_k <= tol or k+1 = max_iter
 //
-// The loop is driven from the device: every iteration's kernels are enqueued up front (or replayed
-// from a CUDA graph) and exit at once when StepCtrl::done is set, so the host never waits inside a
-// step.  The residual is reduced in a fixed order (block partials, then the last block to finish
+// The loop is driven from the device.  Large clouds: every iteration's kernels are enqueued up front and exit
+// at once when StepCtrl::done is set.  Small clouds (launch-latency bound): the whole step is one CUDA graph whose
+// iteration body sits in a conditional WHILE node that step_update_kernel keeps alive through
+// cudaGraphSetConditional until the step is done (landau_api.cu, build_step_graph).  Either way the host never
+// waits inside a step.  The residual is reduced in a fixed order (block partials, then the last block to finish
 // sums them in index order), so iteration counts are reproducible run to run.
 #pragma once
 #include "common.cuh"
@@ -62,7 +64,7 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
                    const double* __restrict__ yn, const double* __restrict__ zn,
                    const double* __restrict__ w, double* __restrict__ xk, double* __restrict__ yk,
                    double* __restrict__ zk, double* __restrict__ rec, double* __restrict__ soa,
-                   double* __restrict__ blockpart) {
+                   double* __restrict__ blockpart, cudaGraphConditionalHandle cond) {
     if (ctrl->done) return;
     __shared__ double s_num[UPD_THREADS / 32], s_den[UPD_THREADS / 32];
     __shared__ int s_last;
@@ -124,6 +126,8 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         if (!isfinite(res)) { ctrl->err = -4; ctrl->done = 1; }
         else if (res <= tol) { ctrl->converged = 1; ctrl->done = 1; }
         else if (it >= max_iter) ctrl->done = 1;
+        // CUDA-graph mode: this kernel is the last node of a WHILE body; keep looping until the step is done
+        if (cond) cudaGraphSetConditional(cond, ctrl->done ? 0u : 1u);
     }
 }
 

@@ -636,3 +636,33 @@ def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
         assert ra == rb and la < lb
     assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
     np.testing.assert_array_equal(ga.moments()["S_eps"], gb.moments()["S_eps"])
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 256), (4, 300), (1, 4096), (4, 8000)])
+def test_graph_step_is_bit_identical_to_the_launch_sequence(B, cfg, n):
+    """Small clouds replay the step as a CUDA graph with a device-driven WHILE node (landau_set_step_graph);
+    the kernels are the same, so states, iteration counts and residuals must be bit-identical to the plain launch
+    sequence, also across set_markers calls that keep the shapes (graph reuse) and for landau_run chunks."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    ga = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gb = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    ga.set_step_graph(2)
+    gb.set_step_graph(0)
+    for rep in range(2):
+        ga.set_markers(wl.v, wl.w, wl.species_id)
+        gb.set_markers(wl.v, wl.w, wl.species_id)
+        ra = [ga.step(wl.dt, wl.tol, wl.max_iter) for _ in range(3)]
+        rb = [gb.step(wl.dt, wl.tol, wl.max_iter) for _ in range(3)]
+        assert ra == rb
+        rca, ia = ga.run(4, wl.dt, wl.tol, wl.max_iter)
+        rcb, ib = gb.run(4, wl.dt, wl.tol, wl.max_iter)
+        assert rca == rcb and ia == ib
+        assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+    la0, lb0 = ga.launch_count(), gb.launch_count()
+    ga.step(wl.dt, wl.tol, wl.max_iter); gb.step(wl.dt, wl.tol, wl.max_iter)
+    assert ga.launch_count() - la0 < gb.launch_count() - lb0      # no pre-enqueued idle iterations
+    # a step that hits max_iter leaves the WHILE loop too
+    ga.set_markers(wl.v, wl.w, wl.species_id); gb.set_markers(wl.v, wl.w, wl.species_id)
+    assert ga.step(wl.dt, 1e-15, 3) == gb.step(wl.dt, 1e-15, 3)
+    assert ga.step(wl.dt, 1e-15, 3) == gb.step(wl.dt, 1e-15, 3)
+    assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
