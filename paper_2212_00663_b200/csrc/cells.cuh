@@ -55,6 +55,43 @@ __device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_re
     a = x; b = y;
 }
 
+// Pass 2 of NT targets of one thread against every source of the cell (sources read once per NT targets:
+// NT = 2 halves the shared-memory traffic per pair).  t? = sum_s' nu_ss' sum_q w_q Q(u_p - u_q)(g_p - g_q).
+template <int NT>
+__device__ __forceinline__ void cells_field(const double* __restrict__ ux, const double* __restrict__ uy,
+                                            const double* __restrict__ uz, const double* __restrict__ Gx,
+                                            const double* __restrict__ Gy, const double* __restrict__ Gz,
+                                            const double* __restrict__ ww, const int* __restrict__ s_off,
+                                            const double* __restrict__ s_nu, int S, const int (&pc)[NT],
+                                            const int (&sp)[NT], double (&tx)[NT], double (&ty)[NT], double (&tz)[NT]) {
+    double px[NT], py[NT], pz[NT], hx[NT], hy[NT], hz[NT];
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        px[t] = ux[pc[t]]; py[t] = uy[pc[t]]; pz[t] = uz[pc[t]];
+        hx[t] = Gx[pc[t]]; hy[t] = Gy[pc[t]]; hz[t] = Gz[pc[t]];
+        tx[t] = ty[t] = tz[t] = 0.0;
+    }
+    for (int sb = 0; sb < S; ++sb) {
+        const int q0 = s_off[sb], q1 = s_off[sb + 1];
+        double ax[NT], ay[NT], az[NT];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) ax[t] = ay[t] = az[t] = 0.0;
+#pragma unroll 4
+        for (int q = q0; q < q1; ++q) {
+            const double qx = ux[q], qy = uy[q], qz = uz[q], gx = Gx[q], gy = Gy[q], gz = Gz[q], wq = ww[q];
+#pragma unroll
+            for (int t = 0; t < NT; ++t)
+                pair_accumulate(px[t] - qx, py[t] - qy, pz[t] - qz, hx[t] - gx, hy[t] - gy, hz[t] - gz, wq, ax[t], ay[t],
+                                az[t]);
+        }
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            const double nu = s_nu[sp[t] * S + sb];
+            tx[t] = fma(nu, ax[t], tx[t]); ty[t] = fma(nu, ay[t], ty[t]); tz[t] = fma(nu, az[t], tz[t]);
+        }
+    }
+}
+
 template <int NQ>
 __global__ void __launch_bounds__(CELLS_THREADS, 1)
 cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const long long* __restrict__ cell_off,
@@ -259,32 +296,33 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 double nx[CELLS_ROUNDS], ny[CELLS_ROUNDS], nz[CELLS_ROUNDS];
                 double num = 0.0, den = 0.0;
 #pragma unroll
-                for (int r = 0; r < CELLS_ROUNDS; ++r) {
+                for (int r = 0; r < CELLS_ROUNDS; ++r) nx[r] = ny[r] = nz[r] = 0.0;
+                auto finish_target = [&](int r, double tx, double ty, double tz) {
                     const int p = r * CELLS_THREADS + tid;
-                    nx[r] = ny[r] = nz[r] = 0.0;
-                    if (r * CELLS_THREADS < n) {                       // uniform: this round has targets
-                        const int pc = min(p, n - 1);
-                        const double px = ux[pc], py = uy[pc], pz = uz[pc];
-                        const double hx = Gx[pc], hy = Gy[pc], hz = Gz[pc];
-                        double tx = 0.0, ty = 0.0, tz = 0.0;
-                        for (int sb = 0; sb < S; ++sb) {
-                            const int q0 = s_off[sb], q1 = s_off[sb + 1];
-                            double ax = 0.0, ay = 0.0, az = 0.0;
-#pragma unroll 4
-                            for (int q = q0; q < q1; ++q)
-                                pair_accumulate(px - ux[q], py - uy[q], pz - uz[q], hx - Gx[q], hy - Gy[q], hz - Gz[q],
-                                                ww[q], ax, ay, az);
-                            const double nu = s_nu[sp[r] * S + sb];
-                            tx = fma(nu, ax, tx); ty = fma(nu, ay, ty); tz = fma(nu, az, tz);
-                        }
-                        if (p < n) {
-                            const double a = fma(dt, tx * im[r], xn[p]), b = fma(dt, ty * im[r], yn[p]),
-                                         c = fma(dt, tz * im[r], zn[p]);
-                            const double dx = a - xk[p], dy = b - yk[p], dz = c - zk[p];
-                            num += wm[r] * (dx * dx + dy * dy + dz * dz);
-                            den += wm[r] * (a * a + b * b + c * c);
-                            nx[r] = a; ny[r] = b; nz[r] = c;
-                        }
+                    if (p < n) {
+                        const double a = fma(dt, tx * im[r], xn[p]), b = fma(dt, ty * im[r], yn[p]),
+                                     c = fma(dt, tz * im[r], zn[p]);
+                        const double dx = a - xk[p], dy = b - yk[p], dz = c - zk[p];
+                        num += wm[r] * (dx * dx + dy * dy + dz * dz);
+                        den += wm[r] * (a * a + b * b + c * c);
+                        nx[r] = a; ny[r] = b; nz[r] = c;
+                    }
+                };
+#pragma unroll
+                for (int r = 0; r < CELLS_ROUNDS; r += 2) {
+                    if ((r + 1) * CELLS_THREADS < n) {                 // uniform: two rounds of targets share the sources
+                        const int pc[2] = {r * CELLS_THREADS + tid, min((r + 1) * CELLS_THREADS + tid, n - 1)};
+                        const int spc[2] = {sp[r], sp[r + 1]};
+                        double tx[2], ty[2], tz[2];
+                        cells_field<2>(ux, uy, uz, Gx, Gy, Gz, ww, s_off, s_nu, S, pc, spc, tx, ty, tz);
+                        finish_target(r, tx[0], ty[0], tz[0]);
+                        finish_target(r + 1, tx[1], ty[1], tz[1]);
+                    } else if (r * CELLS_THREADS < n) {                // uniform: one (partial) round
+                        const int pc[1] = {min(r * CELLS_THREADS + tid, n - 1)};
+                        const int spc[1] = {sp[r]};
+                        double tx[1], ty[1], tz[1];
+                        cells_field<1>(ux, uy, uz, Gx, Gy, Gz, ww, s_off, s_nu, S, pc, spc, tx, ty, tz);
+                        finish_target(r, tx[0], ty[0], tz[0]);
                     }
                 }
                 cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
