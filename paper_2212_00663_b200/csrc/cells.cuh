@@ -39,7 +39,7 @@ struct CellsCfg {
     // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / ux uy uz (pass 2)
     static constexpr int DPM = 10 + 3 * NQ;
     static size_t smem(int cap) {
-        return sizeof(double) * ((size_t)DPM * cap + 64 + 32) + sizeof(int) * (size_t)cap;
+        return sizeof(double) * ((size_t)DPM * cap + 64 + 32 + 3 * CELLS_THREADS) + sizeof(int) * (size_t)cap;
     }
 };
 
@@ -53,6 +53,61 @@ __device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_re
     double x = 0.0, y = 0.0;
     for (int k = 0; k < CELLS_THREADS / 32; ++k) { x += s_red[2 * k]; y += s_red[2 * k + 1]; }
     a = x; b = y;
+}
+
+// Pass 1 of one target against the sources [o0, o1) of its species, node slice i in [i0, i0 + NI): the partial
+// sums  sum_{ijl} a_i a_j a_l k (1 + ln rho)  of Eq. (22) (without the prefactor).  NI = NQ is the whole gradient;
+// NI < NQ lets several threads share one target (small cells), each recomputing the exponential.
+template <int NQ, int NI>
+__device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, double px, double py, double pz,
+                                                   const double* __restrict__ xk, const double* __restrict__ yk,
+                                                   const double* __restrict__ zk, const double* __restrict__ ww,
+                                                   const double* __restrict__ tab, const double* __restrict__ s_e2,
+                                                   const double (&kn)[NQ], const double (&ga)[NQ], double lognorm,
+                                                   double& gx, double& gy, double& gz) {
+    double acc[NI][NQ][NQ];
+#pragma unroll
+    for (int i = 0; i < NI; ++i)
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+            for (int l = 0; l < NQ; ++l) acc[i][j][l] = 0.0;
+#pragma unroll 2
+    for (int q = o0; q < o1; ++q) {
+        const double dx = px - xk[q], dy = py - yk[q], dz = pz - zk[q];
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        const double c = ww[q] * exp_neg_tab(r2, s_e2);
+        const double* t = tab + (size_t)q * 3 * NQ;
+        double ty[NQ], tz[NQ];
+#pragma unroll
+        for (int j = 0; j < NQ; ++j) { ty[j] = t[NQ + j]; tz[j] = t[2 * NQ + j]; }
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            const double cx = c * t[i0 + i];
+#pragma unroll
+            for (int j = 0; j < NQ; ++j) {
+                const double cxy = cx * ty[j];
+#pragma unroll
+                for (int l = 0; l < NQ; ++l) acc[i][j][l] = fma(cxy, tz[l], acc[i][j][l]);
+            }
+        }
+    }
+    gx = gy = gz = 0.0;
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        double ki = kn[0], gi = ga[0];                                // kn[i0 + i] without dynamic register indexing
+#pragma unroll
+        for (int m = 1; m < NQ; ++m) if (m == i0 + i) { ki = kn[m]; gi = ga[m]; }
+#pragma unroll
+        for (int j = 0; j < NQ; ++j)
+#pragma unroll
+            for (int l = 0; l < NQ; ++l) {
+                const double lnrho = lognorm + log(acc[i][j][l])
+                                     - ((ki * ki + kn[j] * kn[j] + kn[l] * kn[l]) + 2.0 * (ki * px + kn[j] * py + kn[l] * pz));
+                const double t = gi * ga[j] * ga[l] * (1.0 + lnrho);
+                gx = fma(t, ki, gx); gy = fma(t, kn[j], gy); gz = fma(t, kn[l], gz);
+            }
+    }
 }
 
 // Pass 2 of NT targets of one thread against every source of the cell (sources read once per NT targets:
@@ -107,7 +162,8 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
     double* ux = tab; double* uy = ux + cap; double* uz = uy + cap;
     double* s_e2 = tab + (size_t)3 * NQ * cap;            // [64]
     double* s_red = s_e2 + 64;                            // [32]
-    int* idx = reinterpret_cast<int*>(s_red + 32);        // [cap] caller index (within the cell) of slot p
+    double* s_part = s_red + 32;                          // [GF][3][TPG] partial sums of split targets (small cells)
+    int* idx = reinterpret_cast<int*>(s_part + 3 * CELLS_THREADS);   // [cap] caller index (within the cell) of slot p
     __shared__ int s_off[LD_MAX_SPECIES + 1];
     __shared__ int s_wcnt[CELLS_THREADS / 32];
     __shared__ int s_cell, s_status;
@@ -174,6 +230,9 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             if (tid == 0) { rec.status = s_status != 0 ? s_status : -1; records[cell] = rec; }
             continue;
         }
+        // threads per target: small cells (NQ = 4 only) put 2 or 4 threads on every target
+        const int GF = (NQ == 4) ? (n <= CELLS_THREADS / 4 ? 4 : (n <= CELLS_THREADS / 2 ? 2 : 1)) : 1;
+        const int TPG = CELLS_THREADS / GF, part = tid / TPG, tg = tid % TPG;
         for (int step = 0; step < n_steps && s_status == 0; ++step) {
             // ---- pass 1 (Eq. 22, factorised): G_p for every species, sources = same species of this cell
             for (int s = 0; s < S; ++s) {
@@ -219,54 +278,46 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 __syncthreads();
                 const double lognorm = -1.5 * log(2.0 * PI * eps);
                 const double pref = -sqrt(2.0 / eps) / (PI * sqrt(PI));
-                for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
-                    const int pt = r0 + tid;
-                    const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
+                if (GF > 1) {
+                    // small cell: GF threads per target, each a slice of NQ/GF x-node indices; partial sums meet in
+                    // shared memory and are added in part order (deterministic)
+                    const int pt = o0 + tg;
+                    const int p = min(pt, o1 - 1);
                     const double px = xk[p], py = yk[p], pz = zk[p];
-                    double acc[NQ][NQ][NQ];
-#pragma unroll
-                    for (int i = 0; i < NQ; ++i)
-#pragma unroll
-                        for (int j = 0; j < NQ; ++j)
-#pragma unroll
-                            for (int l = 0; l < NQ; ++l) acc[i][j][l] = 0.0;
-#pragma unroll 2
-                    for (int q = o0; q < o1; ++q) {
-                        const double dx = px - xk[q], dy = py - yk[q], dz = pz - zk[q];
-                        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                        const double c = ww[q] * exp_neg_tab(r2, s_e2);
-                        const double* t = tab + (size_t)q * 3 * NQ;
-                        double ty[NQ], tz[NQ];
-#pragma unroll
-                        for (int j = 0; j < NQ; ++j) { ty[j] = t[NQ + j]; tz[j] = t[2 * NQ + j]; }
-#pragma unroll
-                        for (int i = 0; i < NQ; ++i) {
-                            const double cx = c * t[i];
-#pragma unroll
-                            for (int j = 0; j < NQ; ++j) {
-                                const double cxy = cx * ty[j];
-#pragma unroll
-                                for (int l = 0; l < NQ; ++l) acc[i][j][l] = fma(cxy, tz[l], acc[i][j][l]);
-                            }
+                    double gx, gy, gz;
+                    if (GF == 2)
+                        cells_pass1_target<NQ, (NQ >= 2 ? NQ / 2 : 1)>(part * (NQ / 2), o0, o1, px, py, pz, xk, yk, zk, ww,
+                                                                       tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                    else
+                        cells_pass1_target<NQ, (NQ >= 4 ? NQ / 4 : 1)>(part * (NQ / 4), o0, o1, px, py, pz, xk, yk, zk, ww,
+                                                                       tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                    s_part[(part * 3 + 0) * TPG + tg] = gx;
+                    s_part[(part * 3 + 1) * TPG + tg] = gy;
+                    s_part[(part * 3 + 2) * TPG + tg] = gz;
+                    __syncthreads();
+                    if (part == 0 && pt < o1) {
+                        double a = 0.0, b = 0.0, c = 0.0;
+                        for (int g2 = 0; g2 < GF; ++g2) {
+                            a += s_part[(g2 * 3 + 0) * TPG + tg]; b += s_part[(g2 * 3 + 1) * TPG + tg];
+                            c += s_part[(g2 * 3 + 2) * TPG + tg];
                         }
+                        a *= pref; b *= pref; c *= pref;
+                        if (!(isfinite(a) && isfinite(b) && isfinite(c))) s_status = -4;
+                        Gx[p] = a; Gy[p] = b; Gz[p] = (T->dim == 2) ? 0.0 : c;
                     }
-                    double gx = 0.0, gy = 0.0, gz = 0.0;
-#pragma unroll
-                    for (int i = 0; i < NQ; ++i)
-#pragma unroll
-                        for (int j = 0; j < NQ; ++j)
-#pragma unroll
-                            for (int l = 0; l < NQ; ++l) {
-                                const double lnrho = lognorm + log(acc[i][j][l])
-                                                     - ((kn[i] * kn[i] + kn[j] * kn[j] + kn[l] * kn[l])
-                                                        + 2.0 * (kn[i] * px + kn[j] * py + kn[l] * pz));
-                                const double t = ga[i] * ga[j] * ga[l] * (1.0 + lnrho);
-                                gx = fma(t, kn[i], gx); gy = fma(t, kn[j], gy); gz = fma(t, kn[l], gz);
-                            }
-                    gx *= pref; gy *= pref; gz *= pref;
-                    if (pt < o1) {
-                        if (!(isfinite(gx) && isfinite(gy) && isfinite(gz))) s_status = -4;
-                        Gx[p] = gx; Gy[p] = gy; Gz[p] = (T->dim == 2) ? 0.0 : gz;
+                } else {
+                    for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
+                        const int pt = r0 + tid;
+                        const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
+                        const double px = xk[p], py = yk[p], pz = zk[p];
+                        double gx, gy, gz;
+                        cells_pass1_target<NQ, NQ>(0, o0, o1, px, py, pz, xk, yk, zk, ww, tab, s_e2, kn, ga, lognorm, gx,
+                                                   gy, gz);
+                        gx *= pref; gy *= pref; gz *= pref;
+                        if (pt < o1) {
+                            if (!(isfinite(gx) && isfinite(gy) && isfinite(gz))) s_status = -4;
+                            Gx[p] = gx; Gy[p] = gy; Gz[p] = (T->dim == 2) ? 0.0 : gz;
+                        }
                     }
                 }
                 __syncthreads();
@@ -308,6 +359,37 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         nx[r] = a; ny[r] = b; nz[r] = c;
                     }
                 };
+                if (GF > 1) {
+                    // small cell: the GF threads of a target take consecutive slices of every source species
+                    const int pc = min(tg, n - 1);
+                    int spt = 0;
+                    for (int t = 1; t < S; ++t) spt += (pc >= s_off[t]) ? 1 : 0;
+                    const double px = ux[pc], py = uy[pc], pz = uz[pc], hx = Gx[pc], hy = Gy[pc], hz = Gz[pc];
+                    double tx = 0.0, ty = 0.0, tz = 0.0;
+                    for (int sb = 0; sb < S; ++sb) {
+                        const int q0 = s_off[sb], len = s_off[sb + 1] - q0;
+                        const int qa = q0 + (len * part) / GF, qb = q0 + (len * (part + 1)) / GF;
+                        double ax = 0.0, ay = 0.0, az = 0.0;
+#pragma unroll 4
+                        for (int q = qa; q < qb; ++q)
+                            pair_accumulate(px - ux[q], py - uy[q], pz - uz[q], hx - Gx[q], hy - Gy[q], hz - Gz[q], ww[q],
+                                            ax, ay, az);
+                        const double nu = s_nu[spt * S + sb];
+                        tx = fma(nu, ax, tx); ty = fma(nu, ay, ty); tz = fma(nu, az, tz);
+                    }
+                    s_part[(part * 3 + 0) * TPG + tg] = tx;
+                    s_part[(part * 3 + 1) * TPG + tg] = ty;
+                    s_part[(part * 3 + 2) * TPG + tg] = tz;
+                    __syncthreads();
+                    if (part == 0) {
+                        double a = 0.0, b = 0.0, c = 0.0;
+                        for (int g2 = 0; g2 < GF; ++g2) {
+                            a += s_part[(g2 * 3 + 0) * TPG + tg]; b += s_part[(g2 * 3 + 1) * TPG + tg];
+                            c += s_part[(g2 * 3 + 2) * TPG + tg];
+                        }
+                        finish_target(0, a, b, c);
+                    }
+                } else
 #pragma unroll
                 for (int r = 0; r < CELLS_ROUNDS; r += 2) {
                     if ((r + 1) * CELLS_THREADS < n) {                 // uniform: two rounds of targets share the sources
