@@ -138,6 +138,15 @@ int landau_set_dimension(landau_ctx* ctx, int dim);
  * Anderson solver. */
 int landau_set_step_graph(landau_ctx* ctx, int mode);
 
+/* SURVEY.md NEXT-4 (robustness): what landau_step / landau_run do with a step whose fixed point does not converge
+ * within max_iter.  max_halvings = 0 (default) is the paper's behaviour: the last iterate is committed and status 1
+ * returned, at the price of an energy jump (reading S8).  max_halvings = k > 0: such a step
+ * is NOT committed but redone as two steps of dt/2, recursively up to k levels (only the deepest level commits an
+ * unconverged iterate).  Every sub-step is a step of Eq. (24), so the conservation laws hold for each of them.
+ * info then reports the summed iterations, the largest residual and converged = all sub-steps converged.  The loop
+ * is driven from the host (one synchronisation per sub-step). */
+int landau_set_substep(landau_ctx* ctx, int max_halvings);
+
 /* how landau_step / landau_run solve Eq. (24).  solver 0 (default) = the paper's plain
  * Jacobi fixed-point iteration; solver 1 = the same fixed point with Anderson acceleration of the given
  * depth (1..10, 3 to 5 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the

@@ -52,7 +52,8 @@ struct StepCtrl {
     int err;
     double residual;
     unsigned int ticket; // last-block-done counter of the residual reduction
-    int _r[3];
+    int hold;            // 1: step_commit keeps v^n when the step did not converge (adaptive sub-stepping)
+    int _r[2];
 };
 
 struct StepRecord {      // mirrors landau_step_info (host struct) field by field

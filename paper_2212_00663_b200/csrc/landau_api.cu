@@ -81,6 +81,7 @@ struct landau_ctx {
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
     int dim = 3;                          // landau_set_dimension
+    int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
     AndersonCtrl* d_aa = nullptr;
     Buf aa_hist;
@@ -955,7 +956,7 @@ int landau_get_markers_host(landau_ctx* c, double* v_out) {
     return finish(c, cl, "get_markers_host");
 }
 
-int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, landau_step_info* info) {
+static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, landau_step_info* info, int hold) {
     if (!c) return LANDAU_EINVAL;
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step: no markers held (landau_set_markers first)");
@@ -973,7 +974,11 @@ int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, 
     cudaStream_t st = c->stream;
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
-    const bool graph_ok = c->graph_mode != 0 && !c->sg.failed && !c->prof_on && c->solver == 0 &&
+    if (hold) {
+        const int one = 1;
+        CU(cudaMemcpyAsync(&c->d_ctrl->hold, &one, sizeof(int), cudaMemcpyHostToDevice, st));
+    }
+    const bool graph_ok = !hold && c->graph_mode != 0 && !c->sg.failed && !c->prof_on && c->solver == 0 &&
                           (c->graph_mode == 2 || npm <= 65536);
     std::vector<char> via_graph(n_steps, 0);
     for (int n = 0; n < n_steps; ++n) {
@@ -1071,6 +1076,49 @@ int landau_set_dimension(landau_ctx* c, int dim) {
     c->state.G_valid = false; c->tmp.G_valid = false;
     CU(cudaMemcpyAsync(&c->d_tab->dim, &c->dim, sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+// One step of length dt with up to `depth` levels of halving: a step whose fixed point does not converge is not
+// committed (StepCtrl::hold) and is redone as two steps of dt/2.  Every sub-step is a step of Eq. (24), so momentum
+// and energy are conserved by each of them.  At depth 0 the step is committed whatever happens (reading S8).
+static int advance_adaptive(landau_ctx* c, double dt, double tol, int max_iter, int depth, landau_step_info* acc) {
+    landau_step_info one = {0, 0.0, 0};
+    const int rc = run_steps(c, 1, dt, tol, max_iter, &one, depth > 0 ? 1 : 0);
+    if (rc < 0) return rc;
+    acc->iterations += one.iterations;
+    if (one.converged || depth == 0) {
+        acc->residual = one.residual > acc->residual ? one.residual : acc->residual;
+        if (!one.converged) acc->converged = 0;
+        return 0;
+    }
+    c->state.G_valid = true;            // nothing moved: G^n of the refused step is still the entropy gradient of v^n
+    for (int half = 0; half < 2; ++half) {
+        const int r2 = advance_adaptive(c, 0.5 * dt, tol, max_iter, depth - 1, acc);
+        if (r2 < 0) return r2;
+    }
+    return 0;
+}
+
+int landau_run(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, landau_step_info* info) {
+    if (!c) return LANDAU_EINVAL;
+    if (c->substep == 0) return run_steps(c, n_steps, dt, tol, max_iter, info, 0);
+    if (n_steps < 1) return fail(c, LANDAU_EINVAL, "step: need n_steps >= 1");
+    int any_unconverged = 0;
+    for (int n = 0; n < n_steps; ++n) {
+        landau_step_info acc = {0, 0.0, 1};
+        const int rc = advance_adaptive(c, dt, tol, max_iter, c->substep, &acc);
+        if (rc < 0) return rc;
+        if (info) info[n] = acc;
+        if (!acc.converged) any_unconverged = 1;
+    }
+    return any_unconverged ? LANDAU_NOT_CONVERGED : LANDAU_OK;
+}
+
+int landau_set_substep(landau_ctx* c, int max_halvings) {
+    if (!c) return LANDAU_EINVAL;
+    if (max_halvings < 0 || max_halvings > 10) return fail(c, LANDAU_EINVAL, "set_substep: max_halvings must be 0..10");
+    c->substep = max_halvings;
     return 0;
 }
 

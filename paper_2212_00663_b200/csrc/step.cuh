@@ -146,6 +146,7 @@ __global__ void step_commit_kernel(const DevLayout* __restrict__ L, StepCtrl* __
     }
     if (p >= npad_max || p >= L->npad) return;
     if (ctrl->err) return;
+    if (ctrl->hold && !ctrl->converged) return;      // adaptive sub-stepping: the caller retries with a shorter step
     xn[p] = xk[p]; yn[p] = yk[p]; zn[p] = zk[p];
 }
 

@@ -666,3 +666,34 @@ def test_graph_step_is_bit_identical_to_the_launch_sequence(B, cfg, n):
     assert ga.step(wl.dt, 1e-15, 3) == gb.step(wl.dt, 1e-15, 3)
     assert ga.step(wl.dt, 1e-15, 3) == gb.step(wl.dt, 1e-15, 3)
     assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+
+
+def test_substep_redoes_unconverged_steps_as_half_steps(B, oracle_mod):
+    """landau_set_substep: a step that cannot converge within max_iter is refused (state untouched) and redone as two
+    half steps; the result must equal the oracle's two converged steps of dt/2, and energy must be conserved where
+    the plain (committing) step leaks it."""
+    wl = W.make(0, n_per_species=256, shuffled=True)
+    dt, max_iter = 0.08, 20                       # the full step needs 34 iterations, the half steps 17
+    g, o = make_pair(B, oracle_mod, wl)
+    gp = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gp.set_markers(wl.v, wl.w, wl.species_id)
+    rc_plain = gp.step(dt, 1e-12, max_iter)
+    assert rc_plain[0] == 1 and not rc_plain[3]
+    g.set_substep(2)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(dt, 1e-12, max_iter)
+    assert rc == 0 and conv and it > max_iter      # iterations of the refused attempt + the half steps
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    for _ in range(2):
+        assert o.step(0.5 * dt, 1e-12, max_iter)[0] == 0
+    assert_field_close(g.get_markers().cpu().numpy(), o.get_markers(), wl.species_id, wl.n_species, tol=1e-11,
+                       what="state after two half steps")
+    m1 = g.moments(with_entropy=False)
+    mp = gp.moments(with_entropy=False)
+    K0 = m0["K"].sum()
+    assert abs(m1["K"].sum() - K0) <= TOL_DRIFT * K0
+    assert abs(mp["K"].sum() - K0) > 100 * TOL_DRIFT * K0          # what the committed unconverged step costs
+    with pytest.raises(B.LandauError):
+        g.set_substep(11)
+    g.set_substep(0)
