@@ -35,12 +35,14 @@ def _kurtosis(mass, n, P, stress, m4):
 
 
 def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1, verbose: bool = False,
-                solver: int = 0, depth: int = 3):
+                solver: int = 0, depth: int = 3, substep: int = 0):
     wl = W.make(config, n_per_species=n_per_species)
     n_steps = int(steps if steps is not None else wl.n_steps)
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
     if solver:
         g.set_solver(solver, depth)
+    if substep:
+        g.set_substep(substep)
     g.set_markers(wl.v, wl.w, wl.species_id)
     S = wl.n_species
     cols = dict(t=[], iterations=[], residual=[], converged=[], K=[], S_eps=[], T=[], T_axis=[], kurt=[], P=[])
@@ -72,7 +74,7 @@ def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1,
     wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
     summary = dict(config=config, workload=wl.name, n_markers=wl.n_markers, n_species=S, steps=n_steps, dt=wl.dt,
                    n_q=wl.n_q, eps=wl.eps.tolist(), kernels=g.last_kernels(),
-                   solver="jacobi" if not solver else f"anderson depth {depth}", wall_s=wall,
+                   solver="jacobi" if not solver else f"anderson depth {depth}", substep_levels=substep, wall_s=wall,
                    steps_per_s=n_steps / wall, iterations_mean=float(H["iterations"][1:].mean()),
                    iterations_max=int(H["iterations"].max()), steps_not_converged=not_conv,
                    energy_drift_rel_max=float(np.abs(K - K[0]).max() / K[0]),
@@ -126,10 +128,12 @@ def main():
     ap.add_argument("--out", default="gpurun_out")
     ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi")
     ap.add_argument("--anderson-depth", type=int, default=3)
+    ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
     ap.add_argument("--tag", default="", help="suffix of the output file names")
     args = ap.parse_args()
     wl, H, summary = run_history(args.config, args.n_per_species, args.steps, verbose=True,
-                                 solver=1 if args.solver == "anderson" else 0, depth=args.anderson_depth)
+                                 solver=1 if args.solver == "anderson" else 0, depth=args.anderson_depth,
+                                 substep=args.substep)
     write(Path(args.out), f"{args.config}{args.tag}", H, summary)
     print(json.dumps(summary))
 
