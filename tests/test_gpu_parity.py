@@ -697,3 +697,57 @@ def test_substep_redoes_unconverged_steps_as_half_steps(B, oracle_mod):
     with pytest.raises(B.LandauError):
         g.set_substep(11)
     g.set_substep(0)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_fuzz_random_small_clouds(B, oracle_mod, seed):
+    """Randomised shapes: 1-5 species with random masses / charges / temperatures / drifts, ragged counts
+    (including 0 and 1), n_q 2-5, random kernel variants; field, entropy and one step against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    S = int(rng.integers(1, 6))
+    mass = np.exp(rng.uniform(0.0, 9.0, S)); mass[0] = 1.0
+    charge = rng.choice([-1.0, 1.0, 2.0], S)
+    counts = rng.integers(0, 260, S); counts[int(rng.integers(0, S))] = max(1, counts.max())
+    if seed % 4 == 0:
+        counts[-1] = 1
+    T = rng.uniform(0.3, 2.0, S)
+    vs, ws, ss = [], [], []
+    for s in range(S):
+        vs.append(rng.standard_normal((counts[s], 3)) * np.sqrt(T[s] / mass[s]) + rng.normal(0, 0.3, 3) * np.sqrt(T[s] / mass[s]))
+        ws.append((0.2 + rng.random(counts[s])) / max(1, counts[s]))
+        ss.append(np.full(counts[s], s, dtype=np.int32))
+    v, w, sid = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss)
+    perm = rng.permutation(len(w))
+    v, w, sid = v[perm], w[perm], sid[perm]
+    eps = rng.uniform(0.03, 0.2, S) * T / mass
+    n_q = int(rng.integers(2, 6))
+    variant = KERNEL_VARIANTS[int(rng.integers(0, len(KERNEL_VARIANTS)))]
+    g = B.Landau(mass, charge, eps, n_q=n_q, **variant)
+    o = oracle_mod.LandauRef(mass, charge, eps, n_q=n_q)
+    g.set_step_graph(int(rng.integers(0, 3)))
+    def close(got, ref, floors, what, tol=TOL_FIELD):
+        """per species: |got - ref| <= tol * max(|ref|, floor); a lone marker has G = V = 0 analytically, so its
+        reference is round-off and needs the floor (the natural size of the quantity for that species)"""
+        assert np.all(np.isfinite(got))
+        for s in range(S):
+            m = sid == s
+            if m.any():
+                err, scale = np.linalg.norm(got[m] - ref[m]), max(np.linalg.norm(ref[m]), floors[s])
+                assert err <= tol * scale, f"{what} species {s}: {err:.3e} vs scale {scale:.3e}"
+
+    Gref, Sref = o.entropy_grad(v, w, sid, with_entropy=True)
+    Ggot, Sgot = g.entropy_grad(v, w, sid, with_entropy=True)
+    close(Ggot.cpu().numpy(), Gref, np.sqrt(np.maximum(counts, 1) / eps), f"fuzz {seed} G")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+    Vref = o.eval_field(v, w, sid)
+    vfloor = np.full(S, 1e-3 * np.linalg.norm(Vref) / np.sqrt(mass.max()))
+    close(g.eval_field(v, w, sid).cpu().numpy(), Vref, vfloor, f"fuzz {seed} V")
+    # a step short enough to contract for any of these clouds
+    vmax = np.abs(Vref).max() / max(np.abs(v).max(), 1e-300)
+    dt = min(0.01, 0.02 / max(vmax, 1e-300))
+    g.set_markers(v, w, sid); o.set_markers(v, w, sid)
+    for _ in range(2):
+        rg = g.step(dt, 1e-12, 80); ro = o.step(dt, 1e-12, 80)
+        assert rg[0] == ro[0] and abs(rg[1] - ro[1]) <= 1
+    if rg[0] == 0:
+        close(g.get_markers().cpu().numpy(), o.get_markers(), np.zeros(S), f"fuzz {seed} state", tol=1e-11)
