@@ -751,3 +751,41 @@ def test_fuzz_random_small_clouds(B, oracle_mod, seed):
         assert rg[0] == ro[0] and abs(rg[1] - ro[1]) <= 1
     if rg[0] == 0:
         close(g.get_markers().cpu().numpy(), o.get_markers(), np.zeros(S), f"fuzz {seed} state", tol=1e-11)
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_fuzz_cells_against_the_single_cell_path(B, seed):
+    """Random ragged batches (cell sizes 0..1024, every thread-split variant of the fused kernel, 1-3 species present
+    per cell): every cell must equal the single-cell path (itself checked against the oracle) after 3 steps."""
+    rng = np.random.default_rng(500 + seed)
+    ref4 = W.make(4, n_per_species=4)
+    mass, charge = ref4.mass, ref4.charge
+    eps = 0.05 / mass
+    sizes = list(rng.integers(0, 300, 14)) + [int(rng.integers(20, 64)), int(rng.integers(65, 128)), 1024, 777]
+    rng.shuffle(sizes)
+    vs, ws, ss, off = [], [], [], [0]
+    for n in sizes:
+        present = rng.choice(3, size=int(rng.integers(1, 4)), replace=False)
+        sid = rng.choice(present, size=n).astype(np.int32)
+        vs.append(rng.standard_normal((n, 3)) / np.sqrt(mass[sid])[:, None])
+        ws.append((0.5 + rng.random(n)) / max(n, 1))
+        ss.append(sid)
+        off.append(off[-1] + n)
+    v, w, sid, off = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss), np.array(off, dtype=np.int64)
+    g = B.Landau(mass, charge, eps)
+    dt, n_steps = 5e-4, 3
+    rc, vout, info = g.cells_run(off, v, w, sid, n_steps, dt, 1e-12, 80)
+    vout = vout.cpu().numpy()
+    assert rc in (0, 1)
+    gs = B.Landau(mass, charge, eps)
+    for k in range(len(sizes)):
+        a, b = off[k], off[k + 1]
+        if a == b:
+            continue
+        gs.set_markers(v[a:b], w[a:b], sid[a:b])
+        rcs, infos = gs.run(n_steps, dt, 1e-12, 80)
+        ref = gs.get_markers().cpu().numpy()
+        assert int(info["steps_not_converged"][k]) == sum(0 if i[2] else 1 for i in infos)
+        if rcs == 0:
+            assert abs(int(info["iterations"][k]) - sum(i[0] for i in infos)) <= n_steps
+            assert rel_l2(vout[a:b], ref) <= 1e-11, (k, b - a)
