@@ -493,15 +493,23 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
         *nparts_out = nchunks;
         return 0;
     }
-    constexpr int R = 2;
+#ifndef LANDAU_ONESIDED_WAVES  // tuning knob (build.py: LANDAU_NVCC_EXTRA): blocks per SM the source chunking aims at
+#define LANDAU_ONESIDED_WAVES 8
+#endif
+    // targets per thread: 2, or 1 for the smallest clouds (more blocks matter more than source reuse there)
+    const int R = cl.npad_max <= 1024 ? 1 : 2;
     const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * R);
     const int stiles = cl.npad_max / PAIR_SRC_TILE;
-    int nchunks = std::max(1, std::min(stiles, ceil_div(5 * c->sm_count, ttiles)));
+    int nchunks = std::max(1, std::min(stiles, ceil_div(LANDAU_ONESIDED_WAVES * c->sm_count, ttiles)));
     nchunks = std::min(nchunks, 32);
     RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
     dim3 grid(ttiles, nchunks);
-    pair_onesided_kernel<R><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
-                                                                 cl.recs(), (double*)c->vpart.p);
+    if (R == 1)
+        pair_onesided_kernel<1><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
+                                                                     cl.recs(), (double*)c->vpart.p);
+    else
+        pair_onesided_kernel<2><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
+                                                                     cl.recs(), (double*)c->vpart.p);
     c->launches += 1;
     *nparts_out = nchunks;
     return 0;
