@@ -1,0 +1,176 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (-m gpu).
+
+The oracle cannot evaluate a whole field at >= 1e5 markers in test time (pass 1 alone is 8e11 exponentials at
+3 x 2^16), but each OUTPUT ROW is a plain sum it computes one by one (`landau_ref_*_rows`): pass 1 and pass 2 are
+compared on sampled rows, the implicit step by re-evaluating Eq. (24) with oracle rows at the
+midpoint the CUDA path returned, and the conservation laws (Eqs. 27, 29) hold at any size.
+These tests replace the uncommitted parity report BASELINE.md section 3 used to cite; they print the measured
+errors (run with -s to see them; profiles/r2_config_size_parity.md keeps one run).
+"""
+import json
+import os
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2212_00663_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-10     # north_star: relative L2 over markers, overall and per species
+TOL_DRIFT = 1e-12     # north_star: per-step relative drift of momentum and energy
+REPORT = {}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the CUDA path has no fallback")
+    from paper_2212_00663_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module", autouse=True)
+def write_report():
+    yield
+    out = Path(os.environ.get("GRAFT_REPO_ROOT", Path(__file__).resolve().parent.parent)) / "gpurun_out"
+    try:
+        out.mkdir(exist_ok=True)
+        (out / "config_size_parity.json").write_text(json.dumps(REPORT, indent=1))
+    except OSError:
+        pass
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def sample_rows(wl, per_species, seed):
+    rng = np.random.default_rng(seed)
+    return np.sort(np.concatenate([rng.choice(np.flatnonzero(wl.species_id == s), per_species, replace=False)
+                                   for s in range(wl.n_species)])).astype(np.int64)
+
+
+def per_species_errors(got, ref, sid, S):
+    e = {"all": rel_l2(got, ref)}
+    for s in range(S):
+        m = sid == s
+        e[f"s{s}"] = rel_l2(got[m], ref[m])
+    return e
+
+
+@pytest.mark.parametrize("cfg,nps", [(4, 1 << 16), (4, 1 << 17), (3, 32768), (2, 8192), (1, 4096)])
+def test_pair_field_config_size_sampled_rows(B, oracle_mod, cfg, nps):
+    """Pass 2 with the AUTOMATIC kernel choice (the symmetric action-reaction kernel at these sizes) at the bench
+    workload 3 x 2^16, the largest single-GPU config 3 x 2^17 and configs 1-3 at full size: sampled target rows
+    against the oracle's literal Eq. (23) (each row a sum over all N - 1 sources), plus Eqs. 27 and 29."""
+    wl = W.make(cfg, n_per_species=nps, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    rng = np.random.default_rng(31 + cfg)
+    G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+    got = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    if wl.n_markers >= 16384:
+        assert "pair=sym" in g.last_kernels()
+    rows = sample_rows(wl, 64, 41 + cfg)
+    ref = o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows)
+    err = per_species_errors(got[rows], ref, wl.species_id[rows], wl.n_species)
+    REPORT[f"pair_field c{cfg} {wl.n_species}x{nps}"] = dict(err, rows=len(rows), kernels=g.last_kernels())
+    print(f"pass 2 c{cfg} {wl.n_species} x {nps}: {err} [{g.last_kernels()}]")
+    assert np.all(np.isfinite(got)) and max(err.values()) <= TOL_FIELD, err
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    assert np.abs((wm * got).sum(axis=0)).max() <= 1e-13 * np.abs(wm * got).sum()          # Eq. 27
+    assert abs((wm * wl.v * got).sum()) <= 1e-13 * np.abs(wm * wl.v * got).sum()             # Eq. 29
+
+
+@pytest.mark.parametrize("cfg,nps", [(4, 1 << 17), (3, 32768), (2, 8192)])
+def test_entropy_grad_config_size_sampled_rows(B, oracle_mod, cfg, nps):
+    """Pass 1 (automatic kernel) at the sizes test_gpu_parity.py does not reach: sampled rows vs literal Eq. (22)."""
+    wl = W.make(cfg, n_per_species=nps, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    rows = sample_rows(wl, 12 if nps > 40000 else 24, 51 + cfg)
+    ref = o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows)
+    err = per_species_errors(G[rows], ref, wl.species_id[rows], wl.n_species)
+    REPORT[f"entropy_grad c{cfg} {wl.n_species}x{nps}"] = dict(err, rows=len(rows), kernels=g.last_kernels())
+    print(f"pass 1 c{cfg} {wl.n_species} x {nps}: {err} [{g.last_kernels()}]")
+    assert np.all(np.isfinite(G)) and max(err.values()) <= TOL_FIELD, err
+
+
+@pytest.mark.parametrize("cfg,nps", [(4, 1 << 16), (3, 32768)])
+def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod, cfg, nps):
+    """One converged landau_step at the bench workload (3 x 2^16 markers, symmetric kernel, the launch sequence
+    bench.py times) and at config 3's full size, checked WITHOUT a full oracle step (which would take hours):
+
+      1. G^n of the CUDA path equals the oracle's literal Eq. (22) on sampled rows (<= 1e-10);
+      2. the returned v^{n+1} solves Eq. (24): on sampled rows  v1 - v0 - dt V_oracle[(v0 + v1)/2 ; G^n]  with
+         V_oracle = the oracle's literal Eq. (23) row sums at the returned midpoint.  The last Jacobi iterate
+         differs from the fixed point by <= rho tol |v1| (rho < 1 the contraction factor), so the defect is
+         bounded by tol = 1e-12 relative to the state in the residual's own energy norm; relative to the
+         displacement |v1 - v0| ~ dt |V| (1e-3 of the state here) that is <= 1e-8;
+      3. Eqs. (26)-(29): momentum and energy drift of the step <= 1e-12 (north_star)."""
+    wl = W.make(cfg, n_per_species=nps, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    rowsG = sample_rows(wl, 8, 61 + cfg)
+    errG = per_species_errors(G[rowsG], o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rowsG), wl.species_id[rowsG],
+                              wl.n_species)
+    assert max(errG.values()) <= TOL_FIELD, errG
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(wl.dt, wl.tol, wl.max_iter)
+    assert rc == 0 and conv and res <= wl.tol, (rc, it, res)
+    assert "pair=sym" in g.last_kernels()
+    v1 = g.get_markers().cpu().numpy()
+    m1 = g.moments(with_entropy=False)
+    rows = sample_rows(wl, 48, 71 + cfg)
+    u = 0.5 * (wl.v + v1)
+    Vo = o.pair_field_rows(u, wl.w, wl.species_id, G, rows)
+    defect = v1[rows] - wl.v[rows] - wl.dt * Vo
+    disp = v1[rows] - wl.v[rows]
+    wm = (wl.w * wl.mass[wl.species_id])[rows][:, None]
+    rel_state = float(np.sqrt((wm * defect ** 2).sum() / (wm * v1[rows] ** 2).sum()))
+    sid = wl.species_id[rows]
+    rel_disp = {f"s{s}": float(np.linalg.norm(defect[sid == s]) / np.linalg.norm(disp[sid == s]))
+                for s in range(wl.n_species)}
+    wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
+    dP = float(np.abs(m1["P"].sum(axis=0) - m0["P"].sum(axis=0)).max()) / wm_abs
+    dK = abs(float(m1["K"].sum() - m0["K"].sum())) / float(m0["K"].sum())
+    REPORT[f"step c{cfg} {wl.n_species}x{nps}"] = dict(iterations=it, residual=res, G_rows=errG, eq24_defect_rel_state=rel_state,
+                                                      eq24_defect_rel_displacement=rel_disp, momentum_drift=dP,
+                                                      energy_drift=dK, kernels=g.last_kernels())
+    print(f"step c{cfg} {wl.n_species} x {nps}: {it} iterations, residual {res:.2e}; Eq. (24) defect / state {rel_state:.2e}, "
+          f"/ displacement {rel_disp}; dP {dP:.1e}, dK/K {dK:.1e}")
+    assert rel_state <= 1e-12
+    assert max(rel_disp.values()) <= 1e-8, rel_disp
+    assert dP <= TOL_DRIFT and dK <= TOL_DRIFT
+
+
+def test_one_fixed_point_iterate_config_size_vs_oracle_rows(B, oracle_mod):
+    """A NON-converged step (max_iter = 2) at 3 x 2^16: the committed iterate v^(2) = v0 + dt V[(v0 + v^(1))/2],
+    v^(1) = v0 + dt V[v0], is reproduced on sampled rows from oracle row sums alone (two nested evaluations of
+    literal Eq. (23); the inner one needs every marker, so v^(1) is rebuilt from the CUDA path's field, itself
+    compared with the oracle on the same rows)."""
+    wl = W.make(4, n_per_species=1 << 16, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    rows = sample_rows(wl, 32, 81)
+    V0 = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    V0o = o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows)
+    assert max(per_species_errors(V0[rows], V0o, wl.species_id[rows], 3).values()) <= TOL_FIELD
+    v_1 = wl.v + wl.dt * V0
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = g.step(wl.dt, 0.0, 2)
+    assert (rc, it, conv) == (1, 2, False)
+    v2 = g.get_markers().cpu().numpy()
+    V1o = o.pair_field_rows(0.5 * (wl.v + v_1), wl.w, wl.species_id, G, rows)
+    err = per_species_errors(v2[rows] - wl.v[rows], wl.dt * V1o, wl.species_id[rows], 3)
+    REPORT["iterate c4 3x65536"] = err
+    print(f"second Jacobi iterate at 3 x 2^16 vs oracle rows: {err}")
+    assert max(err.values()) <= 1e-9, err
