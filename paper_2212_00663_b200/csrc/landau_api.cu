@@ -80,6 +80,10 @@ struct landau_ctx {
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab;
+    Buf sym_acc, sym_tpart, sym_ticket;   // symmetric pair kernel: in-place source sums, target segments, unit tickets
+    // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
+    bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {};
+    size_t attr_cells[LD_MAX_NQ + 1] = {};
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
@@ -117,6 +121,11 @@ struct landau_ctx {
 namespace {
 
 constexpr size_t PIN_BYTES = 1 << 16;
+// pinned read-back area: [0, 8) finish()'s {err, used_fact}; [PIN_CTRL, +sizeof(StepCtrl)) the step control block;
+// [PIN_MOM, ...) per-species moment sums
+constexpr size_t PIN_CTRL = 128, PIN_MOM = 512;
+static_assert(PIN_CTRL >= 2 * sizeof(int) && PIN_CTRL + sizeof(StepCtrl) <= PIN_MOM, "pinned read-back areas overlap");
+static_assert(PIN_MOM + sizeof(double) * LD_MAX_SPECIES * 16 <= PIN_BYTES, "pinned read-back area too small");
 
 int fail(landau_ctx* c, int code, const char* fmt, ...) {
     if (c) {
@@ -127,6 +136,19 @@ int fail(landau_ctx* c, int code, const char* fmt, ...) {
     }
     return code;
 }
+
+// Every entry point runs on the context's device and leaves the caller's current device as it found it.
+struct DevGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DevGuard(const landau_ctx* c) {
+        if (!c) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+    DevGuard(const DevGuard&) = delete;
+    DevGuard& operator=(const DevGuard&) = delete;
+};
 
 #define CU(call)                                                                              \
     do {                                                                                      \
@@ -282,20 +304,36 @@ int npad_upper(int64_t N, int S, int pad) {
 
 // ---- optimised kernels -----------------------------------------------------------------------
 int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; return cl.sym; }
-int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts) {
-    const int G = c->sm_count;
-    const size_t n = (size_t)G * 3 * cl.npad_max;
-    RC(ensure(c, c->vpart, sizeof(double) * n));
-    static bool attr_done = false;
-    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS>;
+// Buffers of the symmetric kernel's output path (pair_sym.cuh): O(N), whatever the grid.
+int ensure_sym_buffers(landau_ctx* c, const Cloud& cl, int G) {
+    const size_t npm = (size_t)cl.npad_max;
+    RC(ensure(c, c->vpart, sizeof(double) * 3 * npm));
+    RC(ensure(c, c->sym_acc, sizeof(double) * 3 * npm));
+    RC(ensure(c, c->sym_tpart, sizeof(double) * 3 * SymL::BT * (npm / SymL::BT + (size_t)G)));
+    RC(ensure(c, c->sym_ticket, sizeof(int) * (npm / SymL::BS + 1)));
+    return 0;
+}
+
+template <typename F>
+int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa, bool& attr_done, int* nparts) {
+    using Cfg = SymCfg<SYM_W, SYM_RT, SYM_RS, F>;
+    const int G = c->sm_count;                 // persistent grid, 1 CTA per SM: all CTAs co-resident (ticket waits)
+    RC(ensure_sym_buffers(c, cl, G));
+    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, F>;
     if (!attr_done) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SymL::SMEM));
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         attr_done = true;
     }
-    zero_slices_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(ctrl, (double2*)c->vpart.p, n / 2);
-    kern<<<G, SymL::THREADS, SymL::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, cl.soas(), (double*)c->vpart.p);
-    c->launches += 2;
-    *nparts = G;
+    const int npm = cl.npad_max;
+    sym_reset_kernel<<<c->sm_count, 256, 0, c->stream>>>(ctrl, (double*)c->sym_acc.p, 3 * (size_t)npm,
+                                                          (int*)c->sym_ticket.p, npm / SymL::BS + 1);
+    kern<<<G, Cfg::THREADS, Cfg::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, npm, soa, (double*)c->sym_acc.p,
+                                                    (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err);
+    sym_combine_kernel<<<ceil_div(npm, 256), 256, 0, c->stream>>>(cl.L(), ctrl, npm, G, SymL::BT, SymL::BS,
+                                                                   (const double*)c->sym_acc.p,
+                                                                   (const double*)c->sym_tpart.p, (double*)c->vpart.p);
+    c->launches += 3;
+    *nparts = 1;
     return 0;
 }
 
@@ -356,10 +394,9 @@ int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks) {
     entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p);
     auto kern = entropy_mma_kernel<NQ>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!c->attr_mma[NQ]) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)M::SMEM));
-        attr_done = true;
+        c->attr_mma[NQ] = true;
     }
     dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
     kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
@@ -452,29 +489,17 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     const bool fp32_field = c->precision == 1 && !ctrl;     // FP32 variant: field evaluation only
     if (use_sym && !fp32_field) {
-        RC(launch_pair_sym(c, cl, ctrl, nparts_out));
+        RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out));
         return 0;
     }
     if (c->precision == 1 && !ctrl && cl.sym) {             // FP32 field variant, symmetric kernel in FP32
-        using SymF = SymCfg<SYM_W, SYM_RT, SYM_RS, float>;
-        const int G = c->sm_count;
-        const size_t n = (size_t)G * 3 * cl.npad_max, n7 = 7 * (size_t)cl.npad_max;
-        RC(ensure(c, c->vpart, sizeof(double) * n));
+        const size_t n7 = 7 * (size_t)cl.npad_max;
         RC(ensure(c, c->soa32, sizeof(float) * n7));
-        auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, float>;
-        static bool attr_done = false;
-        if (!attr_done) {
-            CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SymF::SMEM));
-            attr_done = true;
-        }
         soa_to_f32_kernel<<<c->sm_count * 4, 256, 0, c->stream>>>(n7, cl.soas(), (float*)c->soa32.p);
-        zero_slices_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(nullptr, (double2*)c->vpart.p, n / 2);
-        kern<<<G, SymF::THREADS, SymF::SMEM, c->stream>>>(c->d_tab, cl.L(), nullptr, cl.npad_max,
-                                                          (const float*)c->soa32.p, (double*)c->vpart.p);
+        c->launches += 1;
+        RC(launch_pair_sym<float>(c, cl, nullptr, (const float*)c->soa32.p, c->attr_sym32, nparts_out));
         c->k_pair = "sym_f32";
         snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
-        c->launches += 3;
-        *nparts_out = G;
         return 0;
     }
     if (c->precision == 1 && !ctrl) {                       // FP32 field variant below the symmetric kernel's size
@@ -744,10 +769,9 @@ int launch_cells(landau_ctx* c, int n_cells, int cap, const double* v, const dou
                  double* v_out, int n_steps, double dt, double tol, int max_iter) {
     auto kern = cells_run_kernel<NQ>;
     const size_t smem = CellsCfg<NQ>::smem(cap);
-    static size_t attr_set = 0;
-    if (smem > attr_set) {
+    if (smem > c->attr_cells[NQ]) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = smem;
+        c->attr_cells[NQ] = smem;
     }
     int* counter = (int*)((char*)c->cells_off.p + sizeof(long long) * ((size_t)n_cells + 1));
     const int grid = std::min(n_cells, c->sm_count);
@@ -807,10 +831,13 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     gauss_hermite_gw(c->n_q, c->knot, c->gw);
 
     auto bail = [&](int code) { landau_destroy(c); return code; };
-    int ndev = 0;
+    int ndev = 0, caller_dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete c; return LANDAU_ECUDA; }
-    if (o.device >= 0) { if (cudaSetDevice(o.device) != cudaSuccess) { delete c; return LANDAU_ECUDA; } }
-    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return LANDAU_ECUDA; }
+    if (cudaGetDevice(&caller_dev) != cudaSuccess) { delete c; return LANDAU_ECUDA; }
+    c->device = o.device >= 0 ? o.device : caller_dev;
+    if (c->device >= ndev) { delete c; return LANDAU_ECUDA; }
+    DevGuard dev_guard(c);                 // the caller's current device is left untouched
+    { int cur = -1; if (cudaGetDevice(&cur) != cudaSuccess || cur != c->device) { delete c; return LANDAU_ECUDA; } }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     DevTable t;
     memset(&t, 0, sizeof(t));
@@ -836,6 +863,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
 
 void landau_destroy(landau_ctx* c) {
     if (!c) return;
+    DevGuard dev_guard(c);
     for (auto& ev : c->prof_events) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
     for (auto e : c->prof_pool) cudaEventDestroy(e);
     if (c->d_tab) cudaFree(c->d_tab);
@@ -852,7 +880,8 @@ void landau_destroy(landau_ctx* c) {
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
-                   &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32})
+                   &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32, &c->sym_acc,
+                   &c->sym_tpart, &c->sym_ticket})
         release(*b);
     delete c;
 }
@@ -866,6 +895,7 @@ int landau_get_quadrature(const landau_ctx* c, double* knots, double* weights) {
 int landau_entropy_grad(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid, double* G_out,
                         double* S_eps_out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (!G_out) return fail(c, LANDAU_EINVAL, "entropy_grad: NULL output");
     Cloud& cl = c->tmp;
     RC(pack(c, cl, N, v, w, sid));
@@ -874,7 +904,7 @@ int landau_entropy_grad(landau_ctx* c, int64_t N, const double* v, const double*
                                                                        cl.Gz(), G_out);
     c->launches += 1;
     if (S_eps_out) {
-        double* h = (double*)c->h_pin + 64;
+        double* h = (double*)((char*)c->h_pin + PIN_MOM);
         RC(species_sums(c, cl, true, false, h));
         const double PI = 3.14159265358979323846;
         for (int s = 0; s < c->S; ++s) S_eps_out[s] = -h[s * MOM_OUT + 11] / (PI * sqrt(PI));
@@ -885,6 +915,7 @@ int landau_entropy_grad(landau_ctx* c, int64_t N, const double* v, const double*
 int landau_pair_field(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid,
                       const double* G_in, double* out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (!G_in || !out) return fail(c, LANDAU_EINVAL, "pair_field: NULL array");
     Cloud& cl = c->tmp;
     c->k_entropy = "-";                       // the entropy gradient is supplied: no pass 1 in this call
@@ -898,6 +929,7 @@ int landau_pair_field(landau_ctx* c, int64_t N, const double* v, const double* w
 
 int landau_eval_field(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid, double* out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (!out) return fail(c, LANDAU_EINVAL, "eval_field: NULL output");
     Cloud& cl = c->tmp;
     RC(pack(c, cl, N, v, w, sid));
@@ -909,6 +941,7 @@ int landau_eval_field(landau_ctx* c, int64_t N, const double* v, const double* w
 int landau_eval_field_host(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid,
                            double* out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (!out) return fail(c, LANDAU_EINVAL, "eval_field_host: NULL output");
     const double *dv, *dw;
     const int32_t* ds;
@@ -924,6 +957,7 @@ int landau_eval_field_host(landau_ctx* c, int64_t N, const double* v, const doub
 
 int landau_set_markers(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     cl.N = 0;
     RC(pack(c, cl, N, v, w, sid));
@@ -934,6 +968,7 @@ int landau_set_markers(landau_ctx* c, int64_t N, const double* v, const double* 
 
 int landau_set_markers_host(landau_ctx* c, int64_t N, const double* v, const double* w, const int32_t* sid) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     const double *dv, *dw;
     const int32_t* ds;
     RC(stage_in(c, N, v, w, sid, &dv, &dw, &ds));
@@ -942,6 +977,7 @@ int landau_set_markers_host(landau_ctx* c, int64_t N, const double* v, const dou
 
 int landau_get_markers(landau_ctx* c, double* v_out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "get_markers: no markers held");
     if (!v_out) return fail(c, LANDAU_EINVAL, "get_markers: NULL output");
@@ -953,6 +989,7 @@ int landau_get_markers(landau_ctx* c, double* v_out) {
 
 int landau_get_markers_host(landau_ctx* c, double* v_out) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "get_markers: no markers held");
     if (!v_out) return fail(c, LANDAU_EINVAL, "get_markers: NULL output");
@@ -966,6 +1003,7 @@ int landau_get_markers_host(landau_ctx* c, double* v_out) {
 
 static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_iter, landau_step_info* info, int hold) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step: no markers held (landau_set_markers first)");
     if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
@@ -1053,7 +1091,7 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
     CU(cudaGetLastError());
     // one synchronisation: records + error flags
     std::vector<StepRecord> h(n_steps);
-    StepCtrl* hc = (StepCtrl*)c->h_pin;
+    StepCtrl* hc = (StepCtrl*)((char*)c->h_pin + PIN_CTRL);
     CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(h.data(), c->records.p, sizeof(StepRecord) * (size_t)n_steps, cudaMemcpyDeviceToHost, st));
     c->in_run = true;
@@ -1079,6 +1117,7 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
 
 int landau_set_dimension(landau_ctx* c, int dim) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (dim != 2 && dim != 3) return fail(c, LANDAU_EINVAL, "set_dimension: dim must be 2 or 3");
     c->dim = dim;
     c->state.G_valid = false; c->tmp.G_valid = false;
@@ -1157,6 +1196,7 @@ int landau_step(landau_ctx* c, double dt, double tol, int max_iter, landau_step_
 // one pass-2 evaluations of work).
 int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step_dg: no markers held (landau_set_markers first)");
     if (max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
@@ -1179,7 +1219,7 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     Cloud U = cl;  U.xyzw = c->dg_u;  U.G = c->dg_Gu;        // midpoint u, G(u)
     Cloud VK = cl; VK.xyzw = c->vk;   VK.G = c->dg_Gk;       // iterate v^(k), its entropy integrand
     const double PI = 3.14159265358979323846;
-    double* hs = (double*)c->h_pin + 64;
+    double* hs = (double*)((char*)c->h_pin + PIN_MOM);
     auto total_entropy = [&](Cloud& q, double* S_out) -> int {
         RC(species_sums(c, q, true, false, hs));
         double S = 0.0;
@@ -1199,7 +1239,7 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
                                                            cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
     CU(cudaMemcpyAsync(xk + 3 * (size_t)npm, cl.w(), sizeof(double) * (size_t)npm, cudaMemcpyDeviceToDevice, st));
     c->launches += 1;
-    StepCtrl* hc = (StepCtrl*)c->h_pin;
+    StepCtrl* hc = (StepCtrl*)((char*)c->h_pin + PIN_CTRL);
     std::vector<double> hp(2 * (size_t)ndb);
     for (int k = 0; k < max_iter; ++k) {
         int nparts = 0;
@@ -1251,6 +1291,7 @@ int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, con
                      const int32_t* sid, double* v_out, int n_steps, double dt, double tol, int max_iter,
                      landau_cell_info* info) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     if (n_cells < 1 || !cell_offset || !v || !w || !sid || !v_out)
         return fail(c, LANDAU_EINVAL, "cells_run: NULL array or n_cells < 1");
     if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
@@ -1298,10 +1339,11 @@ int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, con
 
 int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "moments: no markers held");
     if (S_eps && !cl.G_valid) RC(entropy(c, cl));
-    double* h = (double*)c->h_pin + 64;
+    double* h = (double*)((char*)c->h_pin + PIN_MOM);
     RC(species_sums(c, cl, S_eps != nullptr, false, h));
     const double PI = 3.14159265358979323846;
     for (int s = 0; s < c->S; ++s) {
@@ -1316,9 +1358,10 @@ int landau_moments(landau_ctx* c, double* n, double* P, double* K, double* S_eps
 
 int landau_moments_ext(landau_ctx* c, double* stress, double* m4) {
     if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     Cloud& cl = c->state;
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "moments_ext: no markers held");
-    double* h = (double*)c->h_pin + 64;
+    double* h = (double*)((char*)c->h_pin + PIN_MOM);
     RC(species_sums(c, cl, false, m4 != nullptr, h));
     for (int s = 0; s < c->S; ++s) {
         const double* r = h + s * MOM_OUT;
@@ -1348,6 +1391,7 @@ int landau_profile_read(landau_ctx* c, double* pair_ms, int64_t* pair_launches, 
 
 int landau_fp64_peak(landau_ctx* c, int reps, double* flops_out) {
     if (!c || !flops_out || reps < 1) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
     RC(ensure(c, c->V, 1024));
     const int blocks = c->sm_count * 4, threads = 256, iters = 4096;
     cudaEvent_t e0, e1;

@@ -24,8 +24,20 @@
 // arrays copy {x,y,z,w,gx,gy,gz}[npad] staged into shared memory by TMA bulk copies
 // (cp.async.bulk + mbarrier), double buffered across tasks.
 //
-// Output: every CTA adds into its own slice  vpart[cta][3][npad_max]  (zeroed before the launch),
-// already scaled by nu/m; the combine/update kernels sum the G slices in index order.
+// Output, O(N) memory and deterministic (no per-CTA slices, no floating-point atomics):
+//   * target side: a CTA leaves tile I once per run; it stores the tile's accumulators (scaled by nu/m) as one
+//     compact segment  tpart[I + cta][3][BT]  (plain stores; a tile's row of tasks is shared by <= a few
+//     consecutive CTAs, and I + cta is unique per (cta, tile) because both grow along the task order);
+//   * source side: the 3*BS sums of a task are added IN PLACE into  acc[3][npad_max]  (L2 resident).  The
+//     additions to one source unit are ordered by a per-unit ticket: the visits of unit j by the tiles
+//     I' < j/rho are ranked by (local time of the visit in its CTA's run, CTA index) -- a pure function of the
+//     static schedule that every CTA evaluates for itself -- and a CTA adds only when ticket[j] equals its rank.
+//     All CTAs of the persistent grid are co-resident (grid = SM count, 1 CTA/SM) and advance through their
+//     equal runs at the same pace, so a visit's predecessors have (almost always) already passed; the order is
+//     fixed, hence the sum is bit-reproducible.  The wait is bounded: on expiry the kernel raises the layout's
+//     error flag instead of hanging.
+//   sym_reset_kernel zeroes acc and the tickets before the launch; sym_combine_kernel adds, per slot, acc and the
+//   tile's segments in CTA order into ONE field slice [3][npad_max] for the update / combine kernels.
 #pragma once
 #include "common.cuh"
 
@@ -75,6 +87,20 @@ __device__ __host__ inline long long sym_tasks_before(int I, int TU, int rho) {
     return (long long)I * TU - (long long)rho * I * (I - 1) / 2;
 }
 
+// CTA that owns task k when task t belongs to CTA b iff ntasks*b/G <= t < ntasks*(b+1)/G
+__device__ __host__ inline int sym_task_owner(long long k, int G, long long ntasks) {
+    return (int)(((k + 1) * G - 1) / ntasks);
+}
+
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 // FP32 flavour of rsqrt_or_zero (FP32 field variant of BASELINE config 4): MUFU.RSQ + one Newton step;
 // a separation that underflows in FP32 contributes 0 (reading S5 in FP32).
 __device__ __forceinline__ float rsqrt_or_zero(float x) {
@@ -121,7 +147,7 @@ template <int W, int RT, int RS, typename F = double>
 __global__ void __launch_bounds__(W * 32, 1)
 pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 const StepCtrl* __restrict__ ctrl, int npad_max, const F* __restrict__ soa,
-                double* __restrict__ vpart) {
+                double* acc, double* __restrict__ tpart, int* ticket, int* errflag) {
     using C = SymCfg<W, RT, RS, F>;
     using F2 = typename SymVec2<F>::type;
     if (ctrl && ctrl->done) return;
@@ -131,6 +157,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_acc + 3 * C::BS); // [2]
     __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
     __shared__ double s_im[LD_MAX_SPECIES];
+    __shared__ int s_rank[2];
 
     const int S = T->S;
     const int npad = L->npad;
@@ -144,6 +171,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     for (int i = tid; i < S * S; i += C::THREADS) s_nu[i] = T->nu[i];
     if (tid < S) s_im[tid] = T->inv_mass[tid];
     if (tid == 0) {
+        s_rank[0] = 0; s_rank[1] = 0;
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -167,7 +195,18 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         }
     };
 
-    double* myslice = vpart + (size_t)blockIdx.x * 3 * (size_t)npad_max;
+    const int G = (int)gridDim.x;
+    auto store_targets = [&](int tile, int sp, const F (&ax)[RT], const F (&ay)[RT], const F (&az)[RT]) {
+        const double im = s_im[sp];
+        double* seg = tpart + (size_t)(tile + (int)blockIdx.x) * 3 * C::BT;
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const int q = wv * 32 * RT + r * 32 + lane;
+            seg[q] = (double)ax[r] * im;
+            seg[C::BT + q] = (double)ay[r] * im;
+            seg[2 * C::BT + q] = (double)az[r] * im;
+        }
+    };
     F px[RT], py[RT], pz[RT], gx[RT], gy[RT], gz[RT], w0[RT], wp[RT], ax[RT], ay[RT], az[RT];
     int curI = -1, sI = 0;
     uint32_t phase_bits = 0;   // bit s = parity to wait for on stage s
@@ -176,16 +215,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 
     for (long long t = t0; t < t1; ++t) {
         if (I != curI) {
-            if (curI >= 0) {
-                const double im = s_im[sI];
-#pragma unroll
-                for (int r = 0; r < RT; ++r) {
-                    const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
-                    myslice[p] += (double)ax[r] * im;
-                    myslice[(size_t)npad_max + p] += (double)ay[r] * im;
-                    myslice[2 * (size_t)npad_max + p] += (double)az[r] * im;
-                }
-            }
+            if (curI >= 0) store_targets(curI, sI, ax, ay, az);
             curI = I;
             sI = species_of_slot(L, S, I * C::BT);
 #pragma unroll
@@ -209,6 +239,22 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 #pragma unroll
         for (int r = 0; r < RT; ++r) wp[r] = w0[r] * nu;
         for (int i = tid; i < 3 * C::BS; i += C::THREADS) s_acc[i] = F(0);
+        // rank of this visit of source unit j among the visits by all tiles I' < j/rho (header comment)
+        const int par = (int)((t - t0) & 1);
+        if (tid == 0) s_rank[par ^ 1] = 0;
+        if (!diag) {
+            const long long mytau = t - t0;
+            int cnt = 0;
+            for (int Ip = tid; Ip < j / rho; Ip += C::THREADS) {
+                if (Ip == I) continue;
+                const long long kp = sym_tasks_before(Ip, TU, rho) + (j - rho * Ip);
+                const int bp = sym_task_owner(kp, G, ntasks);
+                const long long taup = kp - ntasks * bp / G;
+                cnt += (taup < mytau || (taup == mytau && bp < (int)blockIdx.x)) ? 1 : 0;
+            }
+            cnt = __reduce_add_sync(0xffffffffu, cnt);
+            if (lane == 0 && cnt) atomicAdd(&s_rank[par], cnt);
+        }
         mbar_wait(&s_bar[stage], (phase_bits >> stage) & 1u);
         phase_bits ^= 1u << stage;
         __syncthreads();
@@ -269,31 +315,65 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         }
         if (!diag) {
             const double sc = -s_im[sJ];
+            const int want = s_rank[par];
+            if (tid == 0) {
+                unsigned spins = 0;
+                while (ld_acquire_gpu(ticket + j) != want) {
+                    __nanosleep(40);
+                    if (++spins > (1u << 26)) { atomicExch(errflag, -3); break; }   // a schedule bug must not hang the GPU
+                }
+            }
+            __syncthreads();
             for (int i = tid; i < 3 * C::BS; i += C::THREADS) {
                 const int d = i / C::BS, e = i - d * C::BS;
-                myslice[(size_t)d * npad_max + (size_t)j * C::BS + e] += sc * (double)s_acc[i];
+                double* o = acc + (size_t)d * npad_max + (size_t)j * C::BS + e;
+                __stcg(o, __ldcg(o) + sc * (double)s_acc[i]);
             }
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) st_release_gpu(ticket + j, want + 1);
         }
-        __syncthreads();
         I = In; j = jn; stage ^= 1;
     }
-    {
-        const double im = s_im[sI];
-#pragma unroll
-        for (int r = 0; r < RT; ++r) {
-            const int p = curI * C::BT + wv * 32 * RT + r * 32 + lane;
-            myslice[p] += (double)ax[r] * im;
-            myslice[(size_t)npad_max + p] += (double)ay[r] * im;
-            myslice[2 * (size_t)npad_max + p] += (double)az[r] * im;
-        }
-    }
+    store_targets(curI, sI, ax, ay, az);
 }
 
-// Zero the per-CTA slices (skipped, like every kernel of an iteration, once the step is done).
-__global__ void zero_slices_kernel(const StepCtrl* __restrict__ ctrl, double2* __restrict__ p, size_t n2) {
+// Before a launch of pair_sym_kernel: zero the in-place source-side accumulator and the per-unit tickets
+// (skipped, like every kernel of an iteration, once the step is done).
+__global__ void sym_reset_kernel(const StepCtrl* __restrict__ ctrl, double* __restrict__ acc, size_t n,
+                                 int* __restrict__ ticket, int nticket) {
     if (ctrl && ctrl->done) return;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += stride) p[i] = make_double2(0.0, 0.0);
+    const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (size_t i = i0; i < n; i += stride) acc[i] = 0.0;
+    for (size_t i = i0; i < (size_t)nticket; i += stride) ticket[i] = 0;
+}
+
+// After pair_sym_kernel: field slice out[3][npad_max] = in-place source-side sums + the target-side segments of
+// the slot's tile, added in CTA order (the CTAs whose runs of tasks meet the tile's row).  G = grid of the pair kernel.
+__global__ void sym_combine_kernel(const DevLayout* __restrict__ L, const StepCtrl* __restrict__ ctrl, int npad_max,
+                                   int G, int BT, int BS, const double* __restrict__ acc,
+                                   const double* __restrict__ tpart, double* __restrict__ out) {
+    if (ctrl && ctrl->done) return;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npad_max) return;
+    const size_t np = (size_t)npad_max;
+    const int npad = L->npad;
+    double a = 0.0, b = 0.0, c = 0.0;
+    if (p < npad) {
+        const int rho = BT / BS, TI = npad / BT, TU = npad / BS;
+        const long long ntasks = sym_tasks_before(TI, TU, rho);
+        const int I = p / BT, q = p - I * BT;
+        const long long k0 = sym_tasks_before(I, TU, rho), k1 = sym_tasks_before(I + 1, TU, rho);
+        const int bf = sym_task_owner(k0, G, ntasks), bl = sym_task_owner(k1 - 1, G, ntasks);
+        a = acc[p]; b = acc[np + p]; c = acc[2 * np + p];
+        for (int cta = bf; cta <= bl; ++cta) {
+            if (ntasks * cta / G >= ntasks * (cta + 1) / G) continue;      // a CTA without tasks wrote nothing
+            const double* seg = tpart + (size_t)(I + cta) * 3 * BT + q;
+            a += seg[0]; b += seg[BT]; c += seg[2 * BT];
+        }
+    }
+    out[p] = a; out[np + p] = b; out[2 * np + p] = c;
 }
 
 // {x,y,z,w,G} (packed SoA) -> structure-of-arrays source copy {x,y,z,w,gx,gy,gz}[npad_max], g = G/m.
