@@ -18,8 +18,9 @@
 // Tasks are numbered I-major and dealt to the G persistent CTAs in contiguous, equal runs (static
 // schedule => deterministic summation order).  Inside a task warp w works through the W sub-tiles
 // of 32*RS sources in the order (w + phase) % W (a Latin square: in any phase each sub-tile belongs
-// to exactly one warp), and inside a sub-tile lane l visits source group (l + k) % 32 at step k
-// while the source-side accumulators travel with their sources by one warp shuffle per step.  Each
+// to exactly one warp), and inside a sub-tile lane l visits source group (l + k) % 32 at step k;
+// the source-side accumulators sit in shared memory next to their sources and are read, updated and
+// written back by whichever lane holds the group (conflict free; no shuffles, no atomics).  Each
 // lane keeps RT targets (and their accumulators) in registers.  Sources come from a structure-of-
 // arrays copy {x,y,z,w,gx,gy,gz}[npad] staged into shared memory by TMA bulk copies
 // (cp.async.bulk + mbarrier), double buffered across tasks.
@@ -262,13 +263,10 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         const F* sx = s_src + (size_t)stage * C::NCOMP * C::BS;
         for (int ph = 0; ph < W; ++ph) {
             const int base = ((wv + ph) % W) * C::SUB;
-            F bx[RS], by[RS], bz[RS];
-#pragma unroll
-            for (int s = 0; s < RS; ++s) bx[s] = by[s] = bz[s] = F(0);
 #pragma unroll 1
             for (int k = 0; k < 32; ++k) {
                 const int g = base + ((lane + k) & 31) * RS;
-                F qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS];
+                F qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS], bx[RS], by[RS], bz[RS];
                 if (RS % 2 == 0) {
 #pragma unroll
                     for (int s = 0; s < RS; s += 2) {
@@ -294,21 +292,36 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 if (diag) {
                     sym_step<false, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                 } else {
-                    sym_step<true, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    // the source-side sums live in shared memory next to their sources: in this phase the sub-tile is
+                    // this warp's alone and at step k every lane holds another group, so the read-modify-write is
+                    // conflict free and ordered by the warp's program order (no shuffles, no atomics)
+                    if (RS % 2 == 0) {
 #pragma unroll
-                    for (int s = 0; s < RS; ++s) {
-                        bx[s] = __shfl_sync(0xffffffffu, bx[s], (lane + 1) & 31);
-                        by[s] = __shfl_sync(0xffffffffu, by[s], (lane + 1) & 31);
-                        bz[s] = __shfl_sync(0xffffffffu, bz[s], (lane + 1) & 31);
+                        for (int s = 0; s < RS; s += 2) {
+                            const F2 b0 = *reinterpret_cast<const F2*>(s_acc + g + s);
+                            const F2 b1 = *reinterpret_cast<const F2*>(s_acc + C::BS + g + s);
+                            const F2 b2 = *reinterpret_cast<const F2*>(s_acc + 2 * C::BS + g + s);
+                            bx[s] = b0.x; bx[s + 1] = b0.y; by[s] = b1.x; by[s + 1] = b1.y; bz[s] = b2.x; bz[s + 1] = b2.y;
+                        }
+                    } else {
+#pragma unroll
+                        for (int s = 0; s < RS; ++s) { bx[s] = s_acc[g + s]; by[s] = s_acc[C::BS + g + s]; bz[s] = s_acc[2 * C::BS + g + s]; }
                     }
-                }
-            }
-            if (!diag) {
-                // after 32 rotations lane l again holds source group l of this sub-tile
+                    sym_step<true, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    if (RS % 2 == 0) {
 #pragma unroll
-                for (int s = 0; s < RS; ++s) {
-                    const int e = base + lane * RS + s;
-                    s_acc[e] += bx[s]; s_acc[C::BS + e] += by[s]; s_acc[2 * C::BS + e] += bz[s];
+                        for (int s = 0; s < RS; s += 2) {
+                            F2 b0, b1, b2;
+                            b0.x = bx[s]; b0.y = bx[s + 1]; b1.x = by[s]; b1.y = by[s + 1]; b2.x = bz[s]; b2.y = bz[s + 1];
+                            *reinterpret_cast<F2*>(s_acc + g + s) = b0;
+                            *reinterpret_cast<F2*>(s_acc + C::BS + g + s) = b1;
+                            *reinterpret_cast<F2*>(s_acc + 2 * C::BS + g + s) = b2;
+                        }
+                    } else {
+#pragma unroll
+                        for (int s = 0; s < RS; ++s) { s_acc[g + s] = bx[s]; s_acc[C::BS + g + s] = by[s]; s_acc[2 * C::BS + g + s] = bz[s]; }
+                    }
+                    __syncwarp();
                 }
             }
             __syncthreads();
