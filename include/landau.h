@@ -133,9 +133,9 @@ int landau_set_dimension(landau_ctx* ctx, int dim);
  * conditional WHILE node kept alive from the device (cudaGraphSetConditional in the update kernel) -- no launch
  * per iteration, no pre-enqueued iterations that exit at once.  mode 0: always the plain launch sequence
  * (max_iter iterations enqueued up front, early exit on the device flag).  mode 2: graph at any size.  Same
- * kernels and bit-identical results either way; the graph is captured after the first ordinary step, is reused
- * while shapes and parameters stay the same, and is not used while landau_profile_enable is on or with the
- * Anderson solver. */
+ * kernels and bit-identical results either way (for every solver of landau_set_solver); the graph is captured
+ * after the first ordinary step, is reused while shapes and parameters stay the same, and is not used while
+ * landau_profile_enable is on. */
 int landau_set_step_graph(landau_ctx* ctx, int mode);
 
 /* SURVEY.md NEXT-4 (robustness): what landau_step / landau_run do with a step whose fixed point does not converge
@@ -148,10 +148,14 @@ int landau_set_step_graph(landau_ctx* ctx, int mode);
 int landau_set_substep(landau_ctx* ctx, int max_halvings);
 
 /* how landau_step / landau_run solve Eq. (24).  solver 0 (default) = the paper's plain
- * Jacobi fixed-point iteration; solver 1 = the same fixed point with Anderson acceleration of the given
- * depth (1..10, 3 to 5 is a good default; `depth` is ignored for solver 0).  The equation, the residual, the
- * stopping rule, status codes and conservation properties are unchanged; only the iterates between v^n and
- * the converged v^{n+1} differ.  Still device driven (no host synchronisation inside a step). */
+ * Jacobi fixed-point iteration (`depth` ignored); solver 1 = the same fixed point with Anderson acceleration of the
+ * given depth (1..10, 3 to 5 is a good default); solver 2 = Jacobian-free Newton-Krylov: Newton's method on
+ * F(x) = x - v^n - dt V[(x + v^n)/2 ; G^n] with GMRES(depth) (restart length 1..30, 20 is a good default) in the
+ * energy inner product and Jacobian-vector products by one extra pass 2 each -- for the steps the fixed-point
+ * iteration cannot converge.  The equation, the residual (evaluated at a true evaluation of
+ * g(x) = v^n + dt V), the stopping rule, status codes and conservation properties are unchanged; only the iterates
+ * between v^n and the converged v^{n+1} differ.  `iterations` counts pass-2 evaluations for every solver.  All
+ * three are device driven (no host synchronisation inside a step). */
 int landau_set_solver(landau_ctx* ctx, int solver, int depth);
 
 /* n_steps consecutive steps with one host synchronisation at the end; info (optional, HOST,

@@ -248,7 +248,8 @@ class Landau:
         return rc, int(info.iterations), float(info.residual), bool(info.converged)
 
     def set_solver(self, solver: int = 0, depth: int = 3):
-        """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..10 (NEXT-4)."""
+        """0 = the paper's Jacobi fixed point (default); 1 = Anderson acceleration of depth 1..10; 2 = Jacobian-free
+        Newton-Krylov with GMRES restart length `depth` 1..30 (NEXT-4)."""
         self._check(self._lib.landau_set_solver(self._h, int(solver), int(depth)), "landau_set_solver")
 
     def cells_run(self, cell_offset, v, w, sid, n_steps, dt, tol=1e-12, max_iter=50, out=None, strict=True):

@@ -24,6 +24,7 @@
 #include "step.cuh"
 #include "step_dg.cuh"
 #include "step_anderson.cuh"
+#include "step_newton.cuh"
 #include "cells.cuh"
 
 using namespace landau;
@@ -86,8 +87,10 @@ struct landau_ctx {
     size_t attr_cells[LD_MAX_NQ + 1] = {};
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
-    int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson (NEXT-4)
+    int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson, 2 Newton-Krylov (NEXT-4)
+    int nk_m = 20;                        // GMRES restart length of the Newton-Krylov solver
     AndersonCtrl* d_aa = nullptr;
+    NewtonCtrl* d_nk = nullptr;
     Buf aa_hist;
     Buf cells_off, cells_rec, soa32;
     // CUDA-graph form of a whole step for launch-bound (small) clouds, landau_set_step_graph
@@ -97,7 +100,7 @@ struct landau_ctx {
     struct StepGraph {
         cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
         unsigned long long gen = 0; int64_t N = 0; int npm = 0, max_iter = 0, fixed_nodes = 0, body_nodes = 0;
-        double dt = 0.0, tol = 0.0; int ek = 0, pk = 0; bool failed = false;
+        double dt = 0.0, tol = 0.0; int ek = 0, pk = 0, solver = 0, depth = 0; bool failed = false;
     } sg;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
@@ -637,6 +640,112 @@ __global__ void fp64_peak_kernel(double* out, int iters, double a, double b) {
 
 }  // namespace
 
+
+namespace {
+// ---- a4: the kernels of one implicit step, shared by the plain launch sequence and the CUDA-graph capture ------
+struct StepBufs {
+    int npm, nub;
+    double *xk, *yk, *zk;          // current iterate x (Jacobi: v^(k))
+    double* hist;                  // solver history (Anderson: dF, dG, fprev, gcur; Newton-Krylov: Q, gcur)
+    double* commit;                // [3][npm] state committed at the end of the step
+};
+
+StepBufs step_bufs(landau_ctx* c, const Cloud& cl) {
+    StepBufs b;
+    b.npm = cl.npad_max; b.nub = ceil_div(b.npm, UPD_THREADS);
+    b.xk = (double*)c->vk.p; b.yk = b.xk + b.npm; b.zk = b.yk + b.npm;
+    b.hist = (double*)c->aa_hist.p;
+    b.commit = b.xk;
+    if (c->solver == 1) b.commit = b.hist + (2 * (size_t)c->aa_depth + 1) * 3 * (size_t)b.npm;
+    if (c->solver == 2) b.commit = b.hist + ((size_t)c->nk_m + 1) * 3 * (size_t)b.npm;
+    return b;
+}
+
+size_t step_hist_doubles(const landau_ctx* c, int npm) {
+    if (c->solver == 1) return (2 * (size_t)c->aa_depth + 2) * 3 * (size_t)npm;
+    if (c->solver == 2) return ((size_t)c->nk_m + 4) * 3 * (size_t)npm;
+    return 0;
+}
+
+int step_blockpart_doubles(const landau_ctx* c, int nub) {
+    return std::max(std::max(AA_NRED, NK_NRED) * nub, 4096);
+}
+
+int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b) {
+    cudaStream_t st = c->stream;
+    step_begin_kernel<<<ceil_div(b.npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, b.npm, cl.x(), cl.y(), cl.z(),
+                                                             cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), b.xk, b.yk, b.zk,
+                                                             cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
+    c->launches += 1;
+    if (c->solver == 1) {
+        anderson_begin_kernel<<<1, 32, 0, st>>>(c->d_aa, c->aa_depth);
+        c->launches += 1;
+    }
+    if (c->solver == 2) {
+        nk_begin_kernel<<<1, 32, 0, st>>>(c->d_nk, c->nk_m);
+        c->launches += 1;
+    }
+    return 0;
+}
+
+// One iteration = one pass 2 at the current sources + the solver's update kernels.  `first` skips work that
+// step_begin has already done.  cond != 0: the kernel that decides convergence also drives the WHILE node.
+int enqueue_step_iteration(landau_ctx* c, Cloud& cl, const StepBufs& b, double dt, double tol, int max_iter, bool first,
+                           cudaGraphConditionalHandle cond) {
+    cudaStream_t st = c->stream;
+    const int npm = b.npm;
+    double* rec = cl.sym ? nullptr : cl.recs();
+    double* soa = cl.sym ? cl.soas() : nullptr;
+    int nparts = 0;
+    if (c->solver == 2 && !first) {
+        nk_sources_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_nk, npm, cl.x(), cl.y(), cl.z(),
+                                                               b.xk, b.yk, b.zk, b.hist, rec, soa);
+        c->launches += 1;
+    }
+    RC(pair(c, cl, c->d_ctrl, &nparts));
+    st = c->stream;
+    if (c->solver == 0) {
+        step_update_kernel<<<b.nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
+                                                           (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                           b.xk, b.yk, b.zk, rec, soa, (double*)c->blockpart.p, cond);
+        c->launches += 1;
+    } else if (c->solver == 1) {
+        // NEXT-4: Anderson-accelerated fixed point (step_anderson.cuh); commits g(x_k) of the last evaluation
+        double* dF = b.hist;
+        double* dG = dF + (size_t)c->aa_depth * 3 * npm;
+        double* fprev = dG + (size_t)c->aa_depth * 3 * npm;
+        double* gcur = fprev + 3 * (size_t)npm;
+        anderson_update_kernel<<<b.nub, UPD_THREADS, 0, st>>>(
+            c->d_tab, cl.L(), c->d_ctrl, c->d_aa, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p, cl.x(),
+            cl.y(), cl.z(), cl.w(), b.xk, b.yk, b.zk, dF, dG, fprev, gcur, (double*)c->blockpart.p, cond);
+        anderson_mix_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_aa, npm, cl.x(), cl.y(), cl.z(),
+                                                                 gcur, dG, b.xk, b.yk, b.zk, rec, soa);
+        c->launches += 2;
+    } else {
+        // NEXT-4: Jacobian-free Newton-Krylov (step_newton.cuh); commits g(x) of the last phase-0 evaluation
+        double* Q = b.hist;
+        double* gcur = Q + ((size_t)c->nk_m + 1) * 3 * (size_t)npm;
+        double* Vcur = gcur + 3 * (size_t)npm;
+        double* fvec = Vcur + 3 * (size_t)npm;
+        nk_post_kernel<<<b.nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, c->d_nk, npm, nparts, dt, tol,
+                                                       max_iter, (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
+                                                       cl.w(), b.xk, b.yk, b.zk, Q, gcur, Vcur, fvec,
+                                                       (double*)c->blockpart.p, cond);
+        nk_update_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_nk, npm, Q, fvec, b.xk, b.yk, b.zk);
+        c->launches += 2;
+    }
+    return 0;
+}
+
+void enqueue_step_commit(landau_ctx* c, Cloud& cl, const StepBufs& b) {
+    const size_t np = (size_t)b.npm;
+    step_commit_kernel<<<ceil_div(b.npm, 256), 256, 0, c->stream>>>(cl.L(), c->d_ctrl, b.npm, cl.x(), cl.y(), cl.z(),
+                                                                     b.commit, b.commit + np, b.commit + 2 * np,
+                                                                     (StepRecord*)c->records.p, c->d_cursor);
+    c->launches += 1;
+}
+}  // namespace
+
 // =============================================================================================
 namespace {
 // ---- a4 for launch-bound clouds: one step as a CUDA graph with a conditional WHILE node ----------------------
@@ -654,7 +763,8 @@ void destroy_step_graph(landau_ctx* c) {
 bool step_graph_matches(const landau_ctx* c, const Cloud& cl, double dt, double tol, int max_iter) {
     const auto& g = c->sg;
     return g.exec && g.gen == c->alloc_gen && g.N == cl.N && g.npm == cl.npad_max && g.dt == dt && g.tol == tol &&
-           g.max_iter == max_iter && g.ek == c->entropy_kernel && g.pk == c->pair_kernel;
+           g.max_iter == max_iter && g.ek == c->entropy_kernel && g.pk == c->pair_kernel && g.solver == c->solver &&
+           g.depth == (c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0);
 }
 
 int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_iter) {
@@ -664,10 +774,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
         c->sg.failed = true; cudaGetLastError(); return 0;
     }
     const int npm = cl.npad_max;
-    const int nub = ceil_div(npm, UPD_THREADS);
-    double* xk = (double*)c->vk.p;
-    double* yk = xk + npm;
-    double* zk = yk + npm;
+    const StepBufs sb = step_bufs(c, cl);
     // capture on a private stream (the context's stream may be the legacy default stream, which cannot be captured)
     cudaStream_t user_stream = c->stream;
     cudaStream_t st = c->cap_stream;
@@ -681,13 +788,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
     cudaGraph_t graph = nullptr;
     int fixed = 0, body_nodes = 0;
     if (ok) {
-        if (ok) {
-            step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
-                                                                   cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
-                                                                   cl.sym ? nullptr : cl.recs(),
-                                                                   cl.sym ? cl.soas() : nullptr);
-            c->launches += 1;
-        }
+        if (ok) ok = enqueue_step_begin(c, cl, sb) == 0;
         cudaStreamCaptureStatus status;
         cudaGraph_t g = nullptr;
         const cudaGraphNode_t* deps = nullptr;
@@ -714,15 +815,8 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
             if (ok) {
                 const int64_t l1 = c->launches;
                 c->stream = c->body_stream;
-                int nparts = 0;
-                ok = pair(c, cl, c->d_ctrl, &nparts) == 0;
-                if (ok) {
-                    step_update_kernel<<<nub, UPD_THREADS, 0, c->body_stream>>>(
-                        c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p, cl.x(),
-                        cl.y(), cl.z(), cl.w(), xk, yk, zk, cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr,
-                        (double*)c->blockpart.p, handle);
-                    c->launches += 1;
-                }
+                // the body always rebuilds its sources (first = false): it is replayed for every iteration
+                ok = enqueue_step_iteration(c, cl, sb, dt, tol, max_iter, false, handle) == 0;
                 c->stream = st;
                 body_nodes = (int)(c->launches - l1);
                 cudaGraph_t tmp = nullptr;
@@ -732,9 +826,9 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
         }
         SG_TRY("update dependencies", cudaStreamUpdateCaptureDependencies(st, &cond_node, 1, cudaStreamSetCaptureDependencies));
         if (ok) {
-            step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,
-                                                                    zk, (StepRecord*)c->records.p, c->d_cursor);
-            fixed += 1;
+            const int64_t l2 = c->launches;
+            enqueue_step_commit(c, cl, sb);
+            fixed += (int)(c->launches - l2);
         }
         ce = cudaStreamEndCapture(st, &graph);
         if ((ce != cudaSuccess || !graph) && ok) { ok = false; stage = "end capture"; }
@@ -758,6 +852,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
     auto& g = c->sg;
     g.graph = graph; g.exec = exec; g.gen = c->alloc_gen; g.N = cl.N; g.npm = npm; g.dt = dt; g.tol = tol;
     g.max_iter = max_iter; g.ek = c->entropy_kernel; g.pk = c->pair_kernel; g.fixed_nodes = fixed; g.body_nodes = body_nodes;
+    g.solver = c->solver; g.depth = c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0;
     return 0;
 }
 }  // namespace
@@ -853,6 +948,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_aa, sizeof(AndersonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_nk, sizeof(NewtonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMallocHost(&c->h_pin, PIN_BYTES) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMemcpy(c->d_tab, &t, sizeof(t), cudaMemcpyHostToDevice) != cudaSuccess) return bail(LANDAU_ECUDA);
@@ -870,6 +966,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_ctrl) cudaFree(c->d_ctrl);
     if (c->d_cursor) cudaFree(c->d_cursor);
     if (c->d_aa) cudaFree(c->d_aa);
+    if (c->d_nk) cudaFree(c->d_nk);
     destroy_step_graph(c);
     if (c->body_stream) cudaStreamDestroy(c->body_stream);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -1012,11 +1109,9 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
     RC(ensure(c, c->vk, sizeof(double) * 3 * (size_t)npm));
     RC(ensure(c, c->records, sizeof(StepRecord) * (size_t)n_steps));
     const int nub = ceil_div(npm, UPD_THREADS);
-    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(AA_NRED * nub, 4096)));
-    if (c->solver == 1) RC(ensure(c, c->aa_hist, sizeof(double) * (2 * (size_t)c->aa_depth + 2) * 3 * (size_t)npm));
-    double* xk = (double*)c->vk.p;
-    double* yk = xk + npm;
-    double* zk = yk + npm;
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)step_blockpart_doubles(c, nub)));
+    if (c->solver != 0) RC(ensure(c, c->aa_hist, sizeof(double) * step_hist_doubles(c, npm)));
+    const StepBufs sb = step_bufs(c, cl);
     cudaStream_t st = c->stream;
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
@@ -1024,67 +1119,25 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
         const int one = 1;
         CU(cudaMemcpyAsync(&c->d_ctrl->hold, &one, sizeof(int), cudaMemcpyHostToDevice, st));
     }
-    const bool graph_ok = !hold && c->graph_mode != 0 && !c->sg.failed && !c->prof_on && c->solver == 0 &&
+    const bool graph_ok = !hold && c->graph_mode != 0 && !c->sg.failed && !c->prof_on &&
                           (c->graph_mode == 2 || npm <= 65536);
     std::vector<char> via_graph(n_steps, 0);
     for (int n = 0; n < n_steps; ++n) {
         c->prof_step = n; c->prof_iter = 0;
+        if (!cl.G_valid) RC(entropy(c, cl));     // a preceding landau_moments(S_eps) already evaluated pass 1 here
+        cl.G_valid = false;                      // the step moves the markers
         if (graph_ok && step_graph_matches(c, cl, dt, tol, max_iter)) {
-            if (!cl.G_valid) RC(entropy(c, cl));
             CU(cudaGraphLaunch(c->sg.exec, st));
             c->launches += c->sg.fixed_nodes;
             via_graph[n] = 1;
-            cl.G_valid = false;
             continue;
         }
-        if (!cl.G_valid) RC(entropy(c, cl));     // a preceding landau_moments(S_eps) already evaluated pass 1 here
-        cl.G_valid = false;                      // the step moves the markers
-        step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
-                                                               cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
-                                                               cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
-        c->launches += 1;
-        if (c->solver == 1) {
-            // NEXT-4: Anderson-accelerated fixed point (step_anderson.cuh); commits g(x_k) of the last evaluation
-            double* dF = (double*)c->aa_hist.p;
-            double* dG = dF + (size_t)c->aa_depth * 3 * npm;
-            double* fprev = dG + (size_t)c->aa_depth * 3 * npm;
-            double* gcur = fprev + 3 * (size_t)npm;
-            AndersonCtrl h_aa;
-            memset(&h_aa, 0, sizeof(h_aa));
-            h_aa.m = c->aa_depth;
-            CU(cudaMemcpyAsync(c->d_aa, &h_aa, sizeof(int) * 2, cudaMemcpyHostToDevice, st));
-            for (int k = 0; k < max_iter; ++k) {
-                int nparts = 0;
-                c->prof_iter = k;
-                RC(pair(c, cl, c->d_ctrl, &nparts));
-                anderson_update_kernel<<<nub, UPD_THREADS, 0, st>>>(
-                    c->d_tab, cl.L(), c->d_ctrl, c->d_aa, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p,
-                    cl.x(), cl.y(), cl.z(), cl.w(), xk, yk, zk, dF, dG, fprev, gcur, (double*)c->blockpart.p);
-                anderson_mix_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_aa, npm, cl.x(), cl.y(),
-                                                                         cl.z(), gcur, dG, xk, yk, zk,
-                                                                         cl.sym ? nullptr : cl.recs(),
-                                                                         cl.sym ? cl.soas() : nullptr);
-                c->launches += 2;
-            }
-            step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), gcur,
-                                                                    gcur + npm, gcur + 2 * (size_t)npm,
-                                                                    (StepRecord*)c->records.p, c->d_cursor);
-            c->launches += 1;
-            continue;
-        }
+        RC(enqueue_step_begin(c, cl, sb));
         for (int k = 0; k < max_iter; ++k) {
-            int nparts = 0;
             c->prof_iter = k;
-            RC(pair(c, cl, c->d_ctrl, &nparts));
-            step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
-                                                             (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(),
-                                                             cl.w(), xk, yk, zk, cl.sym ? nullptr : cl.recs(),
-                                                             cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p, 0);
-            c->launches += 1;
+            RC(enqueue_step_iteration(c, cl, sb, dt, tol, max_iter, k == 0, 0));
         }
-        step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk,
-                                                                zk, (StepRecord*)c->records.p, c->d_cursor);
-        c->launches += 1;
+        enqueue_step_commit(c, cl, sb);
         // every buffer now has its size: capture the same sequence as a graph for the steps that follow
         if (graph_ok && !step_graph_matches(c, cl, dt, tol, max_iter)) RC(build_step_graph(c, cl, dt, tol, max_iter));
     }
@@ -1179,11 +1232,15 @@ int landau_set_step_graph(landau_ctx* c, int mode) {
 
 int landau_set_solver(landau_ctx* c, int solver, int depth) {
     if (!c) return LANDAU_EINVAL;
-    if (solver < 0 || solver > 1) return fail(c, LANDAU_EINVAL, "set_solver: solver must be 0 (Jacobi) or 1 (Anderson)");
+    if (solver < 0 || solver > 2)
+        return fail(c, LANDAU_EINVAL, "set_solver: solver must be 0 (Jacobi), 1 (Anderson) or 2 (Newton-Krylov)");
     if (solver == 1 && (depth < 1 || depth > AA_MAXM))
         return fail(c, LANDAU_EINVAL, "set_solver: Anderson depth must be 1..%d", AA_MAXM);
+    if (solver == 2 && (depth < 1 || depth > NK_MAXM))
+        return fail(c, LANDAU_EINVAL, "set_solver: Newton-Krylov restart length must be 1..%d", NK_MAXM);
     c->solver = solver;
     if (solver == 1) c->aa_depth = depth;
+    if (solver == 2) c->nk_m = depth;
     return 0;
 }
 

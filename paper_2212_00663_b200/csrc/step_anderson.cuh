@@ -64,6 +64,11 @@ __device__ inline bool aa_solve(int nc, const double (*G)[AA_MAXM], const double
     return true;
 }
 
+// Start of a step: empty history (a kernel, so that the reset is part of a captured step graph).
+__global__ void anderson_begin_kernel(AndersonCtrl* __restrict__ aa, int m) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) { aa->m = m; aa->_r = 0; }
+}
+
 // g_k = v^n + dt V(u_k), f_k = g_k - x_k; new difference columns; residual; Gram update and solve.
 // hist layout: dF[slot][3][npad_max], dG[slot][3][npad_max], fprev[3][npad_max], gcur[3][npad_max].
 __global__ void __launch_bounds__(UPD_THREADS)
@@ -73,7 +78,7 @@ anderson_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
                        const double* __restrict__ yn, const double* __restrict__ zn, const double* __restrict__ w,
                        const double* __restrict__ xk, const double* __restrict__ yk, const double* __restrict__ zk,
                        double* __restrict__ dF, double* __restrict__ dG, double* __restrict__ fprev,
-                       double* __restrict__ gcur, double* __restrict__ blockpart) {
+                       double* __restrict__ gcur, double* __restrict__ blockpart, cudaGraphConditionalHandle cond) {
     if (ctrl->done) return;
     __shared__ double s_red[UPD_THREADS / 32][AA_NRED];
     __shared__ int s_last;
@@ -181,6 +186,8 @@ anderson_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
             }
         }
         for (int j = 0; j < AA_MAXM; ++j) aa->gamma[j] = gam[j];
+        // CUDA-graph mode: keep the WHILE node that holds this iteration alive until the step is done
+        if (cond) cudaGraphSetConditional(cond, ctrl->done ? 0u : 1u);
     }
 }
 

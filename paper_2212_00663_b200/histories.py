@@ -35,8 +35,12 @@ def _kurtosis(mass, n, P, stress, m4):
 
 
 def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1, verbose: bool = False,
-                solver: int = 0, depth: int = 3, substep: int = 0):
+                solver: int = 0, depth: int = 3, substep: int = 0, n_q=None, max_iter=None):
     wl = W.make(config, n_per_species=n_per_species)
+    if n_q is not None:
+        wl.n_q = int(n_q)
+    if max_iter is not None:
+        wl.max_iter = int(max_iter)
     n_steps = int(steps if steps is not None else wl.n_steps)
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
     if solver:
@@ -74,8 +78,10 @@ def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1,
     wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
     summary = dict(config=config, workload=wl.name, n_markers=wl.n_markers, n_species=S, steps=n_steps, dt=wl.dt,
                    n_q=wl.n_q, eps=wl.eps.tolist(), kernels=g.last_kernels(),
-                   solver="jacobi" if not solver else f"anderson depth {depth}", substep_levels=substep, wall_s=wall,
+                   solver={0: "jacobi", 1: f"anderson depth {depth}", 2: f"newton-krylov restart {depth}"}[solver],
+                   substep_levels=substep, wall_s=wall,
                    steps_per_s=n_steps / wall, iterations_mean=float(H["iterations"][1:].mean()),
+                   pass2_evaluations_total=int(H["iterations"][1:].sum()), max_iter=wl.max_iter,
                    iterations_max=int(H["iterations"].max()), steps_not_converged=not_conv,
                    energy_drift_rel_max=float(np.abs(K - K[0]).max() / K[0]),
                    energy_drift_rel_per_step_max=float(np.abs(np.diff(K)).max() / K[0]),
@@ -126,14 +132,18 @@ def main():
     ap.add_argument("--n-per-species", type=int, default=None)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--out", default="gpurun_out")
-    ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi")
+    ap.add_argument("--solver", choices=["jacobi", "anderson", "newton"], default="jacobi")
     ap.add_argument("--anderson-depth", type=int, default=3)
+    ap.add_argument("--newton-restart", type=int, default=20)
+    ap.add_argument("--n-q", type=int, default=None, help="Gauss-Hermite knots per axis (default: the workload's, 4)")
+    ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
     ap.add_argument("--tag", default="", help="suffix of the output file names")
     args = ap.parse_args()
-    wl, H, summary = run_history(args.config, args.n_per_species, args.steps, verbose=True,
-                                 solver=1 if args.solver == "anderson" else 0, depth=args.anderson_depth,
-                                 substep=args.substep)
+    solver = {"jacobi": 0, "anderson": 1, "newton": 2}[args.solver]
+    wl, H, summary = run_history(args.config, args.n_per_species, args.steps, verbose=True, solver=solver,
+                                 depth=args.newton_restart if solver == 2 else args.anderson_depth,
+                                 substep=args.substep, n_q=args.n_q, max_iter=args.max_iter)
     write(Path(args.out), f"{args.config}{args.tag}", H, summary)
     print(json.dumps(summary))
 

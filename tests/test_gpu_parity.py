@@ -502,6 +502,88 @@ def test_anderson_momentum_conserved_when_not_converged(B):
     g.set_solver(0)
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: Newton-Krylov solver
+@pytest.mark.parametrize("cfg,n,dt", [(0, 256, 0.01), (4, 384, 1e-3), (1, 1024, 0.02), (2, 700, 0.01)])
+@pytest.mark.parametrize("restart", [6, 20])
+def test_newton_krylov_solver_reaches_the_same_step(B, oracle_mod, cfg, n, dt, restart):
+    """landau_set_solver(2, m): Jacobian-free Newton-GMRES(m) on the same Eq. (24).  The converged step must equal
+    the oracle's Jacobi step (unique fixed point, reading N4) to ~tol and conserve momentum and energy to 1e-12."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_solver(2, restart)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(dt, 1e-12, 100)
+    rco, ito, reso, convo = o.step(dt, 1e-12, 100)
+    assert rc == 0 and conv and res <= 1e-12 and rco == 0 and convo, (rc, it, res, ito, reso)
+    v1, ref = g.get_markers().cpu().numpy(), o.get_markers()
+    assert_field_close(v1, ref, wl.species_id, wl.n_species, tol=1e-11, what="Newton-Krylov state")
+    assert_field_close(v1 - wl.v, ref - wl.v, wl.species_id, wl.n_species, tol=1e-8, what="Newton-Krylov displacement")
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= TOL_DRIFT * m0["K"].sum()
+
+
+def test_newton_krylov_converges_where_jacobi_diverges(B, oracle_mod):
+    """A step far beyond the contraction limit of the Jacobi map (dt = 0.3 on config 0: the oracle's and the CUDA
+    path's Jacobi iterations both end at max_iter with a growing residual, the failure of PAPER.md:311-313) is
+    solved by Newton-Krylov; the result satisfies Eq. (24) when its field is re-evaluated by the ORACLE at the
+    returned midpoint, and conserves momentum and energy."""
+    wl = W.make(0, n_per_species=256, shuffled=True)
+    dt = 0.3
+    g, o = make_pair(B, oracle_mod, wl)
+    gj = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gj.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    rcj, itj, resj, convj = gj.step(dt, 1e-12, 60)
+    rco, ito, reso, convo = o.step(dt, 1e-12, 60)
+    assert (rcj, convj) == (1, False) and (rco, convo) == (1, False) and resj > 1e-6 and reso > 1e-6
+    g.set_solver(2, 30)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(dt, 1e-12, 400)
+    assert rc == 0 and conv and res <= 1e-12, (rc, it, res)
+    v1 = g.get_markers().cpu().numpy()
+    G = o.entropy_grad(wl.v, wl.w, wl.species_id)
+    V = o.pair_field(0.5 * (wl.v + v1), wl.w, wl.species_id, G)
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    defect = v1 - wl.v - dt * V
+    assert np.sqrt((wm * defect ** 2).sum() / (wm * v1 ** 2).sum()) <= 2e-12
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= 10 * TOL_DRIFT * m0["K"].sum()
+    with pytest.raises(B.LandauError):
+        g.set_solver(2, 31)
+    # not converged within max_iter: status 1, momentum still conserved (every g(x) has the momentum of v^n)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = g.step(dt, 1e-14, 7)
+    assert rc == 1 and not conv and it == 7
+    m2 = g.moments(with_entropy=False)
+    assert np.abs(m2["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+
+
+@pytest.mark.parametrize("solver,depth", [(1, 3), (2, 12)])
+@pytest.mark.parametrize("cfg,n", [(0, 256), (1, 2000)])
+def test_graph_step_with_accelerated_solvers_is_bit_identical(B, solver, depth, cfg, n):
+    """The CUDA-graph form of the step (conditional WHILE node) also carries the Anderson and Newton-Krylov
+    iterations: same kernels as the plain launch sequence, so states and iteration records are bit-identical."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    ga = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gb = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    for g, mode in ((ga, 2), (gb, 0)):
+        g.set_solver(solver, depth)
+        g.set_step_graph(mode)
+        g.set_markers(wl.v, wl.w, wl.species_id)
+    ra = [ga.step(wl.dt, wl.tol, 80) for _ in range(4)]
+    rb = [gb.step(wl.dt, wl.tol, 80) for _ in range(4)]
+    assert ra == rb and all(r[3] for r in ra)
+    assert "step=graph" in ga.last_kernels() and "step=launch" in gb.last_kernels()
+    assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+
+
 # ------------------------------------------------------------------------------------ NEXT-2: the paper's 2-V setting
 def test_two_v_mode_keeps_vz_zero_and_matches_oracle(B, oracle_mod):
     """landau_set_dimension(2) on the paper's test 3.3 initial data (grid-initialised anisotropic Maxwellians,
