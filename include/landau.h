@@ -128,6 +128,17 @@ int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_ste
  * would seed the physical relaxation into v_z).  x/y results equal the 2-V Eqs. (22)-(24) (reading D1). */
 int landau_set_dimension(landau_ctx* ctx, int dim);
 
+/* SURVEY.md NEXT-4 (second half): Gaussian cutoff of pass 1.  on = 1 (default): a tile of 64 source markers is not
+ * visited when the distance D (in units of sqrt(2 eps_s)) between its bounding box and the box of a block of 128
+ * targets satisfies  D^2 - 2 D |k|_max >= 60 ln 2 + ln(w_max/w_min) + ln N_s  (|k|_max = sqrt(3) times the largest
+ * Gauss-Hermite knot): everything skipped changes no node sum of Eq. (22) by more than 2^-60 relative (derivation in
+ * csrc/entropy.cuh), so results agree with the all-pairs evaluation to round-off.  It pays when eps_s is small against
+ * the extent of the cloud -- the paper's own rule eps_s = 1.2 (L_s/N)^1.98 -- and costs one
+ * box test per tile pair otherwise.  on = 0: all pairs.  landau_cutoff_stats returns the number of (target block,
+ * source tile) pairs considered / skipped by the LAST pass 1 (HOST outputs; synchronises). */
+int landau_set_cutoff(landau_ctx* ctx, int on);
+int landau_cutoff_stats(landau_ctx* ctx, int64_t* tiles_considered, int64_t* tiles_skipped);
+
 /* How landau_step / landau_run issue a step whose cost is launch latency (small clouds).  mode 1 (default,
  * automatic): clouds of <= 65536 padded slots replay the whole step as ONE CUDA graph whose fixed-point body is a
  * conditional WHILE node kept alive from the device (cudaGraphSetConditional in the update kernel) -- no launch

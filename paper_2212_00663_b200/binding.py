@@ -24,7 +24,7 @@ EINVAL, ENOMEM, ECUDA, ENONFINITE, ERANGE = -1, -2, -3, -4, -5
 SYMBOLS = [
     "landau_default_opts", "landau_create", "landau_destroy", "landau_eval_field",
     "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
-    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_set_step_graph", "landau_set_substep", "landau_cells_run",
+    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_set_step_graph", "landau_set_substep", "landau_cells_run", "landau_set_cutoff", "landau_cutoff_stats",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_last_error",
@@ -88,6 +88,8 @@ def load(build_if_missing: bool = True):
     lib.landau_set_dimension.argtypes = [vp, C.c_int]
     lib.landau_set_step_graph.argtypes = [vp, C.c_int]
     lib.landau_set_substep.argtypes = [vp, C.c_int]
+    lib.landau_set_cutoff.argtypes = [vp, C.c_int]
+    lib.landau_cutoff_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.landau_cells_run.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int,
                                      C.POINTER(CellInfo)]
     lib.landau_step_dg.argtypes = [vp, C.c_double, C.c_double, C.c_int, C.POINTER(StepInfo)]
@@ -279,6 +281,16 @@ class Landau:
     def set_substep(self, max_halvings: int = 0):
         """0 = commit unconverged steps (the paper's behaviour); k > 0 = redo them as two half steps, up to k levels."""
         self._check(self._lib.landau_set_substep(self._h, int(max_halvings)), "landau_set_substep")
+
+    def set_cutoff(self, on: bool = True):
+        """Gaussian cutoff of pass 1 (NEXT-4): skip source tiles that cannot change a node sum by 2^-60 relative."""
+        self._check(self._lib.landau_set_cutoff(self._h, int(bool(on))), "landau_set_cutoff")
+
+    def cutoff_stats(self):
+        """(source tiles considered, skipped) by the last pass 1."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.landau_cutoff_stats(self._h, C.byref(a), C.byref(b)), "landau_cutoff_stats")
+        return int(a.value), int(b.value)
 
     def set_dimension(self, dim: int = 3):
         """3 (default) or 2 = the paper's 2-V setting: v_z = 0 is preserved exactly (NEXT-2)."""

@@ -42,6 +42,8 @@ struct DevLayout {
     int _r1;
     double center[LD_MAX_SPECIES][3]; // bounding-box centre of species s (factorised pass 1)
     double halfwidth[LD_MAX_SPECIES]; // max_p |v_p - center|_inf / sqrt(2 eps_s), written once per pass 1
+    double cut_T[LD_MAX_SPECIES];     // Gaussian cutoff of pass 1 (entropy.cuh, tile_is_far): a source tile at box
+                                      // distance d (mollifier units) is skipped when d^2 - 2 d |k|_max >= cut_T[s]
 };
 
 // Device-side control block of the fixed-point loop.

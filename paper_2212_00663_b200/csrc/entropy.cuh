@@ -26,6 +26,66 @@ __device__ __forceinline__ bool fact_usable(const DevTable* __restrict__ T, cons
     return ok;
 }
 
+// ---- Gaussian cutoff of pass 1 (second half; the paper's own rule
+// eps_s = 1.2 (L_s/N)^1.98, shrinks the mollifier like the marker spacing squared, so that almost every
+// same-species pair contributes an exact or numerical zero to Eq. (22)).
+// Criterion.  The node sum A_p(k) = sum_q w_q exp(-|k + d_pq|^2) contains the target's own term w_p exp(-|k|^2).
+// For a source at distance |d| >= D > |k|_max = sqrt(3) k_max from the target,
+//     w_q exp(-|k + d|^2) / (w_p exp(-|k|^2)) <= (w_max/w_min) exp(-(D^2 - 2 D |k|_max)),
+// so if  D^2 - 2 D |k|_max >= cut_T = 60 ln 2 + ln(w_max/w_min) + ln N_s  then ALL sources beyond D together change
+// A_p(k) by less than 2^-60 relative, i.e. ln A_p(k) by < 1e-18: far below the round-off of the sum itself.  D is the
+// distance between the bounding boxes of a target tile and a source tile (64 consecutive slots, mollifier units);
+// whole source tiles are skipped.  Tiles are compact when the caller's marker order is (the paper's mesh order is),
+// and after the Morton bucketing of pack.cuh for any order.
+struct TileBox { double lo[3], hi[3]; };
+
+__device__ __forceinline__ bool tile_is_far(const TileBox& a, const TileBox& b, double cut_T, double kmax3) {
+    double d2 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const double g = fmax(fmax(a.lo[i] - b.hi[i], b.lo[i] - a.hi[i]), 0.0);
+        d2 = fma(g, g, d2);
+    }
+    const double d = sqrt(d2);
+    return !(a.lo[0] <= a.hi[0]) || !(b.lo[0] <= b.hi[0]) || (d > kmax3 && d2 - 2.0 * d * kmax3 >= cut_T);
+}
+
+// Bounding box (mollifier units) of the real markers of every tile of 64 slots; an empty tile gets lo > hi.
+__global__ void __launch_bounds__(64)
+entropy_tilebox_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
+                       const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+                       const double* __restrict__ w, TileBox* __restrict__ box) {
+    const int p = blockIdx.x * 64 + threadIdx.x;
+    const double BIG = 1.7976931348623157e308;
+    double lo[3] = {BIG, BIG, BIG}, hi[3] = {-BIG, -BIG, -BIG};
+    if (p < L->npad && w[p] > 0.0) {
+        const double inv = T->inv_sqrt_2eps[species_of_slot(L, T->S, p)];
+        lo[0] = hi[0] = x[p] * inv; lo[1] = hi[1] = y[p] * inv; lo[2] = hi[2] = z[p] * inv;
+    }
+    __shared__ double s[2][6];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+        if ((threadIdx.x & 31) == 0) { s[threadIdx.x >> 5][d] = lo[d]; s[threadIdx.x >> 5][3 + d] = hi[d]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        box[blockIdx.x].lo[threadIdx.x] = fmin(s[0][threadIdx.x], s[1][threadIdx.x]);
+        box[blockIdx.x].hi[threadIdx.x] = fmax(s[0][3 + threadIdx.x], s[1][3 + threadIdx.x]);
+    }
+}
+
+__device__ __forceinline__ TileBox box_union(const TileBox& a, const TileBox& b) {
+    TileBox r;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { r.lo[i] = fmin(a.lo[i], b.lo[i]); r.hi[i] = fmax(a.hi[i], b.hi[i]); }
+    return r;
+}
+
 constexpr int ENT_THREADS = 128;   // targets per block (one target per thread)
 constexpr int ENT_SRC_TILE = 64;   // sources staged in shared memory per tile
 
@@ -38,7 +98,8 @@ __global__ void __launch_bounds__(ENT_THREADS)
 entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
                        int nchunks, int skip_if_fact, const double* __restrict__ x,
                        const double* __restrict__ y, const double* __restrict__ z,
-                       const double* __restrict__ w, double* __restrict__ part) {
+                       const double* __restrict__ w, const TileBox* __restrict__ box,
+                       unsigned long long* __restrict__ cutstats, double* __restrict__ part) {
     const int slot0 = blockIdx.x * ENT_THREADS;
     if (slot0 >= L->npad) return;
     if (skip_if_fact && fact_usable(T, L)) return;   // the factorised kernel does this pass
@@ -50,6 +111,10 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
     const int tpc = ceil_div(ntiles, nchunks);
     const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
     const int i0 = (NI == NQ) ? 0 : blockIdx.z * NI;
+    static_assert(ENT_THREADS == 2 * ENT_SRC_TILE, "a target tile is two boxes");
+    const TileBox tbox = box_union(box[slot0 / ENT_SRC_TILE], box[slot0 / ENT_SRC_TILE + 1]);
+    const double cutT = L->cut_T[s], kmax3 = 1.7320508075688772 * fabs(T->knot[NQ - 1]);
+    int nskip = 0;
 
     __shared__ double sx[ENT_SRC_TILE], sy[ENT_SRC_TILE], sz[ENT_SRC_TILE], sw[ENT_SRC_TILE];
     double kn[NQ];
@@ -67,6 +132,7 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
             for (int l = 0; l < NQ; ++l) acc[i][j][l] = 0.0;
 
     for (int t = t0; t < t1; ++t) {
+        if (tile_is_far(tbox, box[src0 / ENT_SRC_TILE + t], cutT, kmax3)) { ++nskip; continue; }   // block-uniform
         __syncthreads();
         if (threadIdx.x < ENT_SRC_TILE) {
             const int q = src0 + t * ENT_SRC_TILE + threadIdx.x;
@@ -96,6 +162,10 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
                     for (int l = 0; l < NQ; ++l) acc[i][j][l] = fma(b, ez[l], acc[i][j][l]);
                 }
         }
+    }
+    if (threadIdx.x == 0 && blockIdx.z == 0 && t1 > t0) {
+        atomicAdd(cutstats, (unsigned long long)(t1 - t0));
+        atomicAdd(cutstats + 1, (unsigned long long)nskip);
     }
     const size_t M = (size_t)NQ * NQ * NQ;
 #pragma unroll

@@ -35,20 +35,29 @@ struct FactCfg {
 // One block per species: bounding box of its (real) markers -> centre and half-width.
 __global__ void __launch_bounds__(1024)
 entropy_bounds_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, const double* __restrict__ x,
-                      const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ w) {
+                      const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ w,
+                      int cutoff_on) {
     const int s = blockIdx.x;
     const int p0 = L->off[s], p1 = L->off[s + 1];
     const double BIG = 1.7976931348623157e308;
     double lo[3] = {BIG, BIG, BIG}, hi[3] = {-BIG, -BIG, -BIG};
+    double wlo = BIG, whi = 0.0;
     for (int p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
         if (w[p] > 0.0) {
             const double a = x[p], b = y[p], c = z[p];
             lo[0] = fmin(lo[0], a); hi[0] = fmax(hi[0], a);
             lo[1] = fmin(lo[1], b); hi[1] = fmax(hi[1], b);
             lo[2] = fmin(lo[2], c); hi[2] = fmax(hi[2], c);
+            wlo = fmin(wlo, w[p]); whi = fmax(whi, w[p]);
         }
     }
-    __shared__ double slo[32][3], shi[32][3];
+    __shared__ double slo[32][3], shi[32][3], swlo[32], swhi[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        wlo = fmin(wlo, __shfl_xor_sync(0xffffffffu, wlo, o));
+        whi = fmax(whi, __shfl_xor_sync(0xffffffffu, whi, o));
+    }
+    if ((threadIdx.x & 31) == 0) { swlo[threadIdx.x >> 5] = wlo; swhi[threadIdx.x >> 5] = whi; }
     const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
@@ -70,6 +79,12 @@ entropy_bounds_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L,
             hw = fmax(hw, 0.5 * b - 0.5 * a);
         }
         L->halfwidth[s] = hw * T->inv_sqrt_2eps[s];
+        // Gaussian cutoff threshold of this species (entropy.cuh, tile_is_far)
+        double a = BIG, b = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { a = fmin(a, swlo[k]); b = fmax(b, swhi[k]); }
+        const int cnt = L->count[s];
+        L->cut_T[s] = (cutoff_on && cnt > 0 && a > 0.0 && b >= a)
+                          ? 60.0 * 0.69314718055994531 + log(b / a) + log((double)cnt) : BIG;
     }
 }
 

@@ -30,6 +30,7 @@ constexpr int MMA_THREADS = 128;   // 4 warps, 32 targets each
 constexpr int MMA_TILE = 64;       // sources per stage
 constexpr int MMA_MT = 4;          // 8-target blocks per warp
 constexpr int MMA_ROW = 68;        // doubles per product-table row
+constexpr int MMA_LCAP = 1024;     // source tiles per segment of the active-tile list (Gaussian cutoff)
 
 template <int NQ>
 struct MmaCfg {
@@ -40,7 +41,8 @@ struct MmaCfg {
     static constexpr int NL = NBG * 8;                              // nodes per group (<= 64)
     static constexpr int REC = FactCfg<NQ>::REC;
     static constexpr size_t SMEM =
-        sizeof(double) * (2 * MMA_TILE * MMA_ROW + 2 * MMA_TILE * REC + 64) + 2 * sizeof(uint64_t);
+        sizeof(double) * (2 * MMA_TILE * MMA_ROW + 2 * MMA_TILE * REC + 64) + 2 * sizeof(uint64_t) +
+        sizeof(int) * (MMA_LCAP + 8);
 };
 
 // exp(-r2) for r2 >= 0, FP64, ~1.5 ulp, 10 FP64-pipe instructions: N = round(-r2 * 64/ln 2),
@@ -77,7 +79,8 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 template <int NQ>
 __global__ void __launch_bounds__(MMA_THREADS, 2)
 entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
-                   const double* __restrict__ rec, double* __restrict__ part) {
+                   const double* __restrict__ rec, const TileBox* __restrict__ box,
+                   unsigned long long* __restrict__ cutstats, double* __restrict__ part) {
     using C = MmaCfg<NQ>;
     constexpr int REC = C::REC, MT = MMA_MT, NBG = C::NBG, NL = C::NL, M = C::M;
     const int slot0 = blockIdx.x * MMA_THREADS;
@@ -89,7 +92,6 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     const int ntiles = (src1 - src0) / MMA_TILE;
     const int tpc = ceil_div(ntiles, nchunks);
     const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
-    const int n = max(0, t1 - t0);
     const int node0 = blockIdx.z * NL;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -97,6 +99,8 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     double* s_rec = s_prod + 2 * MMA_TILE * MMA_ROW;                 // [2][MMA_TILE * REC]
     double* s_e2 = s_rec + 2 * MMA_TILE * REC;                       // [64]  2^(j/64)
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_e2 + 64);        // [2]
+    int* s_list = reinterpret_cast<int*>(s_bar + 2);                 // [MMA_LCAP] active source tiles of a segment
+    int* s_wcnt = s_list + MMA_LCAP;                                 // [4]
     const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
     const int lr = lane >> 2, lc = lane & 3;                         // fragment row / column of this lane
     if (tid < 64) s_e2[tid] = T->exp2_tab[tid];
@@ -107,13 +111,15 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     }
     __syncthreads();
 
-    auto issue = [&](int k) {                                        // k-th tile of this chunk -> s_rec[k & 1]
+    // gk counts the tiles loaded by this block so far (stage = gk & 1, mbarrier parity = (gk >> 1) & 1); li is the
+    // tile's position in the active list of the current segment
+    auto issue = [&](int gk, int li) {
         if (tid == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             constexpr uint32_t BYTES = MMA_TILE * REC * (uint32_t)sizeof(double);
-            mbar_expect_tx(&s_bar[k & 1], BYTES);
-            bulk_g2s(s_rec + (size_t)(k & 1) * MMA_TILE * REC,
-                     rec + ((size_t)src0 + (size_t)(t0 + k) * MMA_TILE) * REC, BYTES, &s_bar[k & 1]);
+            mbar_expect_tx(&s_bar[gk & 1], BYTES);
+            bulk_g2s(s_rec + (size_t)(gk & 1) * MMA_TILE * REC,
+                     rec + ((size_t)src0 + (size_t)s_list[li] * MMA_TILE) * REC, BYTES, &s_bar[gk & 1]);
         }
     };
     // product-table builder: lane = node (conflict-free: a warp reads <= NQ distinct factors of ONE record per
@@ -149,15 +155,37 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
 #pragma unroll
         for (int nb = 0; nb < NBG; ++nb) acc[mt][nb][0] = acc[mt][nb][1] = 0.0;
 
-    if (n > 0) {
-        issue(0);
-        if (n > 1) issue(1);
-        build(0);
+    // Gaussian cutoff (entropy.cuh): source tiles whose box is far from this block's 128 targets are not visited
+    static_assert(MMA_THREADS == 2 * MMA_TILE, "a target tile is two boxes");
+    const TileBox tbox = box_union(box[slot0 / MMA_TILE], box[slot0 / MMA_TILE + 1]);
+    const double cutT = L->cut_T[s], kmax3 = 1.7320508075688772 * fabs(T->knot[NQ - 1]);
+    int gbase = 0, nskip = 0;
+    for (int seg0 = t0; seg0 < t1; seg0 += MMA_LCAP) {
+    const int seg1 = min(t1, seg0 + MMA_LCAP);
+    int n = 0;
+    for (int base = seg0; base < seg1; base += MMA_THREADS) {
+        const int t = base + tid;
+        const bool act = t < seg1 && !tile_is_far(tbox, box[src0 / MMA_TILE + t], cutT, kmax3);
+        const unsigned m = __ballot_sync(0xffffffffu, act);
+        if (lane == 0) s_wcnt[wv] = __popc(m);
         __syncthreads();
-        if (n > 2) issue(2);
+        int off = n;
+        for (int q = 0; q < wv; ++q) off += s_wcnt[q];
+        if (act) s_list[off + __popc(m & ((1u << lane) - 1u))] = t;
+        n += s_wcnt[0] + s_wcnt[1] + s_wcnt[2] + s_wcnt[3];
+        __syncthreads();
     }
-    for (int k = 0; k < n; ++k) {
-        if (k + 1 < n) build(k + 1);
+    nskip += (seg1 - seg0) - n;
+    if (n > 0) {
+        issue(gbase, 0);
+        if (n > 1) issue(gbase + 1, 1);
+        build(gbase);
+        __syncthreads();
+        if (n > 2) issue(gbase + 2, 2);
+    }
+    for (int kk = 0; kk < n; ++kk) {
+        const int k = gbase + kk;
+        if (kk + 1 < n) build(k + 1);
         const double* pr = s_prod + (size_t)(k & 1) * MMA_TILE * MMA_ROW;
 #pragma unroll 2
         for (int ks = 0; ks < MMA_TILE / 4; ++ks) {
@@ -179,7 +207,13 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
                 for (int nb = 0; nb < NBG; ++nb) dmma884(acc[mt][nb][0], acc[mt][nb][1], A[mt], Bf[nb]);
         }
         __syncthreads();
-        if (k + 3 < n) issue(k + 3);
+        if (kk + 3 < n) issue(k + 3, kk + 3);
+    }
+    gbase += n;
+    }
+    if (tid == 0 && blockIdx.z == 0 && t1 > t0) {
+        atomicAdd(cutstats, (unsigned long long)(t1 - t0));
+        atomicAdd(cutstats + 1, (unsigned long long)nskip);
     }
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {

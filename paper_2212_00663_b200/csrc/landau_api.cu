@@ -80,7 +80,9 @@ struct landau_ctx {
     void* h_pin = nullptr;                // pinned read-back area
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
-    Buf facttab;
+    Buf facttab, tilebox;
+    unsigned long long* d_cutstats = nullptr;   // pass 1 Gaussian cutoff: {source tiles considered, skipped}
+    int cutoff_on = 1;                          // landau_set_cutoff
     Buf sym_acc, sym_tpart, sym_ticket;   // symmetric pair kernel: in-place source sums, target segments, unit tickets
     // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
     bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {};
@@ -127,7 +129,8 @@ constexpr size_t PIN_BYTES = 1 << 16;
 // pinned read-back area: [0, 8) finish()'s {err, used_fact}; [PIN_CTRL, +sizeof(StepCtrl)) the step control block;
 // [PIN_MOM, ...) per-species moment sums
 constexpr size_t PIN_CTRL = 128, PIN_MOM = 512;
-static_assert(PIN_CTRL >= 2 * sizeof(int) && PIN_CTRL + sizeof(StepCtrl) <= PIN_MOM, "pinned read-back areas overlap");
+static_assert(PIN_CTRL >= 2 * sizeof(int) && PIN_CTRL + 64 + 16 <= PIN_MOM && sizeof(StepCtrl) <= 64,
+              "pinned read-back areas overlap");
 static_assert(PIN_MOM + sizeof(double) * LD_MAX_SPECIES * 16 <= PIN_BYTES, "pinned read-back area too small");
 
 int fail(landau_ctx* c, int code, const char* fmt, ...) {
@@ -376,7 +379,8 @@ template <int NQ, int NI>
 void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks, int skip_if_fact) {
     dim3 grid(cl.npad_max / ENT_THREADS, nchunks, NQ / NI);
     entropy_literal_kernel<NQ, NI><<<grid, ENT_THREADS, 0, c->stream>>>(
-        c->d_tab, cl.L(), cl.npad_max, nchunks, skip_if_fact, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->part.p);
+        c->d_tab, cl.L(), cl.npad_max, nchunks, skip_if_fact, cl.x(), cl.y(), cl.z(), cl.w(),
+        (const TileBox*)c->tilebox.p, c->d_cutstats, (double*)c->part.p);
 }
 
 template <int NQ, int NI>
@@ -403,7 +407,8 @@ int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks) {
     }
     dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
     kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
-                                                    (const double*)c->facttab.p, (double*)c->part.p);
+                                                    (const double*)c->facttab.p, (const TileBox*)c->tilebox.p,
+                                                    c->d_cutstats, (double*)c->part.p);
     return 0;
 }
 
@@ -431,10 +436,16 @@ int entropy(landau_ctx* c, Cloud& cl) {
     nchunks = std::min(nchunks, 64);
     while (nchunks > 1 && (size_t)nchunks * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) --nchunks;
     RC(ensure(c, c->part, (size_t)nchunks * M * cl.npad_max * sizeof(double)));
+    RC(ensure(c, c->tilebox, sizeof(TileBox) * ((size_t)cl.npad_max / ENT_SRC_TILE + 2)));
     {
     ProfScope prof(c, 1);
+    // species extents (range guard of the factorised forms) and weights (Gaussian cutoff threshold); tile boxes
+    CU(cudaMemsetAsync(c->d_cutstats, 0, 2 * sizeof(unsigned long long), c->stream));
+    entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), c->cutoff_on);
+    entropy_tilebox_kernel<<<cl.npad_max / ENT_SRC_TILE, 64, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
+                                                                             cl.z(), cl.w(), (TileBox*)c->tilebox.p);
+    c->launches += 2;
     if (mode != 1) {
-        entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w());
         if (use_mma) switch (nq) {
             case 2: RC((launch_entropy_mma<2>(c, cl, nchunks))); break;
             case 3: RC((launch_entropy_mma<3>(c, cl, nchunks))); break;
@@ -455,7 +466,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
             case 8: RC((launch_entropy_fact<8, 1>(c, cl, nchunks))); break;
             default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
         }
-        c->launches += 3;
+        c->launches += 2;
     }
     if (mode != 2 && mode != 3) {
         const int skip = mode == 0 ? 1 : 0;
@@ -949,6 +960,8 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_aa, sizeof(AndersonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_nk, sizeof(NewtonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_cutstats, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMemset(c->d_cutstats, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMallocHost(&c->h_pin, PIN_BYTES) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMemcpy(c->d_tab, &t, sizeof(t), cudaMemcpyHostToDevice) != cudaSuccess) return bail(LANDAU_ECUDA);
@@ -967,6 +980,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_cursor) cudaFree(c->d_cursor);
     if (c->d_aa) cudaFree(c->d_aa);
     if (c->d_nk) cudaFree(c->d_nk);
+    if (c->d_cutstats) cudaFree(c->d_cutstats);
     destroy_step_graph(c);
     if (c->body_stream) cudaStreamDestroy(c->body_stream);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -978,7 +992,7 @@ void landau_destroy(landau_ctx* c) {
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
                    &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32, &c->sym_acc,
-                   &c->sym_tpart, &c->sym_ticket})
+                   &c->sym_tpart, &c->sym_ticket, &c->tilebox})
         release(*b);
     delete c;
 }
@@ -1219,6 +1233,25 @@ int landau_set_substep(landau_ctx* c, int max_halvings) {
     if (!c) return LANDAU_EINVAL;
     if (max_halvings < 0 || max_halvings > 10) return fail(c, LANDAU_EINVAL, "set_substep: max_halvings must be 0..10");
     c->substep = max_halvings;
+    return 0;
+}
+
+int landau_set_cutoff(landau_ctx* c, int on) {
+    if (!c) return LANDAU_EINVAL;
+    c->cutoff_on = on != 0;
+    c->state.G_valid = false; c->tmp.G_valid = false;
+    ++c->alloc_gen;                                  // a captured step graph has the old setting baked in
+    return 0;
+}
+
+int landau_cutoff_stats(landau_ctx* c, int64_t* tiles_considered, int64_t* tiles_skipped) {
+    if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
+    unsigned long long* h = (unsigned long long*)((char*)c->h_pin + PIN_CTRL + 64);
+    CU(cudaMemcpyAsync(h, c->d_cutstats, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (tiles_considered) *tiles_considered = (int64_t)h[0];
+    if (tiles_skipped) *tiles_skipped = (int64_t)h[1];
     return 0;
 }
 

@@ -584,6 +584,39 @@ def test_graph_step_with_accelerated_solvers_is_bit_identical(B, solver, depth, 
     assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: Gaussian cutoff of pass 1
+@pytest.mark.parametrize("entropy_kernel", [0, 1])
+@pytest.mark.parametrize("test,n_grid", [(3, 40), (1, 32), (2, 48)])
+def test_gaussian_cutoff_paper_meshes_match_the_all_pairs_oracle(B, oracle_mod, entropy_kernel, test, n_grid):
+    """Pass 1 with the Gaussian cutoff on the paper's own meshes and mollifier rule eps_s = 1.2 (L_s/N)^1.98
+    (PAPER.md:208): source tiles beyond the cutoff distance are skipped (stats > 0), and G, S_eps still equal the
+    ORACLE's all-pairs literal Eq. (22) to 1e-10 (the skipped terms are < 2^-60 of every node sum)."""
+    wl = W.paper_test(test, n_grid=n_grid)
+    g, o = make_pair(B, oracle_mod, wl, entropy_kernel=entropy_kernel)
+    Gref, Sref = o.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    Ggot, Sgot = g.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    considered, skipped = g.cutoff_stats()
+    assert considered > 0 and skipped > 0.2 * considered, (considered, skipped)
+    assert_field_close(Ggot.cpu().numpy(), Gref, wl.species_id, wl.n_species, what="entropy gradient with cutoff")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+    g.set_cutoff(False)
+    Gall = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert g.cutoff_stats()[1] < 0.5 * skipped          # cutoff off: only tiles made of padding slots are skipped
+    assert_field_close(Ggot.cpu().numpy(), Gall, wl.species_id, wl.n_species, tol=1e-13, what="cutoff vs all pairs")
+
+
+@pytest.mark.parametrize("eps_rule", [0.05, 0.004, 0.0005])
+def test_gaussian_cutoff_random_clouds_and_weights(B, oracle_mod, eps_rule):
+    """Random 3-V clouds with lognormal (sigma = 1) weights, from BASELINE's mollifier down to one 100 times smaller
+    (where most pairs are numerically zero): cutoff on == oracle all pairs, whatever the marker order."""
+    wl = W.make(4, n_per_species=700, shuffled=True, eps_rule=eps_rule)
+    g, o = make_pair(B, oracle_mod, wl)
+    Gref, Sref = o.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    Ggot, Sgot = g.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    assert_field_close(Ggot.cpu().numpy(), Gref, wl.species_id, wl.n_species, what="entropy gradient with cutoff")
+    np.testing.assert_allclose(Sgot, Sref, rtol=1e-11, atol=1e-12)
+
+
 # ------------------------------------------------------------------------------------ NEXT-2: the paper's 2-V setting
 def test_two_v_mode_keeps_vz_zero_and_matches_oracle(B, oracle_mod):
     """landau_set_dimension(2) on the paper's test 3.3 initial data (grid-initialised anisotropic Maxwellians,
