@@ -134,9 +134,13 @@ int landau_set_dimension(landau_ctx* ctx, int dim);
  * Gauss-Hermite knot): everything skipped changes no node sum of Eq. (22) by more than 2^-60 relative (derivation in
  * csrc/entropy.cuh), so results agree with the all-pairs evaluation to round-off.  It pays when eps_s is small against
  * the extent of the cloud -- the paper's own rule eps_s = 1.2 (L_s/N)^1.98 -- and costs one
- * box test per tile pair otherwise.  on = 0: all pairs.  landau_cutoff_stats returns the number of (target block,
- * source tile) pairs considered / skipped by the LAST pass 1 (HOST outputs; synchronises). */
-int landau_set_cutoff(landau_ctx* ctx, int on);
+ * box test per tile pair otherwise.  on = 0: all pairs.  morton = 1 (default): clouds of 4096 .. 2^21 markers are
+ * bucketed, inside every species, along a Morton curve through the cells of a mesh over the species' bounding box
+ * (stable inside a cell), so that tiles are compact boxes whatever the caller's marker order; morton = 0 keeps the
+ * caller's order inside a species (takes effect at the next landau_set_markers / field evaluation).  Outputs are
+ * in caller order either way.  landau_cutoff_stats returns the number of (target block, source tile) pairs
+ * considered / skipped by the LAST pass 1 (HOST outputs; synchronises). */
+int landau_set_cutoff(landau_ctx* ctx, int on, int morton);
 int landau_cutoff_stats(landau_ctx* ctx, int64_t* tiles_considered, int64_t* tiles_skipped);
 
 /* How landau_step / landau_run issue a step whose cost is launch latency (small clouds).  mode 1 (default,

@@ -88,7 +88,7 @@ def load(build_if_missing: bool = True):
     lib.landau_set_dimension.argtypes = [vp, C.c_int]
     lib.landau_set_step_graph.argtypes = [vp, C.c_int]
     lib.landau_set_substep.argtypes = [vp, C.c_int]
-    lib.landau_set_cutoff.argtypes = [vp, C.c_int]
+    lib.landau_set_cutoff.argtypes = [vp, C.c_int, C.c_int]
     lib.landau_cutoff_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.landau_cells_run.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int,
                                      C.POINTER(CellInfo)]
@@ -282,9 +282,10 @@ class Landau:
         """0 = commit unconverged steps (the paper's behaviour); k > 0 = redo them as two half steps, up to k levels."""
         self._check(self._lib.landau_set_substep(self._h, int(max_halvings)), "landau_set_substep")
 
-    def set_cutoff(self, on: bool = True):
-        """Gaussian cutoff of pass 1 (NEXT-4): skip source tiles that cannot change a node sum by 2^-60 relative."""
-        self._check(self._lib.landau_set_cutoff(self._h, int(bool(on))), "landau_set_cutoff")
+    def set_cutoff(self, on: bool = True, morton: bool = True):
+        """Gaussian cutoff of pass 1 (NEXT-4): skip source tiles that cannot change a node sum by 2^-60 relative;
+        morton: bucket every species along a Morton curve at pack time so that tiles are compact."""
+        self._check(self._lib.landau_set_cutoff(self._h, int(bool(on)), int(bool(morton))), "landau_set_cutoff")
 
     def cutoff_stats(self):
         """(source tiles considered, skipped) by the last pass 1."""

@@ -81,6 +81,9 @@ struct landau_ctx {
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
     Buf facttab, tilebox;
+    Buf cellkey, cellrank, chunkcnt, binoff, spbox;   // Morton bucketing of pack (pack.cuh)
+    int morton_on = 1;                                // landau_set_cutoff(.., morton)
+    size_t attr_cellcount = 0;
     unsigned long long* d_cutstats = nullptr;   // pass 1 Gaussian cutoff: {source tiles considered, skipped}
     int cutoff_on = 1;                          // landau_set_cutoff
     Buf sym_acc, sym_tpart, sym_ticket;   // symmetric pair kernel: in-place source sums, target segments, unit tickets
@@ -367,9 +370,41 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
     CU(cudaMemsetAsync(cl.perm.p, 0xFF, sizeof(int) * (size_t)npm, st));
     pack_count_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, sid, S, (int*)c->blockcnt.p, cl.L());
     pack_scan_kernel<<<1, 32, 0, st>>>(nb, S, pad, (const int*)c->blockcnt.p, (int*)c->blockoff.p, cl.L());
-    pack_scatter_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, sid, S, (const int*)c->blockoff.p, cl.L(),
-                                                      cl.x(), cl.y(), cl.z(), cl.w(), cl.prm());
-    c->launches += 3;
+    c->launches += 2;
+    // clouds with many tiles: order every species along a Morton curve (compact tiles for pass 1's Gaussian cutoff)
+    if (c->morton_on && N >= 4096 && N <= ((int64_t)1 << 21)) {
+        int LC = 0;
+        while (LC < 7 && (N / S) >> (3 * LC) > 32 && ((int64_t)S << (3 * (LC + 1))) <= CELL_MAX_BINS) ++LC;
+        const int nbins = S << (3 * LC);
+        const int nchunks = ceil_div((int)N, CELL_CHUNK);
+        RC(ensure(c, c->cellkey, sizeof(int) * (size_t)N));
+        RC(ensure(c, c->cellrank, sizeof(int) * (size_t)N));
+        RC(ensure(c, c->chunkcnt, sizeof(int) * (size_t)nchunks * nbins));
+        RC(ensure(c, c->binoff, sizeof(int) * (2 * (size_t)nbins + 2)));
+        RC(ensure(c, c->spbox, sizeof(SpeciesBox)));
+        const size_t smem = sizeof(int) * (size_t)nbins;
+        if (smem > 48 * 1024 && smem > c->attr_cellcount) {
+            CU(cudaFuncSetAttribute(pack_cell_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            c->attr_cellcount = smem;
+        }
+        int* binoff = (int*)c->binoff.p;
+        int* bintot = binoff + nbins + 1;
+        pack_box_init_kernel<<<1, 64, 0, st>>>((SpeciesBox*)c->spbox.p);
+        pack_box_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, sid, S, (SpeciesBox*)c->spbox.p);
+        pack_cell_count_kernel<<<nchunks, PACK_THREADS, smem, st>>>((int)N, v, sid, S, LC, nbins,
+                                                                    (const SpeciesBox*)c->spbox.p, (int*)c->cellkey.p,
+                                                                    (int*)c->cellrank.p, (int*)c->chunkcnt.p);
+        pack_cell_scan_chunks_kernel<<<ceil_div(nbins, 256), 256, 0, st>>>(nchunks, nbins, (int*)c->chunkcnt.p, bintot);
+        pack_cell_scan_bins_kernel<<<1, 1024, 0, st>>>(nbins, bintot, binoff);
+        pack_cell_scatter_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, S, LC, nbins, (const int*)c->cellkey.p,
+                                                              (const int*)c->cellrank.p, (const int*)c->chunkcnt.p,
+                                                              binoff, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), cl.prm());
+        c->launches += 6;
+    } else {
+        pack_scatter_kernel<<<nb, PACK_THREADS, 0, st>>>((int)N, v, w, sid, S, (const int*)c->blockoff.p, cl.L(),
+                                                          cl.x(), cl.y(), cl.z(), cl.w(), cl.prm());
+        c->launches += 1;
+    }
     CU(cudaGetLastError());
     return 0;
 }
@@ -992,7 +1027,8 @@ void landau_destroy(landau_ctx* c) {
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
                    &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32, &c->sym_acc,
-                   &c->sym_tpart, &c->sym_ticket, &c->tilebox})
+                   &c->sym_tpart, &c->sym_ticket, &c->tilebox, &c->cellkey,
+                   &c->cellrank, &c->chunkcnt, &c->binoff, &c->spbox})
         release(*b);
     delete c;
 }
@@ -1236,9 +1272,10 @@ int landau_set_substep(landau_ctx* c, int max_halvings) {
     return 0;
 }
 
-int landau_set_cutoff(landau_ctx* c, int on) {
+int landau_set_cutoff(landau_ctx* c, int on, int morton) {
     if (!c) return LANDAU_EINVAL;
     c->cutoff_on = on != 0;
+    c->morton_on = morton != 0;
     c->state.G_valid = false; c->tmp.G_valid = false;
     ++c->alloc_gen;                                  // a captured step graph has the old setting baked in
     return 0;
