@@ -183,7 +183,9 @@ int landau_run(landau_ctx* ctx, int n_steps, double dt, double tol, int max_iter
  * midpoint (the discrete gradient of the quadratic K); the entropy gradient is Gonzalez' midpoint discrete
  * gradient  dbar S/dv_p = w_p G_p(u) + lambda (v_p^{n+1} - v_p^n)  (reading DG1).  Same Jacobi fixed
  * point, residual, status and info conventions as landau_step; every iteration costs two pass-1 and one
- * pass-2 evaluations and the loop is driven from the host (three small read-backs per iteration). */
+ * pass-2 evaluations.  Device driven: the entropies, lambda's sums and the residual are reduced on the device and
+ * every kernel of an iteration exits at once when the step is done; the host enqueues iterations in chunks of 8 and
+ * reads the done flag once per chunk (no read-back inside an iteration). */
 int landau_step_dg(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
 
 /* many spatial collision cells in one call.  The bracket couples only markers of the same

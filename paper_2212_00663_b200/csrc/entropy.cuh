@@ -54,7 +54,8 @@ __device__ __forceinline__ bool tile_is_far(const TileBox& a, const TileBox& b, 
 __global__ void __launch_bounds__(64)
 entropy_tilebox_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
                        const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
-                       const double* __restrict__ w, TileBox* __restrict__ box) {
+                       const double* __restrict__ w, TileBox* __restrict__ box, const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;      // a device-driven loop (step_dg) has finished: the rest of its launches exit
     const int p = blockIdx.x * 64 + threadIdx.x;
     const double BIG = 1.7976931348623157e308;
     double lo[3] = {BIG, BIG, BIG}, hi[3] = {-BIG, -BIG, -BIG};
@@ -99,7 +100,9 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
                        int nchunks, int skip_if_fact, const double* __restrict__ x,
                        const double* __restrict__ y, const double* __restrict__ z,
                        const double* __restrict__ w, const TileBox* __restrict__ box,
-                       unsigned long long* __restrict__ cutstats, double* __restrict__ part) {
+                       unsigned long long* __restrict__ cutstats, double* __restrict__ part,
+                       const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     const int slot0 = blockIdx.x * ENT_THREADS;
     if (slot0 >= L->npad) return;
     if (skip_if_fact && fact_usable(T, L)) return;   // the factorised kernel does this pass
@@ -188,7 +191,8 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
                         const double* __restrict__ px, const double* __restrict__ py,
                         const double* __restrict__ pz, int fact_mode,
                         double* __restrict__ Gx, double* __restrict__ Gy, double* __restrict__ Gz,
-                        double* __restrict__ snode) {
+                        double* __restrict__ snode, const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npad_max || p >= L->npad) return;
     const bool factorised = fact_mode != 0 && fact_usable(T, L);

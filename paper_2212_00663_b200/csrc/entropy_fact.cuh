@@ -36,7 +36,8 @@ struct FactCfg {
 __global__ void __launch_bounds__(1024)
 entropy_bounds_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, const double* __restrict__ x,
                       const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ w,
-                      int cutoff_on) {
+                      int cutoff_on, const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     const int s = blockIdx.x;
     const int p0 = L->off[s], p1 = L->off[s + 1];
     const double BIG = 1.7976931348623157e308;
@@ -94,7 +95,9 @@ template <int NQ>
 __global__ void entropy_fact_prep_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                                          int npad_max, const double* __restrict__ x,
                                          const double* __restrict__ y, const double* __restrict__ z,
-                                         const double* __restrict__ w, double* __restrict__ rec) {
+                                         const double* __restrict__ w, double* __restrict__ rec,
+                                         const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     constexpr int REC = FactCfg<NQ>::REC;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npad_max) return;
@@ -159,7 +162,8 @@ __device__ __forceinline__ double exp_neg(double r2) {
 template <int NQ, int NI>
 __global__ void __launch_bounds__(FACT_THREADS)
 entropy_fact_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
-                    const double* __restrict__ rec, double* __restrict__ part) {
+                    const double* __restrict__ rec, double* __restrict__ part, const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     constexpr int REC = FactCfg<NQ>::REC;
     const int slot0 = blockIdx.x * FACT_THREADS;
     if (slot0 >= L->npad) return;

@@ -80,7 +80,9 @@ template <int NQ>
 __global__ void __launch_bounds__(MMA_THREADS, 2)
 entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
                    const double* __restrict__ rec, const TileBox* __restrict__ box,
-                   unsigned long long* __restrict__ cutstats, double* __restrict__ part) {
+                   unsigned long long* __restrict__ cutstats, double* __restrict__ part,
+                   const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
     using C = MmaCfg<NQ>;
     constexpr int REC = C::REC, MT = MMA_MT, NBG = C::NBG, NL = C::NL, M = C::M;
     const int slot0 = blockIdx.x * MMA_THREADS;

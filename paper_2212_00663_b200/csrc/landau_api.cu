@@ -96,6 +96,7 @@ struct landau_ctx {
     int nk_m = 20;                        // GMRES restart length of the Newton-Krylov solver
     AndersonCtrl* d_aa = nullptr;
     NewtonCtrl* d_nk = nullptr;
+    DgCtrl* d_dg = nullptr;
     Buf aa_hist;
     Buf cells_off, cells_rec, soa32;
     // CUDA-graph form of a whole step for launch-bound (small) clouds, landau_set_step_graph
@@ -411,30 +412,30 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
 
 // ---- a1/a2: entropy gradient of a packed cloud ---------------------------------------------
 template <int NQ, int NI>
-void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks, int skip_if_fact) {
+void launch_entropy_literal(landau_ctx* c, Cloud& cl, int nchunks, int skip_if_fact, const StepCtrl* stop) {
     dim3 grid(cl.npad_max / ENT_THREADS, nchunks, NQ / NI);
     entropy_literal_kernel<NQ, NI><<<grid, ENT_THREADS, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, skip_if_fact, cl.x(), cl.y(), cl.z(), cl.w(),
-        (const TileBox*)c->tilebox.p, c->d_cutstats, (double*)c->part.p);
+        (const TileBox*)c->tilebox.p, c->d_cutstats, (double*)c->part.p, stop);
 }
 
 template <int NQ, int NI>
-int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks) {
+int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
     RC(ensure(c, c->facttab, sizeof(double) * FactCfg<NQ>::REC * (size_t)cl.npad_max));
     entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
-        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p);
+        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p, stop);
     dim3 grid(cl.npad_max / FACT_THREADS, nchunks, NQ / NI);
     entropy_fact_kernel<NQ, NI><<<grid, FACT_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
-                                                                      (const double*)c->facttab.p, (double*)c->part.p);
+                                                                      (const double*)c->facttab.p, (double*)c->part.p, stop);
     return 0;
 }
 
 template <int NQ>
-int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks) {
+int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
     using M = MmaCfg<NQ>;
     RC(ensure(c, c->facttab, sizeof(double) * M::REC * (size_t)cl.npad_max));
     entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
-        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p);
+        c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p, stop);
     auto kern = entropy_mma_kernel<NQ>;
     if (!c->attr_mma[NQ]) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)M::SMEM));
@@ -443,7 +444,7 @@ int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks) {
     dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
     kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
                                                     (const double*)c->facttab.p, (const TileBox*)c->tilebox.p,
-                                                    c->d_cutstats, (double*)c->part.p);
+                                                    c->d_cutstats, (double*)c->part.p, stop);
     return 0;
 }
 
@@ -455,7 +456,8 @@ int mma_groups(int nq) {
                   case 8: return MmaCfg<8>::GROUPS; default: return 1; }
 }
 
-int entropy(landau_ctx* c, Cloud& cl) {
+// stop != nullptr: every kernel of the pass exits at once when stop->done is set (device-driven loops)
+int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     const int nq = c->n_q;
     const size_t M = (size_t)nq * nq * nq;
     const int ttiles = cl.npad_max / ENT_THREADS;
@@ -476,29 +478,29 @@ int entropy(landau_ctx* c, Cloud& cl) {
     ProfScope prof(c, 1);
     // species extents (range guard of the factorised forms) and weights (Gaussian cutoff threshold); tile boxes
     CU(cudaMemsetAsync(c->d_cutstats, 0, 2 * sizeof(unsigned long long), c->stream));
-    entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), c->cutoff_on);
+    entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), c->cutoff_on, stop);
     entropy_tilebox_kernel<<<cl.npad_max / ENT_SRC_TILE, 64, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
-                                                                             cl.z(), cl.w(), (TileBox*)c->tilebox.p);
+                                                                             cl.z(), cl.w(), (TileBox*)c->tilebox.p, stop);
     c->launches += 2;
     if (mode != 1) {
         if (use_mma) switch (nq) {
-            case 2: RC((launch_entropy_mma<2>(c, cl, nchunks))); break;
-            case 3: RC((launch_entropy_mma<3>(c, cl, nchunks))); break;
-            case 4: RC((launch_entropy_mma<4>(c, cl, nchunks))); break;
-            case 5: RC((launch_entropy_mma<5>(c, cl, nchunks))); break;
-            case 6: RC((launch_entropy_mma<6>(c, cl, nchunks))); break;
-            case 7: RC((launch_entropy_mma<7>(c, cl, nchunks))); break;
-            case 8: RC((launch_entropy_mma<8>(c, cl, nchunks))); break;
+            case 2: RC((launch_entropy_mma<2>(c, cl, nchunks, stop))); break;
+            case 3: RC((launch_entropy_mma<3>(c, cl, nchunks, stop))); break;
+            case 4: RC((launch_entropy_mma<4>(c, cl, nchunks, stop))); break;
+            case 5: RC((launch_entropy_mma<5>(c, cl, nchunks, stop))); break;
+            case 6: RC((launch_entropy_mma<6>(c, cl, nchunks, stop))); break;
+            case 7: RC((launch_entropy_mma<7>(c, cl, nchunks, stop))); break;
+            case 8: RC((launch_entropy_mma<8>(c, cl, nchunks, stop))); break;
             default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
         }
         else switch (nq) {
-            case 2: RC((launch_entropy_fact<2, 2>(c, cl, nchunks))); break;
-            case 3: RC((launch_entropy_fact<3, 3>(c, cl, nchunks))); break;
-            case 4: RC((launch_entropy_fact<4, 4>(c, cl, nchunks))); break;
-            case 5: RC((launch_entropy_fact<5, 1>(c, cl, nchunks))); break;
-            case 6: RC((launch_entropy_fact<6, 2>(c, cl, nchunks))); break;
-            case 7: RC((launch_entropy_fact<7, 1>(c, cl, nchunks))); break;
-            case 8: RC((launch_entropy_fact<8, 1>(c, cl, nchunks))); break;
+            case 2: RC((launch_entropy_fact<2, 2>(c, cl, nchunks, stop))); break;
+            case 3: RC((launch_entropy_fact<3, 3>(c, cl, nchunks, stop))); break;
+            case 4: RC((launch_entropy_fact<4, 4>(c, cl, nchunks, stop))); break;
+            case 5: RC((launch_entropy_fact<5, 1>(c, cl, nchunks, stop))); break;
+            case 6: RC((launch_entropy_fact<6, 2>(c, cl, nchunks, stop))); break;
+            case 7: RC((launch_entropy_fact<7, 1>(c, cl, nchunks, stop))); break;
+            case 8: RC((launch_entropy_fact<8, 1>(c, cl, nchunks, stop))); break;
             default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
         }
         c->launches += 2;
@@ -506,13 +508,13 @@ int entropy(landau_ctx* c, Cloud& cl) {
     if (mode != 2 && mode != 3) {
         const int skip = mode == 0 ? 1 : 0;
         switch (nq) {
-            case 2: launch_entropy_literal<2, 2>(c, cl, nchunks, skip); break;
-            case 3: launch_entropy_literal<3, 3>(c, cl, nchunks, skip); break;
-            case 4: launch_entropy_literal<4, 4>(c, cl, nchunks, skip); break;
-            case 5: launch_entropy_literal<5, 1>(c, cl, nchunks, skip); break;
-            case 6: launch_entropy_literal<6, 1>(c, cl, nchunks, skip); break;
-            case 7: launch_entropy_literal<7, 1>(c, cl, nchunks, skip); break;
-            case 8: launch_entropy_literal<8, 1>(c, cl, nchunks, skip); break;
+            case 2: launch_entropy_literal<2, 2>(c, cl, nchunks, skip, stop); break;
+            case 3: launch_entropy_literal<3, 3>(c, cl, nchunks, skip, stop); break;
+            case 4: launch_entropy_literal<4, 4>(c, cl, nchunks, skip, stop); break;
+            case 5: launch_entropy_literal<5, 1>(c, cl, nchunks, skip, stop); break;
+            case 6: launch_entropy_literal<6, 1>(c, cl, nchunks, skip, stop); break;
+            case 7: launch_entropy_literal<7, 1>(c, cl, nchunks, skip, stop); break;
+            case 8: launch_entropy_literal<8, 1>(c, cl, nchunks, skip, stop); break;
             default: return fail(c, LANDAU_EINVAL, "n_q = %d unsupported", nq);
         }
         c->launches += 1;
@@ -520,7 +522,7 @@ int entropy(landau_ctx* c, Cloud& cl) {
     }
     entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
-        mode == 1 ? 0 : (mode >= 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode());
+        mode == 1 ? 0 : (mode >= 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode(), stop);
     c->launches += 1;
     CU(cudaGetLastError());
     cl.G_valid = true;
@@ -995,6 +997,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_aa, sizeof(AndersonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_nk, sizeof(NewtonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_dg, sizeof(DgCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cutstats, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMemset(c->d_cutstats, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
@@ -1015,6 +1018,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_cursor) cudaFree(c->d_cursor);
     if (c->d_aa) cudaFree(c->d_aa);
     if (c->d_nk) cudaFree(c->d_nk);
+    if (c->d_dg) cudaFree(c->d_dg);
     if (c->d_cutstats) cudaFree(c->d_cutstats);
     destroy_step_graph(c);
     if (c->body_stream) cudaStreamDestroy(c->body_stream);
@@ -1318,9 +1322,10 @@ int landau_step(landau_ctx* c, double dt, double tol, int max_iter, landau_step_
     return landau_run(c, 1, dt, tol, max_iter, info);
 }
 
-// NEXT-1: one discrete-gradient step (Eqs. 46-49; step_dg.cuh).  Host-driven loop: every iteration reads the
-// entropy sums, the lambda partials and the residual back (three small synchronisations against two pass-1 and
-// one pass-2 evaluations of work).
+// NEXT-1: one discrete-gradient step (Eqs. 46-49; step_dg.cuh).  Device driven: the entropies, Gonzalez' lambda and the
+// residual are reduced on the device and every kernel of an iteration exits at once when StepCtrl::done is set; the
+// host enqueues the iterations in chunks of DG_CHUNK and reads the done flag once per chunk (no read-back inside an
+// iteration).
 int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_step_info* info) {
     if (!c) return LANDAU_EINVAL;
     DevGuard dev_guard(c);
@@ -1328,6 +1333,7 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     if (cl.N < 1) return fail(c, LANDAU_EINVAL, "step_dg: no markers held (landau_set_markers first)");
     if (max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
         return fail(c, LANDAU_EINVAL, "step_dg: need max_iter >= 1, dt > 0, tol >= 0");
+    constexpr int DG_CHUNK = 8;
     const int npm = cl.npad_max;
     const size_t B4 = sizeof(double) * 4 * (size_t)npm;
     RC(ensure(c, c->vk, B4));
@@ -1336,7 +1342,7 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     RC(ensure(c, c->dg_Gk, B4));
     RC(ensure(c, c->records, sizeof(StepRecord)));
     const int nub = ceil_div(npm, UPD_THREADS), ndb = ceil_div(npm, DG_THREADS);
-    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(2 * nub, 4096)));
+    RC(ensure(c, c->blockpart, sizeof(double) * (size_t)step_blockpart_doubles(c, nub)));
     RC(ensure(c, c->dg_part, sizeof(double) * 2 * (size_t)ndb));
     double* xk = (double*)c->vk.p;
     double* yk = xk + npm;
@@ -1345,73 +1351,64 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     // cloud-shaped views that share the state's layout and permutation
     Cloud U = cl;  U.xyzw = c->dg_u;  U.G = c->dg_Gu;        // midpoint u, G(u)
     Cloud VK = cl; VK.xyzw = c->vk;   VK.G = c->dg_Gk;       // iterate v^(k), its entropy integrand
-    const double PI = 3.14159265358979323846;
-    double* hs = (double*)((char*)c->h_pin + PIN_MOM);
-    auto total_entropy = [&](Cloud& q, double* S_out) -> int {
-        RC(species_sums(c, q, true, false, hs));
-        double S = 0.0;
-        for (int s = 0; s < c->S; ++s) S += -hs[s * MOM_OUT + 11] / (PI * sqrt(PI));
-        *S_out = S;
-        return 0;
-    };
+    double* rec = cl.sym ? nullptr : cl.recs();
+    double* soa = cl.sym ? cl.soas() : nullptr;
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
     CU(cudaMemsetAsync(c->d_ctrl, 0, sizeof(StepCtrl), st));
     c->prof_step = 0; c->prof_iter = 0;
     if (!cl.G_valid) RC(entropy(c, cl));                      // G(v^n), entropy integrand at v^n
     cl.G_valid = false;
-    double S0 = 0.0;
-    RC(total_entropy(cl, &S0));
+    dg_begin_kernel<<<1, 32, 0, st>>>(c->d_dg);
     step_begin_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(),
-                                                           cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk,
-                                                           cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
+                                                           cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), xk, yk, zk, rec, soa);
+    dg_entropy_total_kernel<<<ndb, DG_THREADS, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.w(), cl.snode(), (double*)c->dg_part.p,
+                                                         c->d_dg, 0);
     CU(cudaMemcpyAsync(xk + 3 * (size_t)npm, cl.w(), sizeof(double) * (size_t)npm, cudaMemcpyDeviceToDevice, st));
-    c->launches += 1;
+    c->launches += 3;
     StepCtrl* hc = (StepCtrl*)((char*)c->h_pin + PIN_CTRL);
-    std::vector<double> hp(2 * (size_t)ndb);
     for (int k = 0; k < max_iter; ++k) {
         int nparts = 0;
         c->prof_iter = k;
         if (k > 0) {
-            dg_midpoint_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), npm, cl.x(), cl.y(), cl.z(), cl.w(), xk, yk,
-                                                                    zk, U.x());
-            RC(entropy(c, U));
-            RC(entropy(c, VK));
-            double Sk = 0.0;
-            RC(total_entropy(VK, &Sk));
-            dg_lambda_partial_kernel<<<ndb, DG_THREADS, 0, st>>>(cl.L(), npm, cl.x(), cl.y(), cl.z(), cl.w(), xk, yk, zk,
-                                                                 U.Gx(), U.Gy(), U.Gz(), (double*)c->dg_part.p);
-            CU(cudaMemcpyAsync(hp.data(), c->dg_part.p, sizeof(double) * 2 * (size_t)ndb, cudaMemcpyDeviceToHost, st));
-            CU(cudaStreamSynchronize(st));
-            double lin = 0.0, dv2 = 0.0;
-            for (int b = 0; b < ndb; ++b) { lin += hp[2 * b]; dv2 += hp[2 * b + 1]; }
-            const double lambda = dv2 > 0.0 ? (Sk - S0 - lin) / dv2 : 0.0;
-            dg_build_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), npm, lambda, U.x(), cl.x(), cl.y(),
-                                                                 cl.z(), xk, yk, zk, U.Gx(), U.Gy(), U.Gz(),
-                                                                 cl.sym ? nullptr : cl.recs(),
-                                                                 cl.sym ? cl.soas() : nullptr);
-            c->launches += 3;
+            dg_midpoint_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                                    xk, yk, zk, U.x());
+            RC(entropy(c, U, c->d_ctrl));
+            RC(entropy(c, VK, c->d_ctrl));
+            dg_entropy_total_kernel<<<ndb, DG_THREADS, 0, st>>>(cl.L(), c->d_ctrl, npm, VK.w(), VK.snode(),
+                                                                 (double*)c->dg_part.p, c->d_dg, 1);
+            dg_lambda_kernel<<<ndb, DG_THREADS, 0, st>>>(cl.L(), c->d_ctrl, c->d_dg, npm, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                          xk, yk, zk, U.Gx(), U.Gy(), U.Gz(), (double*)c->dg_part.p);
+            dg_build_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, c->d_dg, npm, U.x(), cl.x(),
+                                                                 cl.y(), cl.z(), xk, yk, zk, U.Gx(), U.Gy(), U.Gz(), rec, soa);
+            c->launches += 4;
         }
         RC(pair(c, cl, c->d_ctrl, &nparts));
         step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                          (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
-                                                         xk, yk, zk, cl.sym ? nullptr : cl.recs(),
-                                                         cl.sym ? cl.soas() : nullptr, (double*)c->blockpart.p, 0);
+                                                         xk, yk, zk, rec, soa, (double*)c->blockpart.p, 0);
         c->launches += 1;
-        CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
-        if (hc->done) break;
+        if ((k + 1) % DG_CHUNK == 0 && k + 1 < max_iter) {    // one look at the flag per chunk of iterations
+            CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            if (hc->done) break;
+        }
     }
     step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk, zk,
                                                             (StepRecord*)c->records.p, c->d_cursor);
     c->launches += 1;
     CU(cudaGetLastError());
-    const int iterations = hc->iterations, converged = hc->converged, cerr = hc->err;
-    const double residual = hc->residual;
+    CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
+    c->in_run = true;
     int rc = finish(c, cl, "step_dg");
+    c->in_run = false;
+    if (c->prof_on) {
+        const int its = hc->iterations;
+        prof_resolve(c, &its, 1);
+    }
     if (rc < 0) return rc;
-    if (cerr) return fail(c, cerr, "step_dg: non-finite residual");
-    if (info) { info->iterations = iterations; info->residual = residual; info->converged = converged; }
-    return converged ? LANDAU_OK : LANDAU_NOT_CONVERGED;
+    if (hc->err) return fail(c, hc->err, "step_dg: non-finite residual");
+    if (info) { info->iterations = hc->iterations; info->residual = hc->residual; info->converged = hc->converged; }
+    return hc->converged ? LANDAU_OK : LANDAU_NOT_CONVERGED;
 }
 
 int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, const double* v, const double* w,
