@@ -52,9 +52,10 @@ WORKLOADS = {
     "c3": (3, 32768),
 }
 DEFAULT_WORKLOAD = "c4_2e16"     # >= 1e5 markers: the size north_star's roofline target is quoted on
-# fixed-point iterations one step of each workload takes (measured on the GPU path, used only to
-# scale the oracle's bounded sample in --impl reference, which must not touch the GPU)
-REF_ITERS = {"c0": 9, "c1": 13, "c2": 10, "c3": 6, "c4_2e14": 9, "c4_2e15": 12, "c4_2e16": 16, "c4_2e17": 20}
+# fixed-point iterations one step of each workload takes: the "ms/step (iters)" column of BASELINE.md section 3,
+# measured on the GPU path; used only to scale the oracle's bounded sample in --impl reference (which must not
+# touch the GPU) to the pass-1 / pass-2 mix of the step the GPU arm runs
+REF_ITERS = {"c0": 9, "c1": 13, "c2": 10, "c3": 6, "c4_2e14": 9, "c4_2e15": 18, "c4_2e16": 16, "c4_2e17": 9}
 
 
 def parse():
@@ -68,9 +69,11 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the oracle sample")
     ap.add_argument("--pair-kernel", type=int, default=0)
     ap.add_argument("--entropy-kernel", type=int, default=0)
-    ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi",
-                    help="fixed-point solver of Eq. (24): the paper's Jacobi iteration (default) or Anderson (NEXT-4)")
+    ap.add_argument("--solver", choices=["jacobi", "anderson", "newton"], default="jacobi",
+                    help="solver of Eq. (24): the paper's Jacobi iteration (default), Anderson or Newton-Krylov (NEXT-4)")
     ap.add_argument("--anderson-depth", type=int, default=3)
+    ap.add_argument("--newton-restart", type=int, default=20)
+    ap.add_argument("--no-dg", action="store_true", help="skip the discrete-gradient step block (NEXT-1)")
     return ap.parse_args()
 
 
@@ -187,8 +190,8 @@ def config_dict(args, wl, iters=None):
          "l2": "inputs re-packed every step; pass-2 working set is L2-resident by design (56 B/marker); "
                "compute-bound path, cache state does not change the timing",
          "parallelism": "replicas only" if args.gpus > 1 else "single GPU",
-         "solver": "jacobi (paper)" if getattr(args, "solver", "jacobi") == "jacobi"
-                   else f"anderson depth {args.anderson_depth}"}
+         "solver": {"jacobi": "jacobi (paper)", "anderson": f"anderson depth {args.anderson_depth}",
+                    "newton": f"newton-krylov restart {args.newton_restart}"}[getattr(args, "solver", "jacobi")]}
     if iters is not None:
         d["iterations_per_step"] = iters
     return d
@@ -205,9 +208,18 @@ def aggregate_over_ranks(times, pairs):
     return times.tolist(), pairs.tolist()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/r1_pair_sym_v2_full.md: 475 MB + 401 MB), valid for that workload only
-NCU_TRAFFIC_BYTES = {("c4_2e16", "sym"): 876e6}
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed summary of
+    an `ncu --set full` capture (profiles/ncu_traffic.csv: workload,kernel,dram_read_bytes,dram_write_bytes,source).
+    None when no capture is on file for this workload / kernel."""
+    try:
+        for ln in (ROOT / "profiles" / "ncu_traffic.csv").read_text().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 5 and f[0] == workload and f[1] == kernel:
+                return {"bytes": float(f[2]) + float(f[3]), "source": f[4]}
+    except (OSError, ValueError):
+        pass
+    return None
 
 
 def run_ours(args):
@@ -231,6 +243,8 @@ def run_ours(args):
                  entropy_kernel=args.entropy_kernel)
     if args.solver == "anderson":
         g.set_solver(1, args.anderson_depth)
+    if args.solver == "newton":
+        g.set_solver(2, args.newton_restart)
     dev = torch.device("cuda", local)
     v_d = torch.tensor(wl.v, device=dev); w_d = torch.tensor(wl.w, device=dev)
     s_d = torch.tensor(wl.species_id, device=dev)
@@ -325,9 +339,15 @@ def run_ours(args):
         pair_s = prof["pair_ms"] * 1e-3 / max(prof["pair_launches"], 1)
         achieved = FLOPS_PER_PAIR * N * (N - 1) / pair_s / 1e12
         peak_meas = g.fp64_peak(5) / 1e12
+        peak_dmma = g.fp64_peak_dmma(5) / 1e12
+        traffic = ncu_traffic(args.workload, "sym" if "pair=sym" in g.last_kernels() else "onesided")
+        same_pairs = float((wl.counts().astype(float) ** 2).sum())
+        ent_s = prof["entropy_ms"] * 1e-3 / max(prof["entropy_launches"], 1)
+        ent_flop = 2.0 * wl.n_q ** 3 + 25.0               # n_q^3 FMAs + 1 exponential per same-species pair
         roofline = {"bound": "alu", "kernel": g.last_kernels(), "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12,
                     "unit": "TFLOP/s", "frac": achieved / (FP64_PEAK_NOMINAL / 1e12),
-                    "traffic": NCU_TRAFFIC_BYTES.get((args.workload, "sym" if "pair=sym" in g.last_kernels() else "")),
+                    "traffic": traffic["bytes"] if traffic else None,
+                    "traffic_source": traffic["source"] if traffic else None,
                     "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
                     "algorithmic_bytes": 56.0 * N + 24.0 * N,
                     "peak_source": "nominal FP64 FMA rate 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md); "
@@ -342,7 +362,11 @@ def run_ours(args):
                     "entropy_kernel_ms": prof["entropy_ms"] / max(prof["entropy_launches"], 1),
                     "entropy_same_species_pairs_per_s": float((wl.counts().astype(float) ** 2).sum()) /
                                                         (prof["entropy_ms"] * 1e-3 / max(prof["entropy_launches"], 1)),
-                    "entropy_share_of_step": prof["entropy_ms"] * 1e-3 / t_prof}
+                    "entropy_share_of_step": prof["entropy_ms"] * 1e-3 / t_prof,
+                    "pass1": {"bound": "alu (FP64 pipe: DMMA + the exponentials)", "flops_per_same_species_pair": ent_flop,
+                              "achieved": ent_flop * same_pairs / ent_s / 1e12, "unit": "TFLOP/s",
+                              "peak_measured_dmma": peak_dmma, "frac_of_measured_dmma": ent_flop * same_pairs / ent_s / 1e12 / peak_dmma,
+                              "frac_of_nominal": ent_flop * same_pairs / ent_s / FP64_PEAK_NOMINAL}}
         h2d = int(v_h.numel() * 8 + w_h.numel() * 8 + s_h.numel() * 4)
         d2h = int(out_h.numel() * 8 + 4 * 8 * wl.n_species)
         K0 = float(m0["K"].sum()); K1 = float(m1["K"].sum())
@@ -357,6 +381,51 @@ def run_ours(args):
                 "e2e": {"value": pairs_e2e / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e_max / args.steps},
                 "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        # HBM-streaming rows (a0 pack, a6 moments): whole API calls (several small launches + one synchronisation),
+        # so these are latency figures at this size, quoted against the measured copy bandwidth
+        try:
+            hbm_gbs = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]
+            hbm_src = "MEASURED_PEAKS.json"
+        except Exception:
+            hbm_gbs, hbm_src = 6650.0, "fallback of B200_PROFILING.md"
+        reps = 10
+        e0.record()
+        for _ in range(reps):
+            g.set_markers(v_d, w_d, s_d)
+        e1.record(); torch.cuda.synchronize()
+        t_pack = e0.elapsed_time(e1) * 1e-3 / reps
+        e0.record()
+        for _ in range(reps):
+            g.moments(with_entropy=False)
+        e1.record(); torch.cuda.synchronize()
+        t_mom = e0.elapsed_time(e1) * 1e-3 / reps
+        line["streaming"] = {"hbm_gbs_peak": hbm_gbs, "peak_source": hbm_src,
+                             "pack": {"ms": 1e3 * t_pack, "algorithmic_bytes": 72.0 * N, "GBps": 72.0 * N / t_pack / 1e9,
+                                      "frac": 72.0 * N / t_pack / 1e9 / hbm_gbs},
+                             "moments": {"ms": 1e3 * t_mom, "algorithmic_bytes": 32.0 * N, "GBps": 32.0 * N / t_mom / 1e9,
+                                         "frac": 32.0 * N / t_mom / 1e9 / hbm_gbs},
+                             "note": "whole API calls incl. launches and one host synchronisation; per-kernel times: profiles/"}
+        if not args.no_dg:
+            # one discrete-gradient step (Eqs. 46-49), device driven; every iteration costs two
+            # pass-1 and one pass-2 evaluations.  Its fixed point (G re-evaluated every iteration) is solved with
+            # Anderson mixing of depth 5: the plain Jacobi sweep stops contracting at >= 1e5 markers
+            g.set_solver(1, 5)
+            g.set_markers(v_d, w_d, s_d)
+            dg_tol = 1e-10 if args.workload.startswith("c4") else wl.tol          # reading DG2 (round-off floor of lambda)
+            rc_dg, it_dg, res_dg, conv_dg = g.step_dg(wl.dt, dg_tol, 100)         # sizes every buffer
+            g.set_markers(v_d, w_d, s_d)
+            torch.cuda.synchronize()
+            e0.record()
+            rc_dg, it_dg, res_dg, conv_dg = g.step_dg(wl.dt, dg_tol, 100)
+            e1.record(); torch.cuda.synchronize()
+            line["dg_step"] = {"ms_per_step": e0.elapsed_time(e1), "iterations": it_dg, "residual": res_dg,
+                               "converged": bool(conv_dg), "tol": dg_tol, "pass1_evaluations": 1 + 2 * (it_dg - 1),
+                               "pass2_evaluations": it_dg, "solver": "anderson depth 5"}
+            g.set_solver(0)
+            if args.solver == "anderson":
+                g.set_solver(1, args.anderson_depth)
+            if args.solver == "newton":
+                g.set_solver(2, args.newton_restart)
         if args.solver == "jacobi":
             # SURVEY.md NEXT-4, reported beside the headline (which stays the paper's Jacobi iteration): the same
             # step with the Anderson-accelerated fixed point, device-resident inputs, after both timed regions

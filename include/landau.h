@@ -239,6 +239,8 @@ int landau_profile_read(landau_ctx* ctx, double* pair_ms, int64_t* pair_launches
  * returns the best rate in FLOP/s (2 per DFMA) through *flops_out (HOST). Used by bench.py for the
  * roofline denominator. */
 int landau_fp64_peak(landau_ctx* ctx, int reps, double* flops_out);
+/* Same for the FP64 tensor instructions (DMMA.8x8x4) that pass 1's contraction issues. */
+int landau_fp64_peak_dmma(landau_ctx* ctx, int reps, double* flops_out);
 
 const char* landau_last_error(const landau_ctx* ctx);
 const char* landau_version(void);

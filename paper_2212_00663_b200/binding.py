@@ -27,7 +27,7 @@ SYMBOLS = [
     "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_set_step_graph", "landau_set_substep", "landau_cells_run", "landau_set_cutoff", "landau_cutoff_stats",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
-    "landau_fp64_peak", "landau_last_error",
+    "landau_fp64_peak", "landau_fp64_peak_dmma", "landau_last_error",
     "landau_version",
 ]
 
@@ -104,6 +104,7 @@ def load(build_if_missing: bool = True):
     lib.landau_profile_enable.argtypes = [vp, C.c_int]
     lib.landau_profile_read.argtypes = [vp, hd, C.POINTER(C.c_int64), hd, C.POINTER(C.c_int64)]
     lib.landau_fp64_peak.argtypes = [vp, C.c_int, hd]
+    lib.landau_fp64_peak_dmma.argtypes = [vp, C.c_int, hd]
     lib.landau_last_error.argtypes = [vp]
     lib.landau_last_error.restype = C.c_char_p
     lib.landau_version.restype = C.c_char_p
@@ -332,6 +333,11 @@ class Landau:
         self._check(self._lib.landau_profile_read(self._h, C.byref(pm), C.byref(pn), C.byref(em), C.byref(en)),
                     "landau_profile_read")
         return dict(pair_ms=pm.value, pair_launches=pn.value, entropy_ms=em.value, entropy_launches=en.value)
+
+    def fp64_peak_dmma(self, reps: int = 5) -> float:
+        out = C.c_double(0.0)
+        self._check(self._lib.landau_fp64_peak_dmma(self._h, int(reps), C.byref(out)), "landau_fp64_peak_dmma")
+        return float(out.value)
 
     def fp64_peak(self, reps: int = 5) -> float:
         out = C.c_double(0.0)

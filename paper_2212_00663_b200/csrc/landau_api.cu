@@ -4,6 +4,7 @@
 #include "../../include/landau.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
@@ -146,6 +147,12 @@ int fail(landau_ctx* c, int code, const char* fmt, ...) {
     }
     return code;
 }
+
+// NVTX range around a phase of the path (visible in Nsight timelines; a no-op without a profiler attached)
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 // Every entry point runs on the context's device and leaves the caller's current device as it found it.
 struct DevGuard {
@@ -350,6 +357,7 @@ int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa
 // ---- a0: pack -----------------------------------------------------------------------------
 int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, const int32_t* sid) {
     if (!c) return LANDAU_EINVAL;
+    NvtxRange nvtx("landau:a0 pack");
     if (N < 1 || !v || !w || !sid) return fail(c, LANDAU_EINVAL, "pack: NULL array or N < 1");
     if (N > (int64_t)1 << 24) return fail(c, LANDAU_EINVAL, "pack: N = %lld exceeds 2^24 markers", (long long)N);
     const int S = c->S;
@@ -458,6 +466,7 @@ int mma_groups(int nq) {
 
 // stop != nullptr: every kernel of the pass exits at once when stop->done is set (device-driven loops)
 int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
+    NvtxRange nvtx("landau:a1-a2 pass 1 (entropy gradient)");
     const int nq = c->n_q;
     const size_t M = (size_t)nq * nq * nq;
     const int ttiles = cl.npad_max / ENT_THREADS;
@@ -533,6 +542,7 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
 // ---- a3: pairwise field of source records -> partial fields ---------------------------------
 // Returns the number of partial slices written to c->vpart (to be summed in index order).
 int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
+    NvtxRange nvtx("landau:a3 pass 2 (pairwise Landau sum)");
     int use_sym = 0;
     if (c->pair_kernel == 2 || c->pair_kernel == 0) use_sym = pair_sym_available(c, cl);
     ProfScope prof(c, 0);
@@ -636,6 +646,7 @@ int field_of_cloud(landau_ctx* c, Cloud& cl, double* out) {
 }
 
 int species_sums(landau_ctx* c, Cloud& cl, bool with_entropy, bool with_m4, double* h_out /* S x MOM_OUT */) {
+    NvtxRange nvtx("landau:a6 moments");
     const int nb = cl.npad_max / MOM_THREADS;
     RC(ensure(c, c->blockpart, sizeof(double) * (size_t)std::max(nb * MOM_NQ, 4096)));
     CU(cudaMemsetAsync(c->d_momout, 0, sizeof(double) * LD_MAX_SPECIES * MOM_OUT, c->stream));
@@ -686,6 +697,23 @@ __global__ void fp64_peak_kernel(double* out, int iters, double a, double b) {
     if (s == 123.456) out[0] = s;
 }
 
+// FP64 tensor-pipe peak: dependent-free DMMA.8x8x4 streams (8 accumulator pairs per thread), 2*8*8*4 flop per warp MMA.
+__global__ void fp64_dmma_peak_kernel(double* out, int iters, double a, double b) {
+    double c0[8], c1[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { c0[k] = threadIdx.x + k; c1[k] = threadIdx.x - k; }
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) dmma884(c0[k], c1[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += c0[k] + c1[k];
+    if (s == 123.456) out[0] = s;
+}
 }  // namespace
 
 
@@ -740,6 +768,7 @@ int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b) {
 // step_begin has already done.  cond != 0: the kernel that decides convergence also drives the WHILE node.
 int enqueue_step_iteration(landau_ctx* c, Cloud& cl, const StepBufs& b, double dt, double tol, int max_iter, bool first,
                            cudaGraphConditionalHandle cond) {
+    NvtxRange nvtx("landau:a4-a5 fixed-point iteration");
     cudaStream_t st = c->stream;
     const int npm = b.npm;
     double* rec = cl.sym ? nullptr : cl.recs();
@@ -1344,6 +1373,12 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     const int nub = ceil_div(npm, UPD_THREADS), ndb = ceil_div(npm, DG_THREADS);
     RC(ensure(c, c->blockpart, sizeof(double) * (size_t)step_blockpart_doubles(c, nub)));
     RC(ensure(c, c->dg_part, sizeof(double) * 2 * (size_t)ndb));
+    const bool anderson = c->solver == 1;          // landau_set_solver(1, depth) also accelerates this fixed point
+    if (anderson) RC(ensure(c, c->aa_hist, sizeof(double) * (2 * (size_t)c->aa_depth + 2) * 3 * (size_t)npm));
+    double* aa_dF = (double*)c->aa_hist.p;
+    double* aa_dG = anderson ? aa_dF + (size_t)c->aa_depth * 3 * npm : nullptr;
+    double* aa_fprev = anderson ? aa_dG + (size_t)c->aa_depth * 3 * npm : nullptr;
+    double* aa_gcur = anderson ? aa_fprev + 3 * (size_t)npm : nullptr;
     double* xk = (double*)c->vk.p;
     double* yk = xk + npm;
     double* zk = yk + npm;
@@ -1365,6 +1400,10 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
                                                          c->d_dg, 0);
     CU(cudaMemcpyAsync(xk + 3 * (size_t)npm, cl.w(), sizeof(double) * (size_t)npm, cudaMemcpyDeviceToDevice, st));
     c->launches += 3;
+    if (anderson) {
+        anderson_begin_kernel<<<1, 32, 0, st>>>(c->d_aa, c->aa_depth);
+        c->launches += 1;
+    }
     StepCtrl* hc = (StepCtrl*)((char*)c->h_pin + PIN_CTRL);
     for (int k = 0; k < max_iter; ++k) {
         int nparts = 0;
@@ -1383,18 +1422,31 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
             c->launches += 4;
         }
         RC(pair(c, cl, c->d_ctrl, &nparts));
-        step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
-                                                         (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
-                                                         xk, yk, zk, rec, soa, (double*)c->blockpart.p, 0);
-        c->launches += 1;
+        if (anderson) {
+            anderson_update_kernel<<<nub, UPD_THREADS, 0, st>>>(
+                c->d_tab, cl.L(), c->d_ctrl, c->d_aa, npm, nparts, dt, tol, max_iter, (const double*)c->vpart.p, cl.x(),
+                cl.y(), cl.z(), cl.w(), xk, yk, zk, aa_dF, aa_dG, aa_fprev, aa_gcur, (double*)c->blockpart.p, 0);
+            anderson_mix_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, c->d_aa, npm, cl.x(), cl.y(), cl.z(),
+                                                                     aa_gcur, aa_dG, xk, yk, zk, rec, soa);
+            c->launches += 2;
+        } else {
+            step_update_kernel<<<nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
+                                                             (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
+                                                             xk, yk, zk, rec, soa, (double*)c->blockpart.p, 0);
+            c->launches += 1;
+        }
         if ((k + 1) % DG_CHUNK == 0 && k + 1 < max_iter) {    // one look at the flag per chunk of iterations
             CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
             CU(cudaStreamSynchronize(st));
             if (hc->done) break;
         }
     }
-    step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), xk, yk, zk,
-                                                            (StepRecord*)c->records.p, c->d_cursor);
+    {
+        const double* cm = anderson ? aa_gcur : xk;
+        step_commit_kernel<<<ceil_div(npm, 256), 256, 0, st>>>(cl.L(), c->d_ctrl, npm, cl.x(), cl.y(), cl.z(), cm,
+                                                                cm + npm, cm + 2 * (size_t)npm,
+                                                                (StepRecord*)c->records.p, c->d_cursor);
+    }
     c->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(hc, c->d_ctrl, sizeof(StepCtrl), cudaMemcpyDeviceToHost, st));
@@ -1510,6 +1562,33 @@ int landau_profile_read(landau_ctx* c, double* pair_ms, int64_t* pair_launches, 
     if (pair_launches) *pair_launches = c->prof_n[0];
     if (entropy_ms) *entropy_ms = c->prof_ms[1];
     if (entropy_launches) *entropy_launches = c->prof_n[1];
+    return 0;
+}
+
+int landau_fp64_peak_dmma(landau_ctx* c, int reps, double* flops_out) {
+    if (!c || !flops_out || reps < 1) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
+    RC(ensure(c, c->V, 1024));
+    const int blocks = c->sm_count * 4, threads = 256, iters = 4096;
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int r = 0; r < reps + 1; ++r) {
+        CU(cudaEventRecord(e0, c->stream));
+        fp64_dmma_peak_kernel<<<blocks, threads, 0, c->stream>>>((double*)c->V.p, iters, 1e-3, 1e-3);
+        CU(cudaEventRecord(e1, c->stream));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        // per warp and MMA: m8 n8 k4 -> 2*8*8*4 = 512 flop; 32 MMAs per loop iteration
+        const double fl = 512.0 * 32.0 * (double)iters * blocks * (threads / 32) / (ms * 1e-3);
+        if (r > 0 && fl > best) best = fl;
+    }
+    c->launches += reps + 1;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *flops_out = best;
     return 0;
 }
 

@@ -452,6 +452,29 @@ def test_dg_step_matches_oracle_and_conserves(B, oracle_mod, cfg, n, dt, tol, st
     np.testing.assert_allclose(m1["S_eps"], o.moments()["S_eps"], rtol=1e-10, atol=1e-12)
 
 
+@pytest.mark.parametrize("cfg,n,dt,tol,state_tol", [(0, 256, 0.01, 1e-12, 1e-11), (4, 300, 1e-3, 1e-10, 1e-8)])
+def test_dg_step_with_anderson_mixing_matches_oracle(B, oracle_mod, cfg, n, dt, tol, state_tol):
+    """landau_set_solver(1, depth) also accelerates the fixed point of the discrete-gradient step (needed at >= 1e5
+    markers, where its plain Jacobi sweep stops contracting): same Eq. (46), so the converged step equals the
+    oracle's O4b step, conserves momentum / energy and does not decrease S_eps."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_solver(1, 5)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments()
+    rc, it, res, conv = g.step_dg(dt, tol, 100)
+    rco, ito, reso, convo = o.step_dg(dt, tol, 100)
+    assert rc == 0 and conv and rco == 0 and convo and it <= ito + 1, (it, res, ito, reso)
+    assert_field_close(g.get_markers().cpu().numpy(), o.get_markers(), wl.species_id, wl.n_species, tol=state_tol,
+                       what="DG state (Anderson)")
+    m1 = g.moments()
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= TOL_DRIFT * m0["K"].sum()
+    assert m1["S_eps"].sum() >= m0["S_eps"].sum() - 1e-13 * abs(m0["S_eps"].sum())
+
+
 # ------------------------------------------------------------------------------------ NEXT-4: Anderson solver
 @pytest.mark.parametrize("cfg,n,dt", [(0, 256, 0.01), (4, 384, 1e-3), (1, 1024, 0.02), (3, 9000, 0.01)])
 @pytest.mark.parametrize("depth", [1, 3, 5])
