@@ -194,10 +194,12 @@ int landau_step_dg(landau_ctx* ctx, double dt, double tol, int max_iter, landau_
  * cell_offset is a HOST array of n_cells + 1 entries).  Every cell is advanced by n_steps steps of Eq. (24)
  * (same Jacobi fixed point, residual, tolerance and readings as landau_step) by ONE kernel launch: one
  * persistent thread block per cell with the cell's state in shared memory.  v_out (DEVICE, same layout, may
- * alias v) receives the new velocities in caller order.  Limits: <= 1024 markers per cell, n_q <= 4.
+ * alias v) receives the new velocities in caller order.  Limit: markers per cell <= 1024 (n_q <= 5), 984 / 890 /
+ * 812 at n_q = 6 / 7 / 8 (the cell's state lives in the 227 KB of shared memory of one thread block).  A cell too
+ * wide for the factorised pass 1 takes the literal form, as the single-cell path does.
  * info (HOST, n_cells entries, may be NULL): per-cell status (0 ok, 1 = some step hit max_iter, < 0 = the
- * cell was rejected and copied through unchanged: -1 invalid markers, -4 non-finite, -5 too wide for the
- * factorised pass 1), iterations summed over the steps, the largest per-step count, and the last residual.
+ * cell was rejected and copied through unchanged: -1 invalid markers, -4 non-finite), iterations summed over the
+ * steps, the largest per-step count, and the last residual.
  * Returns 0, 1 (some cell did not converge) or the most negative cell status. */
 typedef struct {
     int status;

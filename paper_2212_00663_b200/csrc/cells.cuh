@@ -11,9 +11,12 @@
 //   -> write back in caller order.
 // No global-memory traffic, no kernel launch and no host synchronisation inside a step.  Cells are dealt to the
 // CTAs through an atomic counter (cells are independent, so results do not depend on the assignment).
-// Limits: markers per cell <= CELLS_CAP (shared memory), n_q <= 4; a cell that is too wide for the factorised
-// pass 1 (reading N3) reports LANDAU_ERANGE and is left unchanged.  Arithmetic, stopping rule and readings are
-// those of the single-cell path (S4, S5, S7, S8); tests compare every cell with the oracle.
+// Limits: markers per cell <= CellsCfg<NQ>::max_cap() (shared memory: 1024 for n_q <= 5, 984 / 890 / 812 for
+// n_q = 6 / 7 / 8).  A cell that is too wide for the factorised pass 1 (reading N3) takes the literal-separable form
+// of Eq. (22) (3 n_q exponentials per pair, every factor <= 1), as the single-cell path does.  n_q > 4: the n_q^3 node
+// sums of a target are accumulated in slices of x-node indices (registers), the per-pair exponential recomputed per
+// slice.  Arithmetic, stopping rule and readings are those of the single-cell path (S4, S5, S7, S8); tests compare
+// every cell with the oracle.
 #pragma once
 #include "common.cuh"
 #include "entropy.cuh"
@@ -38,8 +41,16 @@ template <int NQ>
 struct CellsCfg {
     // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / ux uy uz (pass 2)
     static constexpr int DPM = 10 + 3 * NQ;
+    // x-node indices per register slice of the node sums: NI * NQ^2 <= 64 accumulators
+    static constexpr int NI = NQ <= 4 ? NQ : 1;
+    static_assert(NQ % NI == 0, "slices must tile the x-node indices");
     static size_t smem(int cap) {
         return sizeof(double) * ((size_t)DPM * cap + 64 + 32 + 3 * CELLS_THREADS) + sizeof(int) * (size_t)cap;
+    }
+    static int max_cap() {                  // largest even cap whose state fits the 227 KB of a CTA
+        int cap = CELLS_CAP;
+        while (cap > 32 && smem(cap) > 227 * 1024 - 1024) cap -= 2;
+        return cap;
     }
 };
 
@@ -58,7 +69,7 @@ __device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_re
 // Pass 1 of one target against the sources [o0, o1) of its species, node slice i in [i0, i0 + NI): the partial
 // sums  sum_{ijl} a_i a_j a_l k (1 + ln rho)  of Eq. (22) (without the prefactor).  NI = NQ is the whole gradient;
 // NI < NQ lets several threads share one target (small cells), each recomputing the exponential.
-template <int NQ, int NI>
+template <int NQ, int NI, bool LITERAL>
 __device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, double px, double py, double pz,
                                                    const double* __restrict__ xk, const double* __restrict__ yk,
                                                    const double* __restrict__ zk, const double* __restrict__ ww,
@@ -75,15 +86,35 @@ __device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, doubl
 #pragma unroll 2
     for (int q = o0; q < o1; ++q) {
         const double dx = px - xk[q], dy = py - yk[q], dz = pz - zk[q];
-        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        const double c = ww[q] * exp_neg_tab(r2, s_e2);
-        const double* t = tab + (size_t)q * 3 * NQ;
-        double ty[NQ], tz[NQ];
+        double c, tx[NI], ty[NQ], tz[NQ];
+        if (LITERAL) {
+            // exp(-|k + d|^2) = prod_axis exp(-(k_a + d_a)^2): every factor <= 1 (wide cells, reading N3)
+            c = ww[q];
 #pragma unroll
-        for (int j = 0; j < NQ; ++j) { ty[j] = t[NQ + j]; tz[j] = t[2 * NQ + j]; }
+            for (int i = 0; i < NI; ++i) {
+                double ki = kn[0];
+#pragma unroll
+                for (int m = 1; m < NQ; ++m) if (m == i0 + i) ki = kn[m];
+                const double a = ki + dx;
+                tx[i] = exp_neg_tab(a * a, s_e2);
+            }
+#pragma unroll
+            for (int j = 0; j < NQ; ++j) {
+                const double a = kn[j] + dy, b = kn[j] + dz;
+                ty[j] = exp_neg_tab(a * a, s_e2); tz[j] = exp_neg_tab(b * b, s_e2);
+            }
+        } else {
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            c = ww[q] * exp_neg_tab(r2, s_e2);
+            const double* t = tab + (size_t)q * 3 * NQ;
+#pragma unroll
+            for (int i = 0; i < NI; ++i) tx[i] = t[i0 + i];
+#pragma unroll
+            for (int j = 0; j < NQ; ++j) { ty[j] = t[NQ + j]; tz[j] = t[2 * NQ + j]; }
+        }
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
-            const double cx = c * t[i0 + i];
+            const double cx = c * tx[i];
 #pragma unroll
             for (int j = 0; j < NQ; ++j) {
                 const double cxy = cx * ty[j];
@@ -102,8 +133,8 @@ __device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, doubl
         for (int j = 0; j < NQ; ++j)
 #pragma unroll
             for (int l = 0; l < NQ; ++l) {
-                const double lnrho = lognorm + log(acc[i][j][l])
-                                     - ((ki * ki + kn[j] * kn[j] + kn[l] * kn[l]) + 2.0 * (ki * px + kn[j] * py + kn[l] * pz));
+                double lnrho = lognorm + log(acc[i][j][l]);
+                if (!LITERAL) lnrho -= (ki * ki + kn[j] * kn[j] + kn[l] * kn[l]) + 2.0 * (ki * px + kn[j] * py + kn[l] * pz);
                 const double t = gi * ga[j] * ga[l] * (1.0 + lnrho);
                 gx = fma(t, ki, gx); gy = fma(t, kn[j], gy); gz = fma(t, kn[l], gz);
             }
@@ -263,16 +294,19 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     cen[d] = 0.5 * a + 0.5 * b;
                     hw = fmax(hw, 0.5 * b - 0.5 * a);
                 }
-                if (!(6.0 * kmax * hw * inv <= FACT_EXP_LIMIT)) { if (tid == 0) s_status = -5; break; }
+                // a cell too wide for the factorised form (reading N3) takes the literal-separable one
+                const bool literal = !(6.0 * kmax * hw * inv <= FACT_EXP_LIMIT);
                 // scaled coordinates (alias of xk..zk) and the per-marker exponential tables
                 for (int p = o0 + tid; p < o1; p += CELLS_THREADS) {
                     const double a = (xn[p] - cen[0]) * inv, b = (yn[p] - cen[1]) * inv, c = (zn[p] - cen[2]) * inv;
                     xk[p] = a; yk[p] = b; zk[p] = c;
-                    double* t = tab + (size_t)p * 3 * NQ;
+                    if (!literal) {
+                        double* t = tab + (size_t)p * 3 * NQ;
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) {
-                        const double k2 = 2.0 * kn[i];
-                        t[i] = exp(k2 * a); t[NQ + i] = exp(k2 * b); t[2 * NQ + i] = exp(k2 * c);
+                        for (int i = 0; i < NQ; ++i) {
+                            const double k2 = 2.0 * kn[i];
+                            t[i] = exp(k2 * a); t[NQ + i] = exp(k2 * b); t[2 * NQ + i] = exp(k2 * c);
+                        }
                     }
                 }
                 __syncthreads();
@@ -285,12 +319,21 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     const int p = min(pt, o1 - 1);
                     const double px = xk[p], py = yk[p], pz = zk[p];
                     double gx, gy, gz;
-                    if (GF == 2)
-                        cells_pass1_target<NQ, (NQ >= 2 ? NQ / 2 : 1)>(part * (NQ / 2), o0, o1, px, py, pz, xk, yk, zk, ww,
-                                                                       tab, s_e2, kn, ga, lognorm, gx, gy, gz);
-                    else
-                        cells_pass1_target<NQ, (NQ >= 4 ? NQ / 4 : 1)>(part * (NQ / 4), o0, o1, px, py, pz, xk, yk, zk, ww,
-                                                                       tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                    if (GF == 2) {
+                        if (literal)
+                            cells_pass1_target<NQ, (NQ >= 2 ? NQ / 2 : 1), true>(part * (NQ / 2), o0, o1, px, py, pz, xk, yk, zk,
+                                                                                 ww, tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                        else
+                            cells_pass1_target<NQ, (NQ >= 2 ? NQ / 2 : 1), false>(part * (NQ / 2), o0, o1, px, py, pz, xk, yk, zk,
+                                                                                  ww, tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                    } else {
+                        if (literal)
+                            cells_pass1_target<NQ, (NQ >= 4 ? NQ / 4 : 1), true>(part * (NQ / 4), o0, o1, px, py, pz, xk, yk, zk,
+                                                                                 ww, tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                        else
+                            cells_pass1_target<NQ, (NQ >= 4 ? NQ / 4 : 1), false>(part * (NQ / 4), o0, o1, px, py, pz, xk, yk, zk,
+                                                                                  ww, tab, s_e2, kn, ga, lognorm, gx, gy, gz);
+                    }
                     s_part[(part * 3 + 0) * TPG + tg] = gx;
                     s_part[(part * 3 + 1) * TPG + tg] = gy;
                     s_part[(part * 3 + 2) * TPG + tg] = gz;
@@ -310,9 +353,19 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         const int pt = r0 + tid;
                         const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
                         const double px = xk[p], py = yk[p], pz = zk[p];
-                        double gx, gy, gz;
-                        cells_pass1_target<NQ, NQ>(0, o0, o1, px, py, pz, xk, yk, zk, ww, tab, s_e2, kn, ga, lognorm, gx,
-                                                   gy, gz);
+                        double gx = 0.0, gy = 0.0, gz = 0.0;
+                        constexpr int NI = CellsCfg<NQ>::NI;
+#pragma unroll 1
+                        for (int i0 = 0; i0 < NQ; i0 += NI) {          // n_q > 4: slices of x-node indices
+                            double sx, sy, sz;
+                            if (literal)
+                                cells_pass1_target<NQ, NI, true>(i0, o0, o1, px, py, pz, xk, yk, zk, ww, tab, s_e2, kn, ga,
+                                                                 lognorm, sx, sy, sz);
+                            else
+                                cells_pass1_target<NQ, NI, false>(i0, o0, o1, px, py, pz, xk, yk, zk, ww, tab, s_e2, kn, ga,
+                                                                  lognorm, sx, sy, sz);
+                            gx += sx; gy += sy; gz += sz;
+                        }
                         gx *= pref; gy *= pref; gz *= pref;
                         if (pt < o1) {
                             if (!(isfinite(gx) && isfinite(gy) && isfinite(gz))) s_status = -4;

@@ -1472,13 +1472,21 @@ int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, con
         return fail(c, LANDAU_EINVAL, "cells_run: NULL array or n_cells < 1");
     if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
         return fail(c, LANDAU_EINVAL, "cells_run: need n_steps >= 1, max_iter >= 1, dt > 0, tol >= 0");
-    if (c->n_q > 4) return fail(c, LANDAU_EINVAL, "cells_run: n_q <= 4 only (n_q = %d)", c->n_q);
+    int cap_max = CELLS_CAP;
+    switch (c->n_q) {
+        case 5: cap_max = CellsCfg<5>::max_cap(); break;
+        case 6: cap_max = CellsCfg<6>::max_cap(); break;
+        case 7: cap_max = CellsCfg<7>::max_cap(); break;
+        case 8: cap_max = CellsCfg<8>::max_cap(); break;
+        default: break;
+    }
     int cap = 0;
     for (int k = 0; k < n_cells; ++k) {
         const int64_t nk = cell_offset[k + 1] - cell_offset[k];
         if (nk < 0) return fail(c, LANDAU_EINVAL, "cells_run: cell_offset must be non-decreasing");
-        if (nk > CELLS_CAP)
-            return fail(c, LANDAU_EINVAL, "cells_run: cell %d has %lld markers, limit %d per cell", k, (long long)nk, CELLS_CAP);
+        if (nk > cap_max)
+            return fail(c, LANDAU_EINVAL, "cells_run: cell %d has %lld markers, limit %d per cell at n_q = %d", k,
+                        (long long)nk, cap_max, c->n_q);
         cap = std::max(cap, (int)nk);
     }
     cap = std::max(32, (cap + 1) & ~1);
@@ -1491,7 +1499,11 @@ int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, con
     switch (c->n_q) {
         case 2: RC((launch_cells<2>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
         case 3: RC((launch_cells<3>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
-        default: RC((launch_cells<4>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        case 4: RC((launch_cells<4>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        case 5: RC((launch_cells<5>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        case 6: RC((launch_cells<6>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        case 7: RC((launch_cells<7>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
+        default: RC((launch_cells<8>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter))); break;
     }
     CU(cudaGetLastError());
     std::vector<CellRecord> h(n_cells);

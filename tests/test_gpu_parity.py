@@ -735,7 +735,7 @@ def test_cells_run_matches_oracle_per_cell(B, oracle_mod):
         assert abs(K1 - K0) <= TOL_DRIFT * K0
 
 
-def test_cells_run_rejects_bad_cells_and_passes_them_through(B):
+def test_cells_run_rejects_bad_cells_and_passes_them_through(B, oracle_mod):
     wl = W.make(0, n_per_species=50, shuffled=True)
     v = np.concatenate([wl.v, wl.v, wl.v]); w = np.concatenate([wl.w, wl.w, wl.w]).copy()
     sid = np.concatenate([wl.species_id] * 3)
@@ -745,13 +745,43 @@ def test_cells_run_rejects_bad_cells_and_passes_them_through(B):
     g = B.Landau(wl.mass, wl.charge, wl.eps)
     rc, vout, info = g.cells_run(off, v, w, sid, 1, wl.dt, 1e-12, 50, strict=False)
     vout = vout.cpu().numpy()
-    assert rc == B.ERANGE and list(info["status"]) == [0, B.EINVAL, B.ERANGE]
-    assert np.array_equal(vout[100:300], v[100:300]) and not np.array_equal(vout[:100], v[:100])
+    assert rc == B.EINVAL and list(info["status"]) == [0, B.EINVAL, 0]
+    assert np.array_equal(vout[100:200], v[100:200]) and not np.array_equal(vout[:100], v[:100])
+    # the wide cell takes the literal form of pass 1 (as the single-cell path does) and equals the oracle's step
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps)
+    o.set_markers(v[200:300], w[200:300], sid[200:300])
+    assert o.step(wl.dt, 1e-12, 50)[0] == 0
+    assert rel_l2(vout[200:300], o.get_markers()) <= 1e-11
+    assert rel_l2(vout[200:300] - v[200:300], o.get_markers() - v[200:300]) <= 1e-8
     with pytest.raises(B.LandauError):
         g.cells_run(off, v, w, sid, 1, wl.dt)
     with pytest.raises(B.LandauError):                           # more than 1024 markers in a cell
         big = W.make(0, n_per_species=600)
         g.cells_run(np.array([0, 1200]), big.v, big.w, big.species_id, 1, 0.01)
+
+
+@pytest.mark.parametrize("n_q", [5, 6, 8])
+def test_cells_run_higher_quadrature_orders_match_oracle(B, oracle_mod, n_q):
+    """landau_cells_run at n_q = 5, 6, 8 (node sums accumulated in register slices): every cell of a ragged batch,
+    one of them wide enough for the literal fallback, equals the oracle's steps on that cell alone."""
+    cells = [W.make(0, n_per_species=n, seed=40 + n, shuffled=True) for n in (23, 150, 330)]
+    v = np.concatenate([c.v for c in cells]); w = np.concatenate([c.w for c in cells])
+    sid = np.concatenate([c.species_id for c in cells])
+    off = np.cumsum([0] + [c.n_markers for c in cells]).astype(np.int64)
+    v[off[1] + 7] = np.array([310.0, -2.0, 5.0]) * np.sqrt(cells[1].eps[sid[off[1] + 7]])   # a wide cell
+    wl = cells[0]
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=n_q)
+    rc, vout, info = g.cells_run(off, v, w, sid, 2, wl.dt, 1e-12, 60)
+    vout = vout.cpu().numpy()
+    assert rc == 0 and list(info["status"]) == [0, 0, 0]
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=n_q)
+    for k in range(3):
+        a, b = off[k], off[k + 1]
+        o.set_markers(v[a:b], w[a:b], sid[a:b])
+        for _ in range(2):
+            assert o.step(wl.dt, 1e-12, 60)[0] == 0
+        assert rel_l2(vout[a:b], o.get_markers()) <= 1e-11, (n_q, k)
+        assert rel_l2(vout[a:b] - v[a:b], o.get_markers() - v[a:b]) <= 1e-8, (n_q, k)
 
 
 def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
