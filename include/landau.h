@@ -122,10 +122,13 @@ int landau_get_markers_host(landau_ctx* ctx, double* v_out /* host */);
 int landau_step(landau_ctx* ctx, double dt, double tol, int max_iter, landau_step_info* info);
 
 /* velocity-space dimension.  3 (default), or 2 = the paper's own 2-V setting (PAPER.md:110,
- * 180): markers must be given with v_z = 0; the z-component of the entropy gradient, which cancels
- * analytically by the antisymmetry of the Gauss-Hermite knots, is then stored as an exact zero, so that
- * v_z = 0 is preserved exactly by every field evaluation and step (in 3-V arithmetic a round-off-sized G_z
- * would seed the physical relaxation into v_z).  x/y results equal the 2-V Eqs. (22)-(24) (reading D1). */
+ * 180): markers must be given with v_z = 0 (v_z is ignored by the passes and left untouched by the steps).  The
+ * passes then run native 2-V kernels: pass 1 sums the n_q^2 planar nodes (k_i, k_j, 0) -- the z-quadrature of
+ * Eq. (22) is done in closed form, G_z is an exact zero -- and pass 2 does the two-component arithmetic of Eq. (23)
+ * (22 instead of 30 FP64 instructions per unordered pair).  x/y results are the paper's 2-V Eqs. (22)-(24) and equal
+ * what the 3-V kernels give on v_z = 0 data (reading D1; pass 2 bit for bit, pass 1 to round-off), and S_eps is the
+ * 3-V value of that data, so 2-V and 3-V runs report comparable entropies.  (Clouds too wide for the factorised pass 1
+ * and landau_cells_run use the 3-V arithmetic with G_z stored as zero.) */
 int landau_set_dimension(landau_ctx* ctx, int dim);
 
 /* SURVEY.md NEXT-4 (second half): Gaussian cutoff of pass 1.  on = 1 (default): a tile of 64 source markers is not
@@ -172,6 +175,16 @@ int landau_set_substep(landau_ctx* ctx, int max_halvings);
  * between v^n and the converged v^{n+1} differ.  `iterations` counts pass-2 evaluations for every solver.  All
  * three are device driven (no host synchronisation inside a step). */
 int landau_set_solver(landau_ctx* ctx, int solver, int depth);
+
+/* Mixed-precision implicit step ("try FP32 pass-2 evaluations for the early iterations").  f32_until > 0:
+ * while the Jacobi iterates of Eq. (24) still move by more than f32_until (the residual r_k of the last iteration),
+ * pass 2 is evaluated by the FP32 flavour of the symmetric kernel (the BASELINE config-4 field variant: ~3e-6 relative
+ * error in V, i.e. ~dt * 3e-6 in the iterate); below it, and always for the iteration that ends the step, by the FP64
+ * kernel.  The fixed point, the stopping rule (r_k <= tol on an FP64 evaluation) and therefore the converged state and
+ * its conservation properties are those of the FP64 step; only the early iterates differ.  A sensible value is 1e-7
+ * (FP32 noise in the iterate is ~3e-9 at dt = 1e-3).  The decision is taken on the device, per iteration.  Applies
+ * to the Jacobi solver on clouds of >= 16384 markers in 3-V; ignored otherwise.  0 (default) = off. */
+int landau_set_mixed_precision(landau_ctx* ctx, double f32_until);
 
 /* n_steps consecutive steps with one host synchronisation at the end; info (optional, HOST,
  * n_steps entries) receives each step's record.  Returns 1 if any step did not converge. */

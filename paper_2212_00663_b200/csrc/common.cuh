@@ -55,7 +55,8 @@ struct StepCtrl {
     double residual;
     unsigned int ticket; // last-block-done counter of the residual reduction
     int hold;            // 1: step_commit keeps v^n when the step did not converge (adaptive sub-stepping)
-    int _r[2];
+    int use_f32;         // mixed-precision step (landau_set_mixed_precision): 1 = the next pass 2 runs in FP32
+    int _r;
 };
 
 struct StepRecord {      // mirrors landau_step_info (host struct) field by field

@@ -185,11 +185,16 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
 // Node sums -> G_p (unscaled: (1/w_p) dS_eps/dv_p) and s_p.  fact_mode: 0 = the node sums are the
 // literal kernel's; 1 = they are the factorised kernel's if fact_usable() (automatic choice), else the
 // literal kernel's; 2 = factorised forced (a cloud that is too wide raises LANDAU_ERANGE = -5).
+// planar = 1: the factorised kernel summed only the n_q^2 nodes (k_i, k_j, 0) of the 2-V setting (v_z = 0, where
+// the node sum does not depend on k_l beyond the factor exp(-k_l^2)); the z-quadrature is then done in closed form:
+//   sum_l a_l k_l [1 + ln rho_ijl] = 0,   sum_l a_l [1 + ln rho_ijl] = (sum_l a_l)(1 + ln rho_ij0) - sum_l a_l k_l^2,
+// the last term dropping out of G by the antisymmetry of the knots in i and j -- which gives the paper's 2-V Eq. (22)
+// exactly and the same s_p as the n_q^3-node evaluation.
 __global__ void __launch_bounds__(128)
 entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, int npad_max,
                         int nchunks, const int* __restrict__ perm, const double* __restrict__ part,
                         const double* __restrict__ px, const double* __restrict__ py,
-                        const double* __restrict__ pz, int fact_mode,
+                        const double* __restrict__ pz, int fact_mode, int planar,
                         double* __restrict__ Gx, double* __restrict__ Gy, double* __restrict__ Gz,
                         double* __restrict__ snode, const StepCtrl* __restrict__ stop) {
     if (stop && stop->done) return;
@@ -214,6 +219,25 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
         cz = (pz[p] - L->center[s][2]) * inv;
     }
     double gx = 0.0, gy = 0.0, gz = 0.0, sn = 0.0;
+    if (planar && factorised) {
+        double az = 0.0, azk2 = 0.0, axy = 0.0;
+        for (int l = 0; l < nq; ++l) { az += T->gw[l]; azk2 = fma(T->gw[l], T->knot[l] * T->knot[l], azk2); }
+        const size_t M2 = (size_t)nq * nq;
+        for (int i = 0; i < nq; ++i)
+            for (int j = 0; j < nq; ++j) {
+                const size_t node = (size_t)i * nq + j;
+                double a = 0.0;
+                for (int c = 0; c < nchunks; ++c) a += part[((size_t)c * M2 + node) * (size_t)npad_max + p];
+                const double ki = T->knot[i], kj = T->knot[j];
+                const double lnrho = lognorm + log(a) - ((ki * ki + kj * kj) + 2.0 * (ki * cx + kj * cy));
+                const double aa = T->gw[i] * T->gw[j];
+                const double t = aa * az * (1.0 + lnrho);
+                gx = fma(t, ki, gx); gy = fma(t, kj, gy);
+                sn = fma(aa * az, lnrho, sn);
+                axy += aa;
+            }
+        sn -= axy * azk2;
+    } else
     for (int i = 0; i < nq; ++i)
         for (int j = 0; j < nq; ++j)
             for (int l = 0; l < nq; ++l) {

@@ -32,9 +32,12 @@ constexpr int MMA_MT = 4;          // 8-target blocks per warp
 constexpr int MMA_ROW = 68;        // doubles per product-table row
 constexpr int MMA_LCAP = 1024;     // source tiles per segment of the active-tile list (Gaussian cutoff)
 
-template <int NQ>
+// NZ = NQ: the 3-V tensor grid of n_q^3 nodes.  NZ = 1: the paper's own 2-V setting (landau_set_dimension(2), v_z = 0):
+// the z-factor of every node is exp(0) = 1 and the z-quadrature is done in closed form by entropy_finalize_kernel, so
+// only the n_q^2 nodes (k_i, k_j, 0) are summed -- a quarter of the tensor work at n_q = 4.
+template <int NQ, int NZ = NQ>
 struct MmaCfg {
-    static constexpr int M = NQ * NQ * NQ;
+    static constexpr int M = NQ * NQ * NZ;
     static constexpr int NB = (M + 7) / 8;                          // 8-node blocks
     static constexpr int NBG = NB <= 8 ? NB : (NQ == 6 ? 7 : 8);    // blocks per node group (gridDim.z)
     static constexpr int GROUPS = (NB + NBG - 1) / NBG;
@@ -75,15 +78,15 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-// grid = (target tiles of 128 slots, source chunks, MmaCfg<NQ>::GROUPS node groups).
-template <int NQ>
+// grid = (target tiles of 128 slots, source chunks, MmaCfg<NQ, NZ>::GROUPS node groups).
+template <int NQ, int NZ = NQ>
 __global__ void __launch_bounds__(MMA_THREADS, 2)
 entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
                    const double* __restrict__ rec, const TileBox* __restrict__ box,
                    unsigned long long* __restrict__ cutstats, double* __restrict__ part,
                    const StepCtrl* __restrict__ stop) {
     if (stop && stop->done) return;
-    using C = MmaCfg<NQ>;
+    using C = MmaCfg<NQ, NZ>;
     constexpr int REC = C::REC, MT = MMA_MT, NBG = C::NBG, NL = C::NL, M = C::M;
     const int slot0 = blockIdx.x * MMA_THREADS;
     if (slot0 >= L->npad) return;
@@ -129,15 +132,15 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     const int be = tid & 63, bq = tid >> 6;
     const int bnd = node0 + be;
     const bool bvalid = be < NL && bnd < M;
-    const int oi = 4 + (bvalid ? bnd / (NQ * NQ) : 0), oj = 4 + NQ + (bvalid ? (bnd / NQ) % NQ : 0),
-              ol = 4 + 2 * NQ + (bvalid ? bnd % NQ : 0);
+    const int oi = 4 + (bvalid ? bnd / (NQ * NZ) : 0), oj = 4 + NQ + (bvalid ? (bnd / NZ) % NQ : 0),
+              ol = 4 + 2 * NQ + (bvalid ? bnd % NZ : 0);
     auto build = [&](int k) {                                        // records of tile k -> product table k & 1
         mbar_wait(&s_bar[k & 1], (uint32_t)(k >> 1) & 1u);
         const double* r = s_rec + (size_t)(k & 1) * MMA_TILE * REC + bq * REC;
         double* row = s_prod + ((size_t)(k & 1) * MMA_TILE + bq) * MMA_ROW;
 #pragma unroll 8
         for (int qi = 0; qi < MMA_TILE / 2; ++qi) {
-            const double v = r[oi] * r[oj] * r[ol];
+            const double v = NZ == 1 ? r[oi] * r[oj] : r[oi] * r[oj] * r[ol];
             if (be < NL) row[be] = bvalid ? v : 0.0;
             if (be < 4) row[64 + be] = r[be];
             r += 2 * REC;

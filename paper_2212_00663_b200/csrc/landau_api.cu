@@ -87,9 +87,11 @@ struct landau_ctx {
     size_t attr_cellcount = 0;
     unsigned long long* d_cutstats = nullptr;   // pass 1 Gaussian cutoff: {source tiles considered, skipped}
     int cutoff_on = 1;                          // landau_set_cutoff
+    double mixed_until = 0.0;                   // landau_set_mixed_precision: FP32 pass 2 while the residual exceeds it
     Buf sym_acc, sym_tpart, sym_ticket;   // symmetric pair kernel: in-place source sums, target segments, unit tickets
     // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
-    bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {};
+    bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {}, attr_mma2v[LD_MAX_NQ + 1] = {};
+    bool attr_sym64_2v = false;
     size_t attr_cells[LD_MAX_NQ + 1] = {};
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
@@ -107,7 +109,7 @@ struct landau_ctx {
     struct StepGraph {
         cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
         unsigned long long gen = 0; int64_t N = 0; int npm = 0, max_iter = 0, fixed_nodes = 0, body_nodes = 0;
-        double dt = 0.0, tol = 0.0; int ek = 0, pk = 0, solver = 0, depth = 0; bool failed = false;
+        double dt = 0.0, tol = 0.0, mixed = 0.0; int ek = 0, pk = 0, solver = 0, depth = 0; bool failed = false;
     } sg;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
@@ -321,6 +323,10 @@ int npad_upper(int64_t N, int S, int pad) {
 
 // ---- optimised kernels -----------------------------------------------------------------------
 int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; return cl.sym; }
+// mixed-precision implicit step: Jacobi solver, 3-V, symmetric kernel (>= 16384 markers)
+bool mixed_step_active(const landau_ctx* c, const Cloud& cl) {
+    return c->mixed_until > 0.0 && c->solver == 0 && c->dim == 3 && cl.sym && c->precision == 0;
+}
 // Buffers of the symmetric kernel's output path (pair_sym.cuh): O(N), whatever the grid.
 int ensure_sym_buffers(landau_ctx* c, const Cloud& cl, int G) {
     const size_t npm = (size_t)cl.npad_max;
@@ -331,24 +337,27 @@ int ensure_sym_buffers(landau_ctx* c, const Cloud& cl, int G) {
     return 0;
 }
 
-template <typename F>
-int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa, bool& attr_done, int* nparts) {
+template <typename F, int DIM = 3>
+int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa, bool& attr_done, int* nparts,
+                    int only_if_f32 = -1) {
     using Cfg = SymCfg<SYM_W, SYM_RT, SYM_RS, F>;
     const int G = c->sm_count;                 // persistent grid, 1 CTA per SM: all CTAs co-resident (ticket waits)
     RC(ensure_sym_buffers(c, cl, G));
-    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, F>;
+    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, F, DIM>;
     if (!attr_done) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         attr_done = true;
     }
     const int npm = cl.npad_max;
     sym_reset_kernel<<<c->sm_count, 256, 0, c->stream>>>(ctrl, (double*)c->sym_acc.p, 3 * (size_t)npm,
-                                                          (int*)c->sym_ticket.p, npm / SymL::BS + 1);
+                                                          (int*)c->sym_ticket.p, npm / SymL::BS + 1, only_if_f32);
     kern<<<G, Cfg::THREADS, Cfg::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, npm, soa, (double*)c->sym_acc.p,
-                                                    (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err);
+                                                    (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err,
+                                                    only_if_f32);
     sym_combine_kernel<<<ceil_div(npm, 256), 256, 0, c->stream>>>(cl.L(), ctrl, npm, G, SymL::BT, SymL::BS,
                                                                    (const double*)c->sym_acc.p,
-                                                                   (const double*)c->sym_tpart.p, (double*)c->vpart.p);
+                                                                   (const double*)c->sym_tpart.p, (double*)c->vpart.p,
+                                                                   only_if_f32);
     c->launches += 3;
     *nparts = 1;
     return 0;
@@ -438,22 +447,29 @@ int launch_entropy_fact(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* s
     return 0;
 }
 
-template <int NQ>
-int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
-    using M = MmaCfg<NQ>;
+template <int NQ, int NZ>
+int launch_entropy_mma_nz(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
+    using M = MmaCfg<NQ, NZ>;
     RC(ensure(c, c->facttab, sizeof(double) * M::REC * (size_t)cl.npad_max));
     entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p, stop);
-    auto kern = entropy_mma_kernel<NQ>;
-    if (!c->attr_mma[NQ]) {
+    auto kern = entropy_mma_kernel<NQ, NZ>;
+    bool& attr = NZ == 1 ? c->attr_mma2v[NQ] : c->attr_mma[NQ];
+    if (!attr) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)M::SMEM));
-        c->attr_mma[NQ] = true;
+        attr = true;
     }
     dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
     kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
                                                     (const double*)c->facttab.p, (const TileBox*)c->tilebox.p,
                                                     c->d_cutstats, (double*)c->part.p, stop);
     return 0;
+}
+
+// 2-V mode (landau_set_dimension(2)): the native planar node grid, n_q^2 nodes instead of n_q^3
+template <int NQ>
+int launch_entropy_mma(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
+    return c->dim == 2 ? launch_entropy_mma_nz<NQ, 1>(c, cl, nchunks, stop) : launch_entropy_mma_nz<NQ, NQ>(c, cl, nchunks, stop);
 }
 
 // node groups (gridDim.z) each kernel splits the n_q^3 node sums into
@@ -531,7 +547,7 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     }
     entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
-        mode == 1 ? 0 : (mode >= 2 ? 2 : 1), cl.Gx(), cl.Gy(), cl.Gz(), cl.snode(), stop);
+        mode == 1 ? 0 : (mode >= 2 ? 2 : 1), (c->dim == 2 && use_mma) ? 1 : 0, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode(), stop);
     c->launches += 1;
     CU(cudaGetLastError());
     cl.G_valid = true;
@@ -549,8 +565,27 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     c->k_pair = use_sym ? "sym" : "onesided";
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     const bool fp32_field = c->precision == 1 && !ctrl;     // FP32 variant: field evaluation only
+    if (use_sym && !fp32_field && ctrl && mixed_step_active(c, cl)) {
+        // mixed-precision step (landau_set_mixed_precision): both flavours are enqueued, the device flag
+        // StepCtrl::use_f32 (set by step_update_kernel from the last residual) decides which one runs
+        const size_t n7 = 7 * (size_t)cl.npad_max;
+        RC(ensure(c, c->soa32, sizeof(float) * n7));
+        soa_to_f32_kernel<<<c->sm_count * 4, 256, 0, c->stream>>>(n7, cl.soas(), (float*)c->soa32.p, ctrl);
+        c->launches += 1;
+        c->k_pair = "sym_mixed";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+        RC(launch_pair_sym<float>(c, cl, ctrl, (const float*)c->soa32.p, c->attr_sym32, nparts_out, 1));
+        RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out, 0));
+        return 0;
+    }
     if (use_sym && !fp32_field) {
-        RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out));
+        if (c->dim == 2) {                     // native 2-V arithmetic (landau_set_dimension(2))
+            c->k_pair = "sym2v";
+            snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+            RC((launch_pair_sym<double, 2>(c, cl, ctrl, cl.soas(), c->attr_sym64_2v, nparts_out)));
+        } else {
+            RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out));
+        }
         return 0;
     }
     if (c->precision == 1 && !ctrl && cl.sym) {             // FP32 field variant, symmetric kernel in FP32
@@ -590,7 +625,16 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     nchunks = std::min(nchunks, 32);
     RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
     dim3 grid(ttiles, nchunks);
-    if (R == 1)
+    if (c->dim == 2) {                         // native 2-V arithmetic (landau_set_dimension(2))
+        c->k_pair = "onesided2v";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+        if (R == 1)
+            pair_onesided_kernel<1, 2><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
+                                                                            cl.recs(), (double*)c->vpart.p);
+        else
+            pair_onesided_kernel<2, 2><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
+                                                                            cl.recs(), (double*)c->vpart.p);
+    } else if (R == 1)
         pair_onesided_kernel<1><<<grid, PAIR_THREADS, 0, c->stream>>>(c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks,
                                                                      cl.recs(), (double*)c->vpart.p);
     else
@@ -751,7 +795,8 @@ int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b) {
     cudaStream_t st = c->stream;
     step_begin_kernel<<<ceil_div(b.npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, b.npm, cl.x(), cl.y(), cl.z(),
                                                              cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), b.xk, b.yk, b.zk,
-                                                             cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr);
+                                                             cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr,
+                                                             mixed_step_active(c, cl) ? 1 : 0);
     c->launches += 1;
     if (c->solver == 1) {
         anderson_begin_kernel<<<1, 32, 0, st>>>(c->d_aa, c->aa_depth);
@@ -784,7 +829,8 @@ int enqueue_step_iteration(landau_ctx* c, Cloud& cl, const StepBufs& b, double d
     if (c->solver == 0) {
         step_update_kernel<<<b.nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                            (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
-                                                           b.xk, b.yk, b.zk, rec, soa, (double*)c->blockpart.p, cond);
+                                                           b.xk, b.yk, b.zk, rec, soa, (double*)c->blockpart.p, cond,
+                                                           mixed_step_active(c, cl) ? c->mixed_until : 0.0);
         c->launches += 1;
     } else if (c->solver == 1) {
         // NEXT-4: Anderson-accelerated fixed point (step_anderson.cuh); commits g(x_k) of the last evaluation
@@ -841,6 +887,7 @@ bool step_graph_matches(const landau_ctx* c, const Cloud& cl, double dt, double 
     const auto& g = c->sg;
     return g.exec && g.gen == c->alloc_gen && g.N == cl.N && g.npm == cl.npad_max && g.dt == dt && g.tol == tol &&
            g.max_iter == max_iter && g.ek == c->entropy_kernel && g.pk == c->pair_kernel && g.solver == c->solver &&
+           g.mixed == c->mixed_until &&
            g.depth == (c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0);
 }
 
@@ -930,6 +977,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
     g.graph = graph; g.exec = exec; g.gen = c->alloc_gen; g.N = cl.N; g.npm = npm; g.dt = dt; g.tol = tol;
     g.max_iter = max_iter; g.ek = c->entropy_kernel; g.pk = c->pair_kernel; g.fixed_nodes = fixed; g.body_nodes = body_nodes;
     g.solver = c->solver; g.depth = c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0;
+    g.mixed = c->mixed_until;
     return 0;
 }
 }  // namespace
@@ -1257,6 +1305,7 @@ int landau_set_dimension(landau_ctx* c, int dim) {
     if (dim != 2 && dim != 3) return fail(c, LANDAU_EINVAL, "set_dimension: dim must be 2 or 3");
     c->dim = dim;
     c->state.G_valid = false; c->tmp.G_valid = false;
+    ++c->alloc_gen;                              // a captured step graph holds the other dimension's kernels
     CU(cudaMemcpyAsync(&c->d_tab->dim, &c->dim, sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return 0;
@@ -1302,6 +1351,14 @@ int landau_set_substep(landau_ctx* c, int max_halvings) {
     if (!c) return LANDAU_EINVAL;
     if (max_halvings < 0 || max_halvings > 10) return fail(c, LANDAU_EINVAL, "set_substep: max_halvings must be 0..10");
     c->substep = max_halvings;
+    return 0;
+}
+
+int landau_set_mixed_precision(landau_ctx* c, double f32_until) {
+    if (!c) return LANDAU_EINVAL;
+    if (!(f32_until >= 0.0) || !isfinite(f32_until))
+        return fail(c, LANDAU_EINVAL, "set_mixed_precision: the switch-over residual must be >= 0 (0 = off)");
+    c->mixed_until = f32_until;
     return 0;
 }
 

@@ -30,10 +30,23 @@ __device__ __forceinline__ void pair_accumulate(double zx, double zy, double zz,
     az = fma(a, fma(-zz, h, cz), az);
 }
 
+// 2-V form of pair_accumulate (landau_set_dimension(2): v_z = 0, g_z = 0): the z terms vanish identically; the x, y
+// results are bit-identical to the 3-V arithmetic on such data.
+__device__ __forceinline__ void pair_accumulate2(double zx, double zy, double cx, double cy, double wq, double& ax,
+                                                 double& ay) {
+    const double r2 = fma(zy, zy, zx * zx);
+    const double d = fma(zy, cy, zx * cx);
+    const double yv = rsqrt_or_zero(r2);
+    const double h = d * (yv * yv);
+    const double a = wq * yv;
+    ax = fma(a, fma(-zx, h, cx), ax);
+    ay = fma(a, fma(-zy, h, cy), ay);
+}
+
 // grid = (target tiles, source chunks).  Each thread owns R targets (slots tile*128R + r*128 + tid).
 // Partial fields are written chunk-major: vpart[((chunk*3 + d) * npad_max) + slot], already scaled
 // by nu_ss'/m_s, so that the combine step is a fixed-order sum over chunks.
-template <int R>
+template <int R, int DIM = 3>
 __global__ void __launch_bounds__(PAIR_THREADS)
 pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                      const StepCtrl* __restrict__ ctrl, int npad_max, int nchunks,
@@ -83,9 +96,13 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
             const double2* q = reinterpret_cast<const double2*>(sm + j * 8);
             const double2 a = q[0], b = q[1], c = q[2], d = q[3];
 #pragma unroll
-            for (int r = 0; r < R; ++r)
-                pair_accumulate(px[r] - a.x, py[r] - a.y, pz[r] - b.x, gx[r] - c.x, gy[r] - c.y,
-                                gz[r] - d.x, b.y, ax[r], ay[r], az[r]);
+            for (int r = 0; r < R; ++r) {
+                if (DIM == 3)
+                    pair_accumulate(px[r] - a.x, py[r] - a.y, pz[r] - b.x, gx[r] - c.x, gy[r] - c.y,
+                                    gz[r] - d.x, b.y, ax[r], ay[r], az[r]);
+                else
+                    pair_accumulate2(px[r] - a.x, py[r] - a.y, gx[r] - c.x, gy[r] - c.y, b.y, ax[r], ay[r]);
+            }
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {

@@ -115,7 +115,10 @@ template <typename F> struct SymVec2;
 template <> struct SymVec2<double> { using type = double2; };
 template <> struct SymVec2<float> { using type = float2; };
 
-template <bool SYM, int RT, int RS, typename F>
+// DIM = 2: the paper's 2-V setting (v_z = 0, g_z = 0; landau_set_dimension(2)): the z components of z, g_p - g_q and
+// of both accumulators are identically zero and are not computed -- 22 instead of 30 FP64 instructions per unordered
+// pair, results bit-identical to the 3-V arithmetic on v_z = 0 data (fma(0, 0, x) = x).
+template <bool SYM, int RT, int RS, typename F, int DIM>
 __device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], const F (&pz)[RT],
                                          const F (&gx)[RT], const F (&gy)[RT], const F (&gz)[RT],
                                          const F (&wp)[RT], F (&ax)[RT], F (&ay)[RT],
@@ -127,31 +130,39 @@ __device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], c
     for (int s = 0; s < RS; ++s) {
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const F zx = px[r] - qx[s], zy = py[r] - qy[s], zz = pz[r] - qz[s];
-            const F cx = gx[r] - hx[s], cy = gy[r] - hy[s], cz = gz[r] - hz[s];
-            const F r2 = sym_fma(zz, zz, sym_fma(zy, zy, zx * zx));
-            const F d = sym_fma(zz, cz, sym_fma(zy, cy, zx * cx));
+            const F zx = px[r] - qx[s], zy = py[r] - qy[s];
+            const F cx = gx[r] - hx[s], cy = gy[r] - hy[s];
+            F r2 = sym_fma(zy, zy, zx * zx), d = sym_fma(zy, cy, zx * cx);
+            F zz = F(0), cz = F(0);
+            if (DIM == 3) {
+                zz = pz[r] - qz[s]; cz = gz[r] - hz[s];
+                r2 = sym_fma(zz, zz, r2); d = sym_fma(zz, cz, d);
+            }
             const F yv = rsqrt_or_zero(r2);
             const F h = d * (yv * yv);
-            const F ux = sym_fma(-zx, h, cx), uy = sym_fma(-zy, h, cy), uz = sym_fma(-zz, h, cz);
+            const F ux = sym_fma(-zx, h, cx), uy = sym_fma(-zy, h, cy);
             const F a = wq[s] * yv;
-            ax[r] = sym_fma(a, ux, ax[r]); ay[r] = sym_fma(a, uy, ay[r]); az[r] = sym_fma(a, uz, az[r]);
+            ax[r] = sym_fma(a, ux, ax[r]); ay[r] = sym_fma(a, uy, ay[r]);
+            F uz = F(0);
+            if (DIM == 3) { uz = sym_fma(-zz, h, cz); az[r] = sym_fma(a, uz, az[r]); }
             if (SYM) {
                 const F b = wp[r] * yv;
-                bx[s] = sym_fma(b, ux, bx[s]); by[s] = sym_fma(b, uy, by[s]); bz[s] = sym_fma(b, uz, bz[s]);
+                bx[s] = sym_fma(b, ux, bx[s]); by[s] = sym_fma(b, uy, by[s]);
+                if (DIM == 3) bz[s] = sym_fma(b, uz, bz[s]);
             }
         }
     }
 }
 
-template <int W, int RT, int RS, typename F = double>
+template <int W, int RT, int RS, typename F = double, int DIM = 3>
 __global__ void __launch_bounds__(W * 32, 1)
 pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 const StepCtrl* __restrict__ ctrl, int npad_max, const F* __restrict__ soa,
-                double* acc, double* __restrict__ tpart, int* ticket, int* errflag) {
+                double* acc, double* __restrict__ tpart, int* ticket, int* errflag, int only_if_f32 = -1) {
     using C = SymCfg<W, RT, RS, F>;
     using F2 = typename SymVec2<F>::type;
     if (ctrl && ctrl->done) return;
+    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;     // mixed-precision step: the other kernel runs
     extern __shared__ __align__(128) unsigned char smem_raw[];
     F* s_src = reinterpret_cast<F*>(smem_raw);                        // [2][NCOMP][BS]
     F* s_acc = s_src + 2 * C::NCOMP * C::BS;                          // [3][BS]
@@ -187,9 +198,10 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     auto issue_load = [&](int unit, int stage) {
         if (tid == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_expect_tx(&s_bar[stage], C::NCOMP * C::BS * (uint32_t)sizeof(F));
+            mbar_expect_tx(&s_bar[stage], (DIM == 3 ? C::NCOMP : C::NCOMP - 2) * C::BS * (uint32_t)sizeof(F));
 #pragma unroll
             for (int c = 0; c < C::NCOMP; ++c)
+                if (DIM == 3 || (c != 2 && c != 6))               // 2-V: the z rows are not needed
                 bulk_g2s(s_src + ((size_t)stage * C::NCOMP + c) * C::BS,
                          soa + (size_t)c * npad_max + (size_t)unit * C::BS, C::BS * (uint32_t)sizeof(F),
                          &s_bar[stage]);
@@ -205,7 +217,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
             const int q = wv * 32 * RT + r * 32 + lane;
             seg[q] = (double)ax[r] * im;
             seg[C::BT + q] = (double)ay[r] * im;
-            seg[2 * C::BT + q] = (double)az[r] * im;
+            seg[2 * C::BT + q] = DIM == 3 ? (double)az[r] * im : 0.0;
         }
     };
     F px[RT], py[RT], pz[RT], gx[RT], gy[RT], gz[RT], w0[RT], wp[RT], ax[RT], ay[RT], az[RT];
@@ -222,10 +234,11 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 #pragma unroll
             for (int r = 0; r < RT; ++r) {
                 const int p = I * C::BT + wv * 32 * RT + r * 32 + lane;
-                px[r] = soa[p]; py[r] = soa[(size_t)npad_max + p]; pz[r] = soa[2 * (size_t)npad_max + p];
+                px[r] = soa[p]; py[r] = soa[(size_t)npad_max + p];
+                pz[r] = DIM == 3 ? soa[2 * (size_t)npad_max + p] : F(0);
                 w0[r] = soa[3 * (size_t)npad_max + p];
                 gx[r] = soa[4 * (size_t)npad_max + p]; gy[r] = soa[5 * (size_t)npad_max + p];
-                gz[r] = soa[6 * (size_t)npad_max + p];
+                gz[r] = DIM == 3 ? soa[6 * (size_t)npad_max + p] : F(0);
                 ax[r] = ay[r] = az[r] = F(0);
             }
         }
@@ -239,7 +252,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         const bool diag = j < rho * (I + 1);
 #pragma unroll
         for (int r = 0; r < RT; ++r) wp[r] = w0[r] * nu;
-        for (int i = tid; i < 3 * C::BS; i += C::THREADS) s_acc[i] = F(0);
+        for (int i = tid; i < DIM * C::BS; i += C::THREADS) s_acc[i] = F(0);
         // rank of this visit of source unit j among the visits by all tiles I' < j/rho (header comment)
         const int par = (int)((t - t0) & 1);
         if (tid == 0) s_rank[par ^ 1] = 0;
@@ -272,25 +285,31 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                     for (int s = 0; s < RS; s += 2) {
                         const F2 a0 = *reinterpret_cast<const F2*>(sx + 0 * C::BS + g + s);
                         const F2 a1 = *reinterpret_cast<const F2*>(sx + 1 * C::BS + g + s);
-                        const F2 a2 = *reinterpret_cast<const F2*>(sx + 2 * C::BS + g + s);
                         const F2 a3 = *reinterpret_cast<const F2*>(sx + 3 * C::BS + g + s);
                         const F2 a4 = *reinterpret_cast<const F2*>(sx + 4 * C::BS + g + s);
                         const F2 a5 = *reinterpret_cast<const F2*>(sx + 5 * C::BS + g + s);
-                        const F2 a6 = *reinterpret_cast<const F2*>(sx + 6 * C::BS + g + s);
-                        qx[s] = a0.x; qx[s + 1] = a0.y; qy[s] = a1.x; qy[s + 1] = a1.y; qz[s] = a2.x; qz[s + 1] = a2.y;
+                        qx[s] = a0.x; qx[s + 1] = a0.y; qy[s] = a1.x; qy[s + 1] = a1.y;
                         qw[s] = a3.x * nu; qw[s + 1] = a3.y * nu;
-                        hx[s] = a4.x; hx[s + 1] = a4.y; hy[s] = a5.x; hy[s + 1] = a5.y; hz[s] = a6.x; hz[s + 1] = a6.y;
+                        hx[s] = a4.x; hx[s + 1] = a4.y; hy[s] = a5.x; hy[s + 1] = a5.y;
+                        qz[s] = qz[s + 1] = hz[s] = hz[s + 1] = F(0);
+                        if (DIM == 3) {
+                            const F2 a2 = *reinterpret_cast<const F2*>(sx + 2 * C::BS + g + s);
+                            const F2 a6 = *reinterpret_cast<const F2*>(sx + 6 * C::BS + g + s);
+                            qz[s] = a2.x; qz[s + 1] = a2.y; hz[s] = a6.x; hz[s + 1] = a6.y;
+                        }
                     }
                 } else {
 #pragma unroll
                     for (int s = 0; s < RS; ++s) {
-                        qx[s] = sx[0 * C::BS + g + s]; qy[s] = sx[1 * C::BS + g + s]; qz[s] = sx[2 * C::BS + g + s];
+                        qx[s] = sx[0 * C::BS + g + s]; qy[s] = sx[1 * C::BS + g + s];
+                        qz[s] = DIM == 3 ? sx[2 * C::BS + g + s] : F(0);
                         qw[s] = sx[3 * C::BS + g + s] * nu;
-                        hx[s] = sx[4 * C::BS + g + s]; hy[s] = sx[5 * C::BS + g + s]; hz[s] = sx[6 * C::BS + g + s];
+                        hx[s] = sx[4 * C::BS + g + s]; hy[s] = sx[5 * C::BS + g + s];
+                        hz[s] = DIM == 3 ? sx[6 * C::BS + g + s] : F(0);
                     }
                 }
                 if (diag) {
-                    sym_step<false, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<false, RT, RS, F, DIM>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                 } else {
                     // the source-side sums live in shared memory next to their sources: in this phase the sub-tile is
                     // this warp's alone and at step k every lane holds another group, so the read-modify-write is
@@ -300,14 +319,20 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                         for (int s = 0; s < RS; s += 2) {
                             const F2 b0 = *reinterpret_cast<const F2*>(s_acc + g + s);
                             const F2 b1 = *reinterpret_cast<const F2*>(s_acc + C::BS + g + s);
-                            const F2 b2 = *reinterpret_cast<const F2*>(s_acc + 2 * C::BS + g + s);
-                            bx[s] = b0.x; bx[s + 1] = b0.y; by[s] = b1.x; by[s + 1] = b1.y; bz[s] = b2.x; bz[s + 1] = b2.y;
+                            bx[s] = b0.x; bx[s + 1] = b0.y; by[s] = b1.x; by[s + 1] = b1.y; bz[s] = bz[s + 1] = F(0);
+                            if (DIM == 3) {
+                                const F2 b2 = *reinterpret_cast<const F2*>(s_acc + 2 * C::BS + g + s);
+                                bz[s] = b2.x; bz[s + 1] = b2.y;
+                            }
                         }
                     } else {
 #pragma unroll
-                        for (int s = 0; s < RS; ++s) { bx[s] = s_acc[g + s]; by[s] = s_acc[C::BS + g + s]; bz[s] = s_acc[2 * C::BS + g + s]; }
+                        for (int s = 0; s < RS; ++s) {
+                            bx[s] = s_acc[g + s]; by[s] = s_acc[C::BS + g + s];
+                            bz[s] = DIM == 3 ? s_acc[2 * C::BS + g + s] : F(0);
+                        }
                     }
-                    sym_step<true, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<true, RT, RS, F, DIM>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                     if (RS % 2 == 0) {
 #pragma unroll
                         for (int s = 0; s < RS; s += 2) {
@@ -315,11 +340,14 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                             b0.x = bx[s]; b0.y = bx[s + 1]; b1.x = by[s]; b1.y = by[s + 1]; b2.x = bz[s]; b2.y = bz[s + 1];
                             *reinterpret_cast<F2*>(s_acc + g + s) = b0;
                             *reinterpret_cast<F2*>(s_acc + C::BS + g + s) = b1;
-                            *reinterpret_cast<F2*>(s_acc + 2 * C::BS + g + s) = b2;
+                            if (DIM == 3) *reinterpret_cast<F2*>(s_acc + 2 * C::BS + g + s) = b2;
                         }
                     } else {
 #pragma unroll
-                        for (int s = 0; s < RS; ++s) { s_acc[g + s] = bx[s]; s_acc[C::BS + g + s] = by[s]; s_acc[2 * C::BS + g + s] = bz[s]; }
+                        for (int s = 0; s < RS; ++s) {
+                            s_acc[g + s] = bx[s]; s_acc[C::BS + g + s] = by[s];
+                            if (DIM == 3) s_acc[2 * C::BS + g + s] = bz[s];
+                        }
                     }
                     __syncwarp();
                 }
@@ -337,7 +365,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 }
             }
             __syncthreads();
-            for (int i = tid; i < 3 * C::BS; i += C::THREADS) {
+            for (int i = tid; i < DIM * C::BS; i += C::THREADS) {
                 const int d = i / C::BS, e = i - d * C::BS;
                 double* o = acc + (size_t)d * npad_max + (size_t)j * C::BS + e;
                 __stcg(o, __ldcg(o) + sc * (double)s_acc[i]);
@@ -354,8 +382,9 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 // Before a launch of pair_sym_kernel: zero the in-place source-side accumulator and the per-unit tickets
 // (skipped, like every kernel of an iteration, once the step is done).
 __global__ void sym_reset_kernel(const StepCtrl* __restrict__ ctrl, double* __restrict__ acc, size_t n,
-                                 int* __restrict__ ticket, int nticket) {
+                                 int* __restrict__ ticket, int nticket, int only_if_f32 = -1) {
     if (ctrl && ctrl->done) return;
+    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (size_t i = i0; i < n; i += stride) acc[i] = 0.0;
@@ -366,8 +395,9 @@ __global__ void sym_reset_kernel(const StepCtrl* __restrict__ ctrl, double* __re
 // the slot's tile, added in CTA order (the CTAs whose runs of tasks meet the tile's row).  G = grid of the pair kernel.
 __global__ void sym_combine_kernel(const DevLayout* __restrict__ L, const StepCtrl* __restrict__ ctrl, int npad_max,
                                    int G, int BT, int BS, const double* __restrict__ acc,
-                                   const double* __restrict__ tpart, double* __restrict__ out) {
+                                   const double* __restrict__ tpart, double* __restrict__ out, int only_if_f32 = -1) {
     if (ctrl && ctrl->done) return;
+    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npad_max) return;
     const size_t np = (size_t)npad_max;
@@ -407,8 +437,10 @@ __global__ void build_soa_kernel(const DevTable* __restrict__ T, const DevLayout
     for (int c = 0; c < 7; ++c) soa[(size_t)c * npad_max + p] = v[c];
 }
 
-// FP64 SoA source copy -> FP32 (FP32 field variant).
-__global__ void soa_to_f32_kernel(size_t n, const double* __restrict__ a, float* __restrict__ b) {
+// FP64 SoA source copy -> FP32 (FP32 field variant; mixed-precision step: only while ctrl->use_f32 is set).
+__global__ void soa_to_f32_kernel(size_t n, const double* __restrict__ a, float* __restrict__ b,
+                                  const StepCtrl* __restrict__ ctrl = nullptr) {
+    if (ctrl && (ctrl->done || !ctrl->use_f32)) return;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) b[i] = (float)a[i];
 }

@@ -26,10 +26,10 @@ __global__ void step_begin_kernel(const DevTable* __restrict__ T, const DevLayou
                                   const double* __restrict__ Gx, const double* __restrict__ Gy,
                                   const double* __restrict__ Gz, double* __restrict__ xk,
                                   double* __restrict__ yk, double* __restrict__ zk,
-                                  double* __restrict__ rec, double* __restrict__ soa) {
+                                  double* __restrict__ rec, double* __restrict__ soa, int start_f32 = 0) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p == 0) {
-        ctrl->done = 0; ctrl->iterations = 0; ctrl->converged = 0; ctrl->ticket = 0u;
+        ctrl->done = 0; ctrl->iterations = 0; ctrl->converged = 0; ctrl->ticket = 0u; ctrl->use_f32 = start_f32;
         ctrl->residual = __longlong_as_double(0x7ff0000000000000LL);
     }
     if (p >= npad_max) return;
@@ -64,7 +64,7 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
                    const double* __restrict__ yn, const double* __restrict__ zn,
                    const double* __restrict__ w, double* __restrict__ xk, double* __restrict__ yk,
                    double* __restrict__ zk, double* __restrict__ rec, double* __restrict__ soa,
-                   double* __restrict__ blockpart, cudaGraphConditionalHandle cond) {
+                   double* __restrict__ blockpart, cudaGraphConditionalHandle cond, double f32_until = 0.0) {
     if (ctrl->done) return;
     __shared__ double s_num[UPD_THREADS / 32], s_den[UPD_THREADS / 32];
     __shared__ int s_last;
@@ -123,8 +123,12 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         const int it = ctrl->iterations + 1;
         ctrl->iterations = it;
         ctrl->residual = res;
+        // mixed-precision step: pass 2 runs in FP32 while the iterates still move by more than f32_until; an iterate
+        // that came from an FP32 evaluation never ends the step as converged (the next evaluation is FP64)
+        const int was_f32 = ctrl->use_f32;
+        ctrl->use_f32 = (f32_until > 0.0 && res > f32_until) ? 1 : 0;
         if (!isfinite(res)) { ctrl->err = -4; ctrl->done = 1; }
-        else if (res <= tol) { ctrl->converged = 1; ctrl->done = 1; }
+        else if (res <= tol && !was_f32) { ctrl->converged = 1; ctrl->done = 1; }
         else if (it >= max_iter) ctrl->done = 1;
         // CUDA-graph mode: this kernel is the last node of a WHILE body; keep looping until the step is done
         if (cond) cudaGraphSetConditional(cond, ctrl->done ? 0u : 1u);

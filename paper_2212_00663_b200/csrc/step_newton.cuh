@@ -9,14 +9,15 @@
 // (d(Q Gamma)/dz ~ Gamma/|z|^2, SURVEY.md reading S8).  Newton's method solves  (I - g'(x)) d = g(x) - x  and
 // sets x <- x + d; the linear systems are solved by GMRES(m) in the energy inner product <a,b> = sum_p w_p m_s a_p.b_p
 // (the norm of the residual r_k, reading S7) with Jacobian-vector products by one-sided differences of the FIELD,
-//     (I - g'(x)) q  ~  q - dt (V[u(x) + e q/2] - V[u(x)])/e,       e = 2e-9 |x| / |q|,
-// i.e. ONE more pass 2 (the same kernel, markers moved by e q / 2) per Krylov vector.  The difference quotient is
-// accurate to ~1e-7 (round-off of the moved positions, eps_mach |u| / e) plus e times the local curvature, which
-// for the closest pairs (|z| ~ 1e-3 of the thermal speed) is ~1e-5: a linear solve is therefore never asked for
-// more than 1e-6, and Newton's outer iteration -- whose residual is a TRUE evaluation of g(x) - x -- supplies the
-// rest.  GMRES minimises the linear residual over the Krylov space, so it needs no more products than Jacobi needs
+//     (I - g'(x)) q  ~  q - dt (V[u(x) + e q/2] - V[u(x)])/e,       e = 1e-11 |x| / |q|,
+// i.e. ONE more pass 2 (the same kernel, markers moved by e q / 2) per Krylov vector.  The difference quotient has
+// two errors: round-off of the moved positions, eps_mach |u| / e ~ 1e-5, and e q_p against the separation of the
+// closest pairs -- a Krylov vector concentrated on two nearly coincident markers (|z| ~ 1e-6 of the thermal speed
+// occurs) moves them by e / sqrt(w m) ~ 1e-9, which a larger step would not resolve.  A linear
+// solve is therefore never asked for more than 1e-4, and Newton's outer iteration -- whose residual is a TRUE
+// evaluation of g(x) - x -- supplies the rest (measured: profiles/r2_solvers.md).  GMRES minimises the linear residual over the Krylov space, so it needs no more products than Jacobi needs
 // sweeps when Jacobi converges, and a few more per outlying eigenvalue when it does not.  Inexact Newton: the first
-// system is solved to 1e-3, later ones to what the tolerance still asks for (clamped to [1e-6, 1e-3]).
+// system is solved to 1e-3, later ones to what the tolerance still asks for (clamped to [1e-4, 1e-3]).
 // Globalisation: if a Newton update does not reduce the residual, it is halved (up to 6 times) before the next
 // linearisation (backtracking on |g(x) - x|).
 //
@@ -34,6 +35,12 @@
 
 namespace landau {
 
+#ifndef NK_EPS_REL      // tuning knobs of the difference quotient (see the header comment)
+#define NK_EPS_REL 1e-11
+#endif
+#ifndef NK_ETA_MIN
+#define NK_ETA_MIN 1e-4
+#endif
 constexpr int NK_MAXM = 30;
 constexpr int NK_NRED = NK_MAXM + 2;
 
@@ -202,11 +209,11 @@ nk_post_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, 
         } else {
             const double beta = sqrt(s_tot[0]);
             nk->beta = beta;
-            nk->eps_fd = 2e-9 * fmax(sqrt(s_tot[2]), 1e-300);         // |q| = 1 in the same norm
+            nk->eps_fd = NK_EPS_REL * fmax(sqrt(s_tot[2]), 1e-300);   // |q| = 1 in the same norm
             // inexact Newton: first system to 1e-3, later ones to what the tolerance still asks for, never beyond
             // the accuracy of the difference quotient
             double eta = nk->newton_its <= 1 ? 1e-3 : 0.3 * tol / res;
-            eta = fmin(1e-3, fmax(eta, 1e-6));
+            eta = fmin(1e-3, fmax(eta, NK_ETA_MIN));
             nk->eta = eta;
             nk->res_prev = res;
             nk->backtracks = 0; nk->have_update = 0; nk->lam = 1.0;

@@ -43,8 +43,10 @@ def _sample_plan(n_steps: int):
 
 
 def run(test: int, n_grid: int = 32, steps=None, solver: int = 0, depth: int = 3, verbose: bool = False,
-        substep: int = 0):
+        substep: int = 0, max_iter=None):
     wl = W.paper_test(test, n_grid, n_steps=steps)
+    if max_iter is not None:
+        wl.max_iter = int(max_iter)
     t0, v0, T0 = wl.notes["t0_seconds"], wl.notes["v0_m_per_s"], wl.notes["T0_eV"]
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
     g.set_dimension(2)
@@ -83,7 +85,8 @@ def run(test: int, n_grid: int = 32, steps=None, solver: int = 0, depth: int = 3
     T2 = 0.5 * (H["Tx"] + H["Ty"])                                  # 2-V species temperature
     out = dict(test=test, name=wl.name, n_grid=n_grid, n_markers=wl.n_markers, steps=wl.n_steps,
                dt_seconds=wl.dt * t0, t_end_seconds=float(t[-1]), t0_seconds=t0, eps=wl.eps.tolist(),
-               solver="jacobi" if not solver else f"anderson depth {depth}", substep_levels=substep, wall_s=wall,
+               solver={0: "jacobi", 1: f"anderson depth {depth}", 2: f"newton-krylov restart {depth}"}[solver],
+               max_iter=wl.max_iter, substep_levels=substep, wall_s=wall,
                steps_per_s=wl.n_steps / wall, iterations_mean=float(np.mean(iters)), iterations_max=int(np.max(iters)),
                steps_not_converged=int(notconv), energy_error_rel_max=float(np.abs(K - K[0]).max() / K[0]),
                momentum_error_rel_max=float(np.abs(Pt - Pt[0]).max() / wm_abs),
@@ -137,14 +140,18 @@ def main():
     ap.add_argument("--test", type=int, required=True, choices=[1, 2, 3])
     ap.add_argument("--n-grid", type=int, default=32)
     ap.add_argument("--steps", type=int, default=None, help="default: t_max/dt = 1e5 (PAPER.md:210-214)")
-    ap.add_argument("--solver", choices=["jacobi", "anderson"], default="jacobi")
+    ap.add_argument("--solver", choices=["jacobi", "anderson", "newton"], default="jacobi")
     ap.add_argument("--anderson-depth", type=int, default=3)
+    ap.add_argument("--newton-restart", type=int, default=20)
+    ap.add_argument("--max-iter", type=int, default=None)
     ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
     ap.add_argument("--out", default="gpurun_out")
     ap.add_argument("--tag", default="")
     args = ap.parse_args()
-    wl, H, out = run(args.test, args.n_grid, args.steps, 1 if args.solver == "anderson" else 0, args.anderson_depth,
-                     verbose=True, substep=args.substep)
+    solver = {"jacobi": 0, "anderson": 1, "newton": 2}[args.solver]
+    wl, H, out = run(args.test, args.n_grid, args.steps, solver,
+                     args.newton_restart if solver == 2 else args.anderson_depth, verbose=True, substep=args.substep,
+                     max_iter=args.max_iter)
     write(Path(args.out), args.test, H, out, args.tag)
     print(json.dumps(out))
 

@@ -676,6 +676,48 @@ def test_two_v_mode_keeps_vz_zero_and_matches_oracle(B, oracle_mod):
         g.set_dimension(4)
 
 
+@pytest.mark.parametrize("test,n_grid,n_q,kernels", [(3, 24, 4, {}), (1, 16, 3, {}), (2, 20, 6, {}),
+                                                      (3, 100, 4, {}), (3, 24, 4, dict(pair_kernel=2, entropy_kernel=3))])
+def test_native_two_v_kernels_match_oracle_and_the_three_v_path(B, oracle_mod, test, n_grid, n_q, kernels):
+    """landau_set_dimension(2) runs native 2-V kernels (n_q^2 planar nodes in pass 1, two-component pair arithmetic in
+    pass 2).  On the paper's meshes (v_z = 0): G, S_eps and V equal the ORACLE's 3-V
+    formulas on the same data (reading D1: that IS the paper's 2-V scheme) to 1e-10, and the 3-V CUDA path on the same
+    data to 1e-13 (pass 2 is bit-identical: the dropped terms are fma(0, 0, x))."""
+    wl = W.paper_test(test, n_grid=n_grid)
+    g2, o = make_pair(B, oracle_mod, wl, n_q=n_q, **kernels)
+    g3 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=n_q, nu0=wl.nu0, **kernels)
+    g2.set_dimension(2)
+    G2, S2 = g2.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    G3, S3 = g3.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    G2, G3 = G2.cpu().numpy(), G3.cpu().numpy()
+    assert np.all(G2[:, 2] == 0.0)
+    assert_field_close(G2[:, :2], G3[:, :2], wl.species_id, wl.n_species, tol=1e-13, what="2-V vs 3-V entropy gradient")
+    np.testing.assert_allclose(S2, S3, rtol=1e-13)
+    if wl.n_markers <= 4000:
+        Gref, Sref = o.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+        assert_field_close(G2[:, :2], Gref[:, :2], wl.species_id, wl.n_species, what="2-V entropy gradient")
+        np.testing.assert_allclose(S2, Sref, rtol=1e-11, atol=1e-12)
+    else:
+        rows = np.arange(0, wl.n_markers, 97).astype(np.int64)
+        Gref = o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows)
+        assert_field_close(G2[rows][:, :2], Gref[:, :2], wl.species_id[rows], wl.n_species, what="2-V entropy gradient rows")
+    Gin = G3.copy(); Gin[:, 2] = 0.0
+    V2 = g2.pair_field(wl.v, wl.w, wl.species_id, Gin).cpu().numpy()
+    V3 = g3.pair_field(wl.v, wl.w, wl.species_id, Gin).cpu().numpy()
+    assert "2v" in g2.last_kernels() and "2v" not in g3.last_kernels()
+    assert np.array_equal(V2[:, :2], V3[:, :2]) and np.all(V2[:, 2] == 0.0)
+    rows = np.arange(0, wl.n_markers, max(1, wl.n_markers // 300)).astype(np.int64)
+    Vref = o.pair_field_rows(wl.v, wl.w, wl.species_id, Gin, rows)
+    assert_field_close(V2[rows][:, :2], Vref[:, :2], wl.species_id[rows], wl.n_species, what="2-V pair field")
+    # one implicit step, both ways
+    g2.set_markers(wl.v, wl.w, wl.species_id); g3.set_markers(wl.v, wl.w, wl.species_id)
+    r2, r3 = g2.step(wl.dt, 1e-12, 50), g3.step(wl.dt, 1e-12, 50)
+    assert r2[0] == r3[0] and abs(r2[1] - r3[1]) <= 1 and abs(r2[2] - r3[2]) <= 1e-3 * r3[2] + 1e-13
+    a, b = g2.get_markers().cpu().numpy(), g3.get_markers().cpu().numpy()
+    assert np.all(a[:, 2] == 0.0)
+    assert_field_close(a[:, :2], b[:, :2], wl.species_id, wl.n_species, tol=1e-12, what="2-V vs 3-V step")
+
+
 # ------------------------------------------------------------------------------------ NEXT-3: many collision cells
 def _make_cells(rng_seed=5):
     """A ragged batch: cells of different sizes, species mixes and orders, one empty cell."""
