@@ -405,6 +405,28 @@ def run_ours(args):
                              "moments": {"ms": 1e3 * t_mom, "algorithmic_bytes": 32.0 * N, "GBps": 32.0 * N / t_mom / 1e9,
                                          "frac": 32.0 * N / t_mom / 1e9 / hbm_gbs},
                              "note": "whole API calls incl. launches and one host synchronisation; per-kernel times: profiles/"}
+        if N >= 16384 and args.solver == "jacobi":
+            # mixed-precision implicit step (landau_set_mixed_precision): FP32 pass 2 while the residual is above 1e-7,
+            # FP64 for the iterations that finish the step; same fixed point, same stopping rule.  Reported beside
+            # the headline, which stays pure FP64.
+            v_ref = step_device()[3].clone()
+            g.set_mixed_precision(1e-7)
+            step_device()
+            torch.cuda.synchronize()
+            e0.record()
+            it_mx, conv_mx = 0, True
+            for _ in range(2):
+                it, conv, m_mx, v_mx = step_device()
+                it_mx += it; conv_mx &= bool(conv)
+            e1.record(); torch.cuda.synchronize()
+            t_mx = e0.elapsed_time(e1) * 1e-3 / 2
+            g.set_mixed_precision(0.0)
+            line["mixed_precision_step"] = {
+                "f32_until_residual": 1e-7, "ms_per_step": 1e3 * t_mx, "steps_per_s": 1.0 / t_mx,
+                "iterations_per_step": it_mx / 2, "all_converged": conv_mx, "kernels": "pair=sym_mixed",
+                "state_rel_diff_vs_fp64_step": float(torch.linalg.norm(v_mx - v_ref) / torch.linalg.norm(v_ref)),
+                "energy_drift_rel": abs(float(m_mx["K"].sum()) - K0) / K0,
+                "speedup_vs_fp64_step": (t_dev_max / args.steps) / t_mx}
         if not args.no_dg:
             # one discrete-gradient step (Eqs. 46-49), device driven; every iteration costs two
             # pass-1 and one pass-2 evaluations.  Its fixed point (G re-evaluated every iteration) is solved with

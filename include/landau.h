@@ -176,6 +176,22 @@ int landau_set_substep(landau_ctx* ctx, int max_halvings);
  * three are device driven (no host synchronisation inside a step). */
 int landau_set_solver(landau_ctx* ctx, int solver, int depth);
 
+/* SURVEY.md NEXT-4 (robustness): exact local treatment of stiff two-marker interactions inside landau_step /
+ * landau_run (Jacobi and Anderson solvers).  The pair term of Eq. (23) is not Lipschitz at z = 0; two markers that have
+ * drifted to within ~dt nu w |Gamma| / m of each other make the fixed-point map of Eq. (24) expand in their relative
+ * coordinate, and the iteration ends at max_iter with a residual ~1e-8 -- the paper's "unable to fully converge on
+ * occasion", reproduced step for step by the oracle.  theta > 0: pairs whose stiffness
+ *   L_pq = (dt/2) nu_ss' (w_q/m_s + w_p/m_s') |g_p - g_q| / |v_p - v_q|^2   (at v^n)
+ * exceeds theta are found by the first pass-2 evaluation of every step, and in every iteration their mutual term is
+ * taken out of the explicit update and solved implicitly and exactly (a two-marker midpoint equation that reduces to
+ * one scalar root; csrc/stiff_pairs.cuh).  SAME equation, residual, stopping rule and status codes: at convergence
+ * every marker satisfies Eq. (24); only the path of the iteration changes, so steps that the plain iteration can
+ * converge give the same v^{n+1} to ~tol.  0.2 is a good value.  theta = 0 (default): off, the paper's plain
+ * iteration.  landau_stiff_pairs_last returns how many stiff pairs the last step found and how many of them its last
+ * iteration had to leave to the plain update (HOST outputs; synchronises). */
+int landau_set_stiff_pairs(landau_ctx* ctx, double theta);
+int landau_stiff_pairs_last(landau_ctx* ctx, int* n_pairs, int* n_skipped);
+
 /* Mixed-precision implicit step ("try FP32 pass-2 evaluations for the early iterations").  f32_until > 0:
  * while the Jacobi iterates of Eq. (24) still move by more than f32_until (the residual r_k of the last iteration),
  * pass 2 is evaluated by the FP32 flavour of the symmetric kernel (the BASELINE config-4 field variant: ~3e-6 relative

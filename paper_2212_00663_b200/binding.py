@@ -24,7 +24,7 @@ EINVAL, ENOMEM, ECUDA, ENONFINITE, ERANGE = -1, -2, -3, -4, -5
 SYMBOLS = [
     "landau_default_opts", "landau_create", "landau_destroy", "landau_eval_field",
     "landau_eval_field_host", "landau_entropy_grad", "landau_pair_field", "landau_set_markers",
-    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_set_step_graph", "landau_set_substep", "landau_cells_run", "landau_set_cutoff", "landau_cutoff_stats", "landau_set_mixed_precision",
+    "landau_set_markers_host", "landau_get_markers", "landau_get_markers_host", "landau_step", "landau_step_dg", "landau_set_solver", "landau_set_dimension", "landau_set_step_graph", "landau_set_substep", "landau_cells_run", "landau_set_cutoff", "landau_cutoff_stats", "landau_set_mixed_precision", "landau_set_stiff_pairs", "landau_stiff_pairs_last",
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_fp64_peak_dmma", "landau_last_error",
@@ -90,6 +90,8 @@ def load(build_if_missing: bool = True):
     lib.landau_set_substep.argtypes = [vp, C.c_int]
     lib.landau_set_cutoff.argtypes = [vp, C.c_int, C.c_int]
     lib.landau_set_mixed_precision.argtypes = [vp, C.c_double]
+    lib.landau_set_stiff_pairs.argtypes = [vp, C.c_double]
+    lib.landau_stiff_pairs_last.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     lib.landau_cutoff_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.landau_cells_run.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int,
                                      C.POINTER(CellInfo)]
@@ -283,6 +285,17 @@ class Landau:
     def set_substep(self, max_halvings: int = 0):
         """0 = commit unconverged steps (the paper's behaviour); k > 0 = redo them as two half steps, up to k levels."""
         self._check(self._lib.landau_set_substep(self._h, int(max_halvings)), "landau_set_substep")
+
+    def set_stiff_pairs(self, theta: float = 0.0):
+        """> 0: pairs with stiffness L_pq > theta are solved implicitly and exactly inside the fixed-point iteration
+        (same Eq. (24); NEXT-4 robustness); 0 = off (the paper's plain iteration)."""
+        self._check(self._lib.landau_set_stiff_pairs(self._h, float(theta)), "landau_set_stiff_pairs")
+
+    def stiff_pairs_last(self):
+        """(pairs treated by the last step, overflow flag)."""
+        a, b = C.c_int(0), C.c_int(0)
+        self._check(self._lib.landau_stiff_pairs_last(self._h, C.byref(a), C.byref(b)), "landau_stiff_pairs_last")
+        return int(a.value), int(b.value)
 
     def set_mixed_precision(self, f32_until: float = 0.0):
         """> 0: pass 2 of the implicit step runs in FP32 while the residual exceeds f32_until (then FP64); 0 = off."""

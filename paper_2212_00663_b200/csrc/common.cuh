@@ -67,6 +67,17 @@ struct StepRecord {      // mirrors landau_step_info (host struct) field by fiel
 
 __host__ __device__ inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// Which of several alternative kernels enqueued for one iteration of a device-driven step actually runs.
+// 0: always; 1 / 2: only if the mixed-precision flag is set / clear; 3 / 4: only for the first / a later iteration.
+constexpr int GATE_NONE = 0, GATE_F32 = 1, GATE_F64 = 2, GATE_FIRST = 3, GATE_LATER = 4;
+__device__ __forceinline__ bool gate_closed(const StepCtrl* __restrict__ ctrl, int gate) {
+    if (!ctrl || gate == GATE_NONE) return false;
+    if (gate == GATE_F32) return ctrl->use_f32 != 1;
+    if (gate == GATE_F64) return ctrl->use_f32 != 0;
+    if (gate == GATE_FIRST) return ctrl->iterations != 0;
+    return ctrl->iterations == 0;
+}
+
 __device__ __forceinline__ int species_of_slot(const DevLayout* __restrict__ L, int S, int slot) {
     int s = 0;
 #pragma unroll 1

@@ -26,6 +26,7 @@
 #include "step_dg.cuh"
 #include "step_anderson.cuh"
 #include "step_newton.cuh"
+#include "stiff_pairs.cuh"
 #include "cells.cuh"
 
 using namespace landau;
@@ -88,6 +89,11 @@ struct landau_ctx {
     unsigned long long* d_cutstats = nullptr;   // pass 1 Gaussian cutoff: {source tiles considered, skipped}
     int cutoff_on = 1;                          // landau_set_cutoff
     double mixed_until = 0.0;                   // landau_set_mixed_precision: FP32 pass 2 while the residual exceeds it
+    double stiff_dt = 0.0;                      // dt of the step being enqueued (stiff_begin_kernel)
+    double stiff_theta = 0.0;                   // landau_set_stiff_pairs: pairs with stiffness above it are solved implicitly
+    StiffCtrl* d_stiff = nullptr;
+    Buf stiff_mark, stiff_scratch;
+    bool attr_sym64_det = false, attr_sym64_2v_det = false;
     Buf sym_acc, sym_tpart, sym_ticket;   // symmetric pair kernel: in-place source sums, target segments, unit tickets
     // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
     bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {}, attr_mma2v[LD_MAX_NQ + 1] = {};
@@ -109,7 +115,7 @@ struct landau_ctx {
     struct StepGraph {
         cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
         unsigned long long gen = 0; int64_t N = 0; int npm = 0, max_iter = 0, fixed_nodes = 0, body_nodes = 0;
-        double dt = 0.0, tol = 0.0, mixed = 0.0; int ek = 0, pk = 0, solver = 0, depth = 0; bool failed = false;
+        double dt = 0.0, tol = 0.0, mixed = 0.0, stiff = 0.0; int ek = 0, pk = 0, solver = 0, depth = 0; bool failed = false;
     } sg;
     Buf dg_u, dg_Gu, dg_Gk, dg_part;      // discrete-gradient step (step_dg.cuh)
     int64_t launches = 0;
@@ -136,7 +142,7 @@ constexpr size_t PIN_BYTES = 1 << 16;
 // pinned read-back area: [0, 8) finish()'s {err, used_fact}; [PIN_CTRL, +sizeof(StepCtrl)) the step control block;
 // [PIN_MOM, ...) per-species moment sums
 constexpr size_t PIN_CTRL = 128, PIN_MOM = 512;
-static_assert(PIN_CTRL >= 2 * sizeof(int) && PIN_CTRL + 64 + 16 <= PIN_MOM && sizeof(StepCtrl) <= 64,
+static_assert(PIN_CTRL >= 2 * sizeof(int) && PIN_CTRL + 96 + 16 <= PIN_MOM && sizeof(StepCtrl) <= 64,
               "pinned read-back areas overlap");
 static_assert(PIN_MOM + sizeof(double) * LD_MAX_SPECIES * 16 <= PIN_BYTES, "pinned read-back area too small");
 
@@ -324,8 +330,9 @@ int npad_upper(int64_t N, int S, int pad) {
 // ---- optimised kernels -----------------------------------------------------------------------
 int pair_sym_available(landau_ctx* c, Cloud& cl) { (void)c; return cl.sym; }
 // mixed-precision implicit step: Jacobi solver, 3-V, symmetric kernel (>= 16384 markers)
+bool stiff_active(const landau_ctx* c) { return c->stiff_theta > 0.0 && c->solver != 2; }
 bool mixed_step_active(const landau_ctx* c, const Cloud& cl) {
-    return c->mixed_until > 0.0 && c->solver == 0 && c->dim == 3 && cl.sym && c->precision == 0;
+    return c->mixed_until > 0.0 && c->solver == 0 && c->dim == 3 && cl.sym && c->precision == 0 && !stiff_active(c);
 }
 // Buffers of the symmetric kernel's output path (pair_sym.cuh): O(N), whatever the grid.
 int ensure_sym_buffers(landau_ctx* c, const Cloud& cl, int G) {
@@ -337,27 +344,27 @@ int ensure_sym_buffers(landau_ctx* c, const Cloud& cl, int G) {
     return 0;
 }
 
-template <typename F, int DIM = 3>
+template <typename F, int DIM = 3, bool DETECT = false>
 int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa, bool& attr_done, int* nparts,
-                    int only_if_f32 = -1) {
+                    int gate = GATE_NONE) {
     using Cfg = SymCfg<SYM_W, SYM_RT, SYM_RS, F>;
     const int G = c->sm_count;                 // persistent grid, 1 CTA per SM: all CTAs co-resident (ticket waits)
     RC(ensure_sym_buffers(c, cl, G));
-    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, F, DIM>;
+    auto kern = pair_sym_kernel<SYM_W, SYM_RT, SYM_RS, F, DIM, DETECT>;
     if (!attr_done) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         attr_done = true;
     }
     const int npm = cl.npad_max;
     sym_reset_kernel<<<c->sm_count, 256, 0, c->stream>>>(ctrl, (double*)c->sym_acc.p, 3 * (size_t)npm,
-                                                          (int*)c->sym_ticket.p, npm / SymL::BS + 1, only_if_f32);
+                                                          (int*)c->sym_ticket.p, npm / SymL::BS + 1, gate);
     kern<<<G, Cfg::THREADS, Cfg::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, npm, soa, (double*)c->sym_acc.p,
                                                     (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err,
-                                                    only_if_f32);
+                                                    gate, c->d_stiff, (int*)c->stiff_mark.p);
     sym_combine_kernel<<<ceil_div(npm, 256), 256, 0, c->stream>>>(cl.L(), ctrl, npm, G, SymL::BT, SymL::BS,
                                                                    (const double*)c->sym_acc.p,
                                                                    (const double*)c->sym_tpart.p, (double*)c->vpart.p,
-                                                                   only_if_f32);
+                                                                   gate);
     c->launches += 3;
     *nparts = 1;
     return 0;
@@ -557,7 +564,9 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
 
 // ---- a3: pairwise field of source records -> partial fields ---------------------------------
 // Returns the number of partial slices written to c->vpart (to be summed in index order).
-int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
+// detect: 0 = plain evaluation; 1 = this is the first evaluation of a step with the stiff-pair treatment on (find
+// the pairs); 2 = enqueue both flavours, gated on the device by the iteration count (CUDA-graph body)
+int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out, int detect = 0) {
     NvtxRange nvtx("landau:a3 pass 2 (pairwise Landau sum)");
     int use_sym = 0;
     if (c->pair_kernel == 2 || c->pair_kernel == 0) use_sym = pair_sym_available(c, cl);
@@ -574,17 +583,20 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
         c->launches += 1;
         c->k_pair = "sym_mixed";
         snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
-        RC(launch_pair_sym<float>(c, cl, ctrl, (const float*)c->soa32.p, c->attr_sym32, nparts_out, 1));
-        RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out, 0));
+        RC(launch_pair_sym<float>(c, cl, ctrl, (const float*)c->soa32.p, c->attr_sym32, nparts_out, GATE_F32));
+        RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out, GATE_F64));
         return 0;
     }
     if (use_sym && !fp32_field) {
+        const int g_det = detect == 2 ? GATE_FIRST : GATE_NONE, g_plain = detect == 2 ? GATE_LATER : GATE_NONE;
         if (c->dim == 2) {                     // native 2-V arithmetic (landau_set_dimension(2))
             c->k_pair = "sym2v";
             snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
-            RC((launch_pair_sym<double, 2>(c, cl, ctrl, cl.soas(), c->attr_sym64_2v, nparts_out)));
+            if (detect) RC((launch_pair_sym<double, 2, true>(c, cl, ctrl, cl.soas(), c->attr_sym64_2v_det, nparts_out, g_det)));
+            if (detect != 1) RC((launch_pair_sym<double, 2>(c, cl, ctrl, cl.soas(), c->attr_sym64_2v, nparts_out, g_plain)));
         } else {
-            RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out));
+            if (detect) RC((launch_pair_sym<double, 3, true>(c, cl, ctrl, cl.soas(), c->attr_sym64_det, nparts_out, g_det)));
+            if (detect != 1) RC(launch_pair_sym<double>(c, cl, ctrl, cl.soas(), c->attr_sym64, nparts_out, g_plain));
         }
         return 0;
     }
@@ -625,6 +637,28 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out) {
     nchunks = std::min(nchunks, 32);
     RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
     dim3 grid(ttiles, nchunks);
+    if (detect) {
+        // stiff-pair steps (landau_set_stiff_pairs): the first evaluation of a step also finds the stiff pairs
+        const int g_det = detect == 2 ? GATE_FIRST : GATE_NONE;
+        StiffCtrl* sc = c->d_stiff;
+        int* mk = (int*)c->stiff_mark.p;
+        double* vp = (double*)c->vpart.p;
+#define LD_ONESIDED(RR, DD, DET, GATE) pair_onesided_kernel<RR, DD, DET><<<grid, PAIR_THREADS, 0, c->stream>>>( \
+            c->d_tab, cl.L(), ctrl, cl.npad_max, nchunks, cl.recs(), vp, GATE, sc, mk)
+        if (c->dim == 2) { if (R == 1) LD_ONESIDED(1, 2, true, g_det); else LD_ONESIDED(2, 2, true, g_det); }
+        else             { if (R == 1) LD_ONESIDED(1, 3, true, g_det); else LD_ONESIDED(2, 3, true, g_det); }
+        c->launches += 1;
+        if (detect == 2) {
+            if (c->dim == 2) { if (R == 1) LD_ONESIDED(1, 2, false, GATE_LATER); else LD_ONESIDED(2, 2, false, GATE_LATER); }
+            else             { if (R == 1) LD_ONESIDED(1, 3, false, GATE_LATER); else LD_ONESIDED(2, 3, false, GATE_LATER); }
+            c->launches += 1;
+        }
+#undef LD_ONESIDED
+        c->k_pair = c->dim == 2 ? "onesided2v" : "onesided";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+        *nparts_out = nchunks;
+        return 0;
+    }
     if (c->dim == 2) {                         // native 2-V arithmetic (landau_set_dimension(2))
         c->k_pair = "onesided2v";
         snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
@@ -806,6 +840,13 @@ int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b) {
         nk_begin_kernel<<<1, 32, 0, st>>>(c->d_nk, c->nk_m);
         c->launches += 1;
     }
+    if (stiff_active(c)) {
+        double* scr = (double*)c->stiff_scratch.p;
+        stiff_begin_kernel<<<c->S, 256, 0, st>>>(c->d_tab, cl.L(), c->d_stiff, (int*)c->stiff_mark.p, b.npm, c->stiff_dt,
+                                                 c->stiff_theta, cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), scr,
+                                                 (unsigned int*)(scr + 2 * LD_MAX_SPECIES));
+        c->launches += 1;
+    }
     return 0;
 }
 
@@ -824,8 +865,15 @@ int enqueue_step_iteration(landau_ctx* c, Cloud& cl, const StepBufs& b, double d
                                                                b.xk, b.yk, b.zk, b.hist, rec, soa);
         c->launches += 1;
     }
-    RC(pair(c, cl, c->d_ctrl, &nparts));
+    const bool stiff = stiff_active(c);
+    RC(pair(c, cl, c->d_ctrl, &nparts, !stiff ? 0 : (cond ? 2 : (first ? 1 : 0))));
     st = c->stream;
+    if (stiff) {
+        stiff_fix_kernel<<<STIFF_CAP / 128, 128, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, c->d_stiff, (const int*)c->stiff_mark.p,
+                                                         npm, nparts, dt, cl.x(), cl.y(), cl.z(), rec, soa,
+                                                         (double*)c->vpart.p);
+        c->launches += 1;
+    }
     if (c->solver == 0) {
         step_update_kernel<<<b.nub, UPD_THREADS, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, npm, nparts, dt, tol, max_iter,
                                                            (const double*)c->vpart.p, cl.x(), cl.y(), cl.z(), cl.w(),
@@ -887,7 +935,7 @@ bool step_graph_matches(const landau_ctx* c, const Cloud& cl, double dt, double 
     const auto& g = c->sg;
     return g.exec && g.gen == c->alloc_gen && g.N == cl.N && g.npm == cl.npad_max && g.dt == dt && g.tol == tol &&
            g.max_iter == max_iter && g.ek == c->entropy_kernel && g.pk == c->pair_kernel && g.solver == c->solver &&
-           g.mixed == c->mixed_until &&
+           g.mixed == c->mixed_until && g.stiff == c->stiff_theta &&
            g.depth == (c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0);
 }
 
@@ -977,7 +1025,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
     g.graph = graph; g.exec = exec; g.gen = c->alloc_gen; g.N = cl.N; g.npm = npm; g.dt = dt; g.tol = tol;
     g.max_iter = max_iter; g.ek = c->entropy_kernel; g.pk = c->pair_kernel; g.fixed_nodes = fixed; g.body_nodes = body_nodes;
     g.solver = c->solver; g.depth = c->solver == 1 ? c->aa_depth : c->solver == 2 ? c->nk_m : 0;
-    g.mixed = c->mixed_until;
+    g.mixed = c->mixed_until; g.stiff = c->stiff_theta;
     return 0;
 }
 }  // namespace
@@ -1075,6 +1123,8 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     if (cudaMalloc(&c->d_aa, sizeof(AndersonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_nk, sizeof(NewtonCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_dg, sizeof(DgCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMalloc(&c->d_stiff, sizeof(StiffCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
+    if (cudaMemset(c->d_stiff, 0, sizeof(StiffCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cutstats, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMemset(c->d_cutstats, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_momout, sizeof(double) * LD_MAX_SPECIES * MOM_OUT) != cudaSuccess) return bail(LANDAU_ECUDA);
@@ -1096,6 +1146,7 @@ void landau_destroy(landau_ctx* c) {
     if (c->d_aa) cudaFree(c->d_aa);
     if (c->d_nk) cudaFree(c->d_nk);
     if (c->d_dg) cudaFree(c->d_dg);
+    if (c->d_stiff) cudaFree(c->d_stiff);
     if (c->d_cutstats) cudaFree(c->d_cutstats);
     destroy_step_graph(c);
     if (c->body_stream) cudaStreamDestroy(c->body_stream);
@@ -1109,7 +1160,7 @@ void landau_destroy(landau_ctx* c) {
                    &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
                    &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32, &c->sym_acc,
                    &c->sym_tpart, &c->sym_ticket, &c->tilebox, &c->cellkey,
-                   &c->cellrank, &c->chunkcnt, &c->binoff, &c->spbox})
+                   &c->cellrank, &c->chunkcnt, &c->binoff, &c->spbox, &c->stiff_mark, &c->stiff_scratch})
         release(*b);
     delete c;
 }
@@ -1242,6 +1293,14 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
     const int nub = ceil_div(npm, UPD_THREADS);
     RC(ensure(c, c->blockpart, sizeof(double) * (size_t)step_blockpart_doubles(c, nub)));
     if (c->solver != 0) RC(ensure(c, c->aa_hist, sizeof(double) * step_hist_doubles(c, npm)));
+    if (stiff_active(c)) {
+        RC(ensure(c, c->stiff_mark, sizeof(int) * (size_t)npm));
+        if (!c->stiff_scratch.p) {
+            RC(ensure(c, c->stiff_scratch, sizeof(double) * (2 * LD_MAX_SPECIES + 2)));
+            CU(cudaMemsetAsync(c->stiff_scratch.p, 0, sizeof(double) * (2 * LD_MAX_SPECIES + 2), c->stream));
+        }
+        c->stiff_dt = dt;
+    }
     const StepBufs sb = step_bufs(c, cl);
     cudaStream_t st = c->stream;
     CU(cudaMemsetAsync(c->d_cursor, 0, sizeof(int), st));
@@ -1351,6 +1410,25 @@ int landau_set_substep(landau_ctx* c, int max_halvings) {
     if (!c) return LANDAU_EINVAL;
     if (max_halvings < 0 || max_halvings > 10) return fail(c, LANDAU_EINVAL, "set_substep: max_halvings must be 0..10");
     c->substep = max_halvings;
+    return 0;
+}
+
+int landau_set_stiff_pairs(landau_ctx* c, double theta) {
+    if (!c) return LANDAU_EINVAL;
+    if (!(theta >= 0.0) || !isfinite(theta))
+        return fail(c, LANDAU_EINVAL, "set_stiff_pairs: the stiffness threshold must be >= 0 (0 = off)");
+    c->stiff_theta = theta;
+    return 0;
+}
+
+int landau_stiff_pairs_last(landau_ctx* c, int* n_pairs, int* n_skipped) {
+    if (!c) return LANDAU_EINVAL;
+    DevGuard dev_guard(c);
+    int* h = (int*)((char*)c->h_pin + PIN_CTRL + 96);
+    CU(cudaMemcpyAsync(h, c->d_stiff, 4 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (n_pairs) *n_pairs = h[0] < STIFF_CAP ? h[0] : STIFF_CAP;
+    if (n_skipped) *n_skipped = h[2] + h[3] + (h[1] ? 1 : 0);
     return 0;
 }
 

@@ -10,6 +10,7 @@
 // (action-reaction) kernel is in pair_sym.cuh.
 #pragma once
 #include "common.cuh"
+#include "stiff_pairs.cuh"
 
 namespace landau {
 
@@ -46,12 +47,14 @@ __device__ __forceinline__ void pair_accumulate2(double zx, double zy, double cx
 // grid = (target tiles, source chunks).  Each thread owns R targets (slots tile*128R + r*128 + tid).
 // Partial fields are written chunk-major: vpart[((chunk*3 + d) * npad_max) + slot], already scaled
 // by nu_ss'/m_s, so that the combine step is a fixed-order sum over chunks.
-template <int R, int DIM = 3>
+template <int R, int DIM = 3, bool DETECT = false>
 __global__ void __launch_bounds__(PAIR_THREADS)
 pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                      const StepCtrl* __restrict__ ctrl, int npad_max, int nchunks,
-                     const double* __restrict__ rec, double* __restrict__ vpart) {
+                     const double* __restrict__ rec, double* __restrict__ vpart, int gate = GATE_NONE,
+                     StiffCtrl* stiff = nullptr, int* stiff_mark = nullptr) {
     if (ctrl && ctrl->done) return;
+    if (gate_closed(ctrl, gate)) return;
     const int npad = L->npad;
     const int slot0 = blockIdx.x * (PAIR_THREADS * R);
     if (slot0 >= npad) return;
@@ -61,15 +64,16 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
     for (int i = threadIdx.x; i < S * S; i += PAIR_THREADS) s_nu[i] = T->nu[i];
 
     double px[R], py[R], pz[R], gx[R], gy[R], gz[R];
-    double tx[R], ty[R], tz[R];
-    int sp[R];
+    double tx[R], ty[R], tz[R], pw[R];
+    int sp[R], ps[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         int p = slot0 + r * PAIR_THREADS + threadIdx.x;
+        ps[r] = p < npad ? p : -1;
         if (p >= npad) p = npad - 1;              // clamped duplicate; its result is not written
         const double2* rp = reinterpret_cast<const double2*>(rec + (size_t)p * 8);
         const double2 a = rp[0], b = rp[1], c = rp[2], d = rp[3];
-        px[r] = a.x; py[r] = a.y; pz[r] = b.x;    // (the weight b.y is not needed for a target)
+        px[r] = a.x; py[r] = a.y; pz[r] = b.x; pw[r] = b.y;   // (the weight is only used by the stiff-pair detection)
         gx[r] = c.x; gy[r] = c.y; gz[r] = d.x;
         tx[r] = ty[r] = tz[r] = 0.0;
         sp[r] = species_of_slot(L, S, p);
@@ -97,6 +101,17 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
             const double2 a = q[0], b = q[1], c = q[2], d = q[3];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
+                if (DETECT) {
+                    // first evaluation of a step: stiff pairs (stiff_pairs.cuh); every pair is seen from both sides
+                    const double zx = px[r] - a.x, zy = py[r] - a.y, zz = pz[r] - b.x;
+                    const double r2 = fma(zz, zz, fma(zy, zy, zx * zx));
+                    const int q = t * PAIR_SRC_TILE + j;
+                    if (r2 < stiff->thr2[sp[r] * S + sb] && ps[r] >= 0 && ps[r] < q) {
+                        const double nu = s_nu[sp[r] * S + sb];
+                        stiff_candidate(stiff, stiff_mark, ps[r], q, r2, gx[r] - c.x, gy[r] - c.y, gz[r] - d.x, nu * b.y,
+                                        nu * pw[r], T->inv_mass[sp[r]], T->inv_mass[sb]);
+                    }
+                }
                 if (DIM == 3)
                     pair_accumulate(px[r] - a.x, py[r] - a.y, pz[r] - b.x, gx[r] - c.x, gy[r] - c.y,
                                     gz[r] - d.x, b.y, ax[r], ay[r], az[r]);

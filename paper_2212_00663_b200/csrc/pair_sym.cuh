@@ -41,6 +41,7 @@
 //   tile's segments in CTA order into ONE field slice [3][npad_max] for the update / combine kernels.
 #pragma once
 #include "common.cuh"
+#include "stiff_pairs.cuh"
 
 namespace landau {
 
@@ -118,14 +119,21 @@ template <> struct SymVec2<float> { using type = float2; };
 // DIM = 2: the paper's 2-V setting (v_z = 0, g_z = 0; landau_set_dimension(2)): the z components of z, g_p - g_q and
 // of both accumulators are identically zero and are not computed -- 22 instead of 30 FP64 instructions per unordered
 // pair, results bit-identical to the 3-V arithmetic on v_z = 0 data (fma(0, 0, x) = x).
-template <bool SYM, int RT, int RS, typename F, int DIM>
+// What the detection variant of the kernel (first pass-2 evaluation of a step, stiff_pairs.cuh) hands to sym_step.
+struct StiffDetect {
+    StiffCtrl* sc; int* mark;
+    double thr2, im_p, im_q;
+    int tslot, sslot;            // slot of target r = 0 (targets are 32 apart) and of source s = 0
+};
+
+template <bool SYM, int RT, int RS, typename F, int DIM, bool DETECT = false>
 __device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], const F (&pz)[RT],
                                          const F (&gx)[RT], const F (&gy)[RT], const F (&gz)[RT],
                                          const F (&wp)[RT], F (&ax)[RT], F (&ay)[RT],
                                          F (&az)[RT], const F (&qx)[RS], const F (&qy)[RS],
                                          const F (&qz)[RS], const F (&hx)[RS], const F (&hy)[RS],
                                          const F (&hz)[RS], const F (&wq)[RS], F (&bx)[RS],
-                                         F (&by)[RS], F (&bz)[RS]) {
+                                         F (&by)[RS], F (&bz)[RS], const StiffDetect* det = nullptr) {
 #pragma unroll
     for (int s = 0; s < RS; ++s) {
 #pragma unroll
@@ -137,6 +145,14 @@ __device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], c
             if (DIM == 3) {
                 zz = pz[r] - qz[s]; cz = gz[r] - hz[s];
                 r2 = sym_fma(zz, zz, r2); d = sym_fma(zz, cz, d);
+            }
+            if (DETECT) {
+                if ((double)r2 < det->thr2) {
+                    const int pp = det->tslot + 32 * r, qq = det->sslot + s;
+                    if (SYM || pp < qq)             // a diagonal task sees every pair from both sides
+                        stiff_candidate(det->sc, det->mark, pp, qq, (double)r2, (double)cx, (double)cy, (double)cz,
+                                        (double)wq[s], (double)wp[r], det->im_p, det->im_q);
+                }
             }
             const F yv = rsqrt_or_zero(r2);
             const F h = d * (yv * yv);
@@ -154,15 +170,16 @@ __device__ __forceinline__ void sym_step(const F (&px)[RT], const F (&py)[RT], c
     }
 }
 
-template <int W, int RT, int RS, typename F = double, int DIM = 3>
+template <int W, int RT, int RS, typename F = double, int DIM = 3, bool DETECT = false>
 __global__ void __launch_bounds__(W * 32, 1)
 pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                 const StepCtrl* __restrict__ ctrl, int npad_max, const F* __restrict__ soa,
-                double* acc, double* __restrict__ tpart, int* ticket, int* errflag, int only_if_f32 = -1) {
+                double* acc, double* __restrict__ tpart, int* ticket, int* errflag, int gate = GATE_NONE,
+                StiffCtrl* stiff = nullptr, int* stiff_mark = nullptr) {
     using C = SymCfg<W, RT, RS, F>;
     using F2 = typename SymVec2<F>::type;
     if (ctrl && ctrl->done) return;
-    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;     // mixed-precision step: the other kernel runs
+    if (gate_closed(ctrl, gate)) return;      // mixed-precision / stiff-pair steps: the alternative kernel runs
     extern __shared__ __align__(128) unsigned char smem_raw[];
     F* s_src = reinterpret_cast<F*>(smem_raw);                        // [2][NCOMP][BS]
     F* s_acc = s_src + 2 * C::NCOMP * C::BS;                          // [3][BS]
@@ -274,6 +291,12 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         __syncthreads();
 
         const F* sx = s_src + (size_t)stage * C::NCOMP * C::BS;
+        StiffDetect det;
+        if (DETECT) {
+            det.sc = stiff; det.mark = stiff_mark; det.thr2 = stiff->thr2[sI * S + sJ];
+            det.im_p = s_im[sI]; det.im_q = s_im[sJ];
+            det.tslot = I * C::BT + wv * 32 * RT + lane;
+        }
         for (int ph = 0; ph < W; ++ph) {
             const int base = ((wv + ph) % W) * C::SUB;
 #pragma unroll 1
@@ -308,8 +331,10 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                         hz[s] = DIM == 3 ? sx[6 * C::BS + g + s] : F(0);
                     }
                 }
+                if (DETECT) det.sslot = j * C::BS + g;
                 if (diag) {
-                    sym_step<false, RT, RS, F, DIM>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<false, RT, RS, F, DIM, DETECT>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw,
+                                                            bx, by, bz, &det);
                 } else {
                     // the source-side sums live in shared memory next to their sources: in this phase the sub-tile is
                     // this warp's alone and at step k every lane holds another group, so the read-modify-write is
@@ -332,7 +357,8 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                             bz[s] = DIM == 3 ? s_acc[2 * C::BS + g + s] : F(0);
                         }
                     }
-                    sym_step<true, RT, RS, F, DIM>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    sym_step<true, RT, RS, F, DIM, DETECT>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw,
+                                                           bx, by, bz, &det);
                     if (RS % 2 == 0) {
 #pragma unroll
                         for (int s = 0; s < RS; s += 2) {
@@ -382,9 +408,9 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
 // Before a launch of pair_sym_kernel: zero the in-place source-side accumulator and the per-unit tickets
 // (skipped, like every kernel of an iteration, once the step is done).
 __global__ void sym_reset_kernel(const StepCtrl* __restrict__ ctrl, double* __restrict__ acc, size_t n,
-                                 int* __restrict__ ticket, int nticket, int only_if_f32 = -1) {
+                                 int* __restrict__ ticket, int nticket, int gate = GATE_NONE) {
     if (ctrl && ctrl->done) return;
-    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;
+    if (gate_closed(ctrl, gate)) return;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (size_t i = i0; i < n; i += stride) acc[i] = 0.0;
@@ -395,9 +421,9 @@ __global__ void sym_reset_kernel(const StepCtrl* __restrict__ ctrl, double* __re
 // the slot's tile, added in CTA order (the CTAs whose runs of tasks meet the tile's row).  G = grid of the pair kernel.
 __global__ void sym_combine_kernel(const DevLayout* __restrict__ L, const StepCtrl* __restrict__ ctrl, int npad_max,
                                    int G, int BT, int BS, const double* __restrict__ acc,
-                                   const double* __restrict__ tpart, double* __restrict__ out, int only_if_f32 = -1) {
+                                   const double* __restrict__ tpart, double* __restrict__ out, int gate = GATE_NONE) {
     if (ctrl && ctrl->done) return;
-    if (ctrl && only_if_f32 >= 0 && ctrl->use_f32 != only_if_f32) return;
+    if (gate_closed(ctrl, gate)) return;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npad_max) return;
     const size_t np = (size_t)npad_max;

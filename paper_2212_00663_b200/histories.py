@@ -35,7 +35,7 @@ def _kurtosis(mass, n, P, stress, m4):
 
 
 def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1, verbose: bool = False,
-                solver: int = 0, depth: int = 3, substep: int = 0, n_q=None, max_iter=None):
+                solver: int = 0, depth: int = 3, substep: int = 0, n_q=None, max_iter=None, stiff: float = 0.0):
     wl = W.make(config, n_per_species=n_per_species)
     if n_q is not None:
         wl.n_q = int(n_q)
@@ -47,8 +47,11 @@ def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1,
         g.set_solver(solver, depth)
     if substep:
         g.set_substep(substep)
+    if stiff:
+        g.set_stiff_pairs(stiff)
     g.set_markers(wl.v, wl.w, wl.species_id)
     S = wl.n_species
+    stiff_pairs = []
     cols = dict(t=[], iterations=[], residual=[], converged=[], K=[], S_eps=[], T=[], T_axis=[], kurt=[], P=[])
 
     def sample(t, info):
@@ -68,6 +71,8 @@ def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1,
     for k in range(n_steps):
         rc, it, res, conv = g.step(wl.dt, wl.tol, wl.max_iter)
         not_conv += 0 if conv else 1
+        if stiff:
+            stiff_pairs.append(g.stiff_pairs_last()[0])
         sample((k + 1) * wl.dt, (it, res, conv))
         if verbose and (k + 1) % 50 == 0:
             print(f"  step {k + 1}/{n_steps}: {it} iterations, T = {cols['T'][-1]}", flush=True)
@@ -81,7 +86,9 @@ def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1,
                    solver={0: "jacobi", 1: f"anderson depth {depth}", 2: f"newton-krylov restart {depth}"}[solver],
                    substep_levels=substep, wall_s=wall,
                    steps_per_s=n_steps / wall, iterations_mean=float(H["iterations"][1:].mean()),
-                   pass2_evaluations_total=int(H["iterations"][1:].sum()), max_iter=wl.max_iter,
+                   pass2_evaluations_total=int(H["iterations"][1:].sum()), max_iter=wl.max_iter, stiff_theta=stiff,
+                   stiff_pairs_per_step_max=int(max(stiff_pairs)) if stiff_pairs else 0,
+                   steps_with_stiff_pairs=int(sum(1 for x in stiff_pairs if x > 0)),
                    iterations_max=int(H["iterations"].max()), steps_not_converged=not_conv,
                    energy_drift_rel_max=float(np.abs(K - K[0]).max() / K[0]),
                    energy_drift_rel_per_step_max=float(np.abs(np.diff(K)).max() / K[0]),
@@ -137,13 +144,15 @@ def main():
     ap.add_argument("--newton-restart", type=int, default=20)
     ap.add_argument("--n-q", type=int, default=None, help="Gauss-Hermite knots per axis (default: the workload's, 4)")
     ap.add_argument("--max-iter", type=int, default=None)
+    ap.add_argument("--stiff", type=float, default=0.0,
+                    help="landau_set_stiff_pairs threshold (0 = off): stiff two-marker interactions solved implicitly")
     ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
     ap.add_argument("--tag", default="", help="suffix of the output file names")
     args = ap.parse_args()
     solver = {"jacobi": 0, "anderson": 1, "newton": 2}[args.solver]
     wl, H, summary = run_history(args.config, args.n_per_species, args.steps, verbose=True, solver=solver,
                                  depth=args.newton_restart if solver == 2 else args.anderson_depth,
-                                 substep=args.substep, n_q=args.n_q, max_iter=args.max_iter)
+                                 substep=args.substep, n_q=args.n_q, max_iter=args.max_iter, stiff=args.stiff)
     write(Path(args.out), f"{args.config}{args.tag}", H, summary)
     print(json.dumps(summary))
 

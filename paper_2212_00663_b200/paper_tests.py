@@ -43,15 +43,18 @@ def _sample_plan(n_steps: int):
 
 
 def run(test: int, n_grid: int = 32, steps=None, solver: int = 0, depth: int = 3, verbose: bool = False,
-        substep: int = 0, max_iter=None):
+        substep: int = 0, max_iter=None, native_2v: bool = True, stiff: float = 0.0):
     wl = W.paper_test(test, n_grid, n_steps=steps)
     if max_iter is not None:
         wl.max_iter = int(max_iter)
     t0, v0, T0 = wl.notes["t0_seconds"], wl.notes["v0_m_per_s"], wl.notes["T0_eV"]
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
-    g.set_dimension(2)
+    if native_2v:
+        g.set_dimension(2)
     if substep:
         g.set_substep(substep)
+    if stiff:
+        g.set_stiff_pairs(stiff)
     if solver:
         g.set_solver(solver, depth)
     g.set_markers(wl.v, wl.w, wl.species_id)
@@ -86,7 +89,8 @@ def run(test: int, n_grid: int = 32, steps=None, solver: int = 0, depth: int = 3
     out = dict(test=test, name=wl.name, n_grid=n_grid, n_markers=wl.n_markers, steps=wl.n_steps,
                dt_seconds=wl.dt * t0, t_end_seconds=float(t[-1]), t0_seconds=t0, eps=wl.eps.tolist(),
                solver={0: "jacobi", 1: f"anderson depth {depth}", 2: f"newton-krylov restart {depth}"}[solver],
-               max_iter=wl.max_iter, substep_levels=substep, wall_s=wall,
+               max_iter=wl.max_iter, substep_levels=substep, wall_s=wall, kernels=g.last_kernels(),
+               two_v_kernels=bool(native_2v), stiff_theta=stiff,
                steps_per_s=wl.n_steps / wall, iterations_mean=float(np.mean(iters)), iterations_max=int(np.max(iters)),
                steps_not_converged=int(notconv), energy_error_rel_max=float(np.abs(K - K[0]).max() / K[0]),
                momentum_error_rel_max=float(np.abs(Pt - Pt[0]).max() / wm_abs),
@@ -144,6 +148,10 @@ def main():
     ap.add_argument("--anderson-depth", type=int, default=3)
     ap.add_argument("--newton-restart", type=int, default=20)
     ap.add_argument("--max-iter", type=int, default=None)
+    ap.add_argument("--stiff", type=float, default=0.0,
+                    help="landau_set_stiff_pairs threshold (0 = off): stiff two-marker interactions solved implicitly")
+    ap.add_argument("--three-v-kernels", action="store_true",
+                    help="run the v_z = 0 data through the 3-V kernels (no landau_set_dimension(2)), for timing comparisons")
     ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
     ap.add_argument("--out", default="gpurun_out")
     ap.add_argument("--tag", default="")
@@ -151,7 +159,7 @@ def main():
     solver = {"jacobi": 0, "anderson": 1, "newton": 2}[args.solver]
     wl, H, out = run(args.test, args.n_grid, args.steps, solver,
                      args.newton_restart if solver == 2 else args.anderson_depth, verbose=True, substep=args.substep,
-                     max_iter=args.max_iter)
+                     max_iter=args.max_iter, native_2v=not args.three_v_kernels, stiff=args.stiff)
     write(Path(args.out), args.test, H, out, args.tag)
     print(json.dumps(out))
 

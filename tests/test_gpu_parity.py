@@ -607,6 +607,94 @@ def test_graph_step_with_accelerated_solvers_is_bit_identical(B, solver, depth, 
     assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: stiff pairs
+def _cloud_with_close_markers(n, offsets, seed=77):
+    """Config-0 cloud in which electrons 1.. are copies of electron 0 displaced by `offsets` (same species, close)."""
+    wl = W.make(0, n_per_species=n, seed=seed)
+    e = np.flatnonzero(wl.species_id == 0)
+    for k, off in enumerate(offsets):
+        wl.v[e[k + 1]] = wl.v[e[0]] + np.asarray(off)
+    return wl
+
+
+@pytest.mark.parametrize("solver,depth", [(0, 0), (1, 5)])
+@pytest.mark.parametrize("offsets", [[(3e-7, 1e-7, -2e-7)], [(3e-7, 1e-7, -2e-7), (-2e-7, 4e-7, 1e-7)]])
+def test_stiff_pairs_are_solved_where_the_plain_iteration_cycles(B, oracle_mod, solver, depth, offsets):
+    """Two (three) electrons within ~4e-7 of each other: the pair term of Eq. (23) is not Lipschitz at z = 0, the
+    Jacobi map of Eq. (24) expands in their relative coordinate and BOTH the oracle's literal iteration and the CUDA
+    path's end at max_iter.  landau_set_stiff_pairs solves those two (three) markers' mutual terms
+    implicitly and exactly inside the iteration: the step converges, and the result satisfies Eq. (24) for EVERY marker
+    when its field is re-evaluated by the ORACLE at the returned midpoint; momentum and energy are conserved."""
+    wl = _cloud_with_close_markers(200, offsets)
+    g, o = make_pair(B, oracle_mod, wl)
+    gp = B.Landau(wl.mass, wl.charge, wl.eps)
+    gp.set_markers(wl.v, wl.w, wl.species_id)
+    o.set_markers(wl.v, wl.w, wl.species_id)
+    rp, ro = gp.step(wl.dt, 1e-12, 60), o.step(wl.dt, 1e-12, 60)
+    assert rp[0] == 1 and ro[0] == 1 and rp[2] > 1e-10 and ro[2] > 1e-10       # the plain iteration cycles on both sides
+    if solver:
+        g.set_solver(solver, depth)
+    g.set_stiff_pairs(0.2)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=False)
+    rc, it, res, conv = g.step(wl.dt, 1e-12, 60)
+    n_pairs, n_skipped = g.stiff_pairs_last()
+    assert rc == 0 and conv and it <= 25, (rc, it, res)
+    assert n_pairs == len(offsets) * (len(offsets) + 1) // 2
+    v1 = g.get_markers().cpu().numpy()
+    G = o.entropy_grad(wl.v, wl.w, wl.species_id)
+    V = o.pair_field(0.5 * (wl.v + v1), wl.w, wl.species_id, G)
+    defect = v1 - wl.v - wl.dt * V
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    assert np.sqrt((wm * defect ** 2).sum() / (wm * v1 ** 2).sum()) <= 2e-12
+    e = np.flatnonzero(wl.species_id == 0)[:len(offsets) + 1]
+    assert np.abs(defect[e]).max() <= 1e-9 * np.abs(v1[e] - wl.v[e]).max()    # the eliminated markers themselves
+    m1 = g.moments(with_entropy=False)
+    wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
+    assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
+    assert abs(m1["K"].sum() - m0["K"].sum()) <= TOL_DRIFT * m0["K"].sum()
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 256), (4, 6000), (1, 3000)])
+def test_stiff_pair_option_changes_nothing_without_stiff_pairs(B, cfg, n):
+    """With no pair above the threshold the option only adds the detection to the first evaluation: bit-identical
+    steps (plain launches and CUDA-graph replay), zero pairs reported."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    ga = B.Landau(wl.mass, wl.charge, wl.eps)
+    gb = B.Landau(wl.mass, wl.charge, wl.eps)
+    gc = B.Landau(wl.mass, wl.charge, wl.eps)
+    gb.set_stiff_pairs(0.2); gb.set_step_graph(0)
+    gc.set_stiff_pairs(0.2); gc.set_step_graph(2)
+    for g in (ga, gb, gc):
+        g.set_markers(wl.v, wl.w, wl.species_id)
+    ra = [ga.step(wl.dt, wl.tol, 50) for _ in range(3)]
+    rb = [gb.step(wl.dt, wl.tol, 50) for _ in range(3)]
+    rcc = [gc.step(wl.dt, wl.tol, 50) for _ in range(3)]
+    assert ra == rb == rcc and gb.stiff_pairs_last() == (0, 0) and gc.stiff_pairs_last() == (0, 0)
+    assert "step=graph" in gc.last_kernels()
+    va = ga.get_markers().cpu().numpy()
+    assert np.array_equal(va, gb.get_markers().cpu().numpy()) and np.array_equal(va, gc.get_markers().cpu().numpy())
+
+
+def test_stiff_pairs_large_cloud_symmetric_kernel(B, oracle_mod):
+    """The detection inside the symmetric kernel (>= 16384 markers): a planted close pair is found and treated, the
+    converged step satisfies Eq. (24) on oracle rows (the planted markers included)."""
+    wl = W.make(3, n_per_species=9000, shuffled=True)
+    e = np.flatnonzero(wl.species_id == 0)
+    wl.v[e[1]] = wl.v[e[0]] + np.array([2e-7, -1e-7, 3e-7])
+    g, o = make_pair(B, oracle_mod, wl)
+    g.set_stiff_pairs(0.2)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = g.step(wl.dt, 1e-12, 60)
+    assert rc == 0 and conv and "pair=sym" in g.last_kernels() and g.stiff_pairs_last()[0] >= 1
+    v1 = g.get_markers().cpu().numpy()
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    rows = np.concatenate([e[:2], np.arange(5, wl.n_markers, 97)]).astype(np.int64)
+    V = o.pair_field_rows(0.5 * (wl.v + v1), wl.w, wl.species_id, G, rows)
+    defect = v1[rows] - wl.v[rows] - wl.dt * V
+    assert np.abs(defect).max() <= 1e-9 * np.abs(v1[rows] - wl.v[rows]).max()
+
+
 # ------------------------------------------------------------------------------------ NEXT-4: Gaussian cutoff of pass 1
 @pytest.mark.parametrize("entropy_kernel", [0, 1])
 @pytest.mark.parametrize("test,n_grid", [(3, 40), (1, 32), (2, 48)])
