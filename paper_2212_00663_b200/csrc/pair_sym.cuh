@@ -119,6 +119,37 @@ template <> struct SymVec2<float> { using type = float2; };
 // DIM = 2: the paper's 2-V setting (v_z = 0, g_z = 0; landau_set_dimension(2)): the z components of z, g_p - g_q and
 // of both accumulators are identically zero and are not computed -- 22 instead of 30 FP64 instructions per unordered
 // pair, results bit-identical to the 3-V arithmetic on v_z = 0 data (fma(0, 0, x) = x).
+// The 3-V step exactly as profiled in profiles/r2_pair_sym_full.md (the generic sym_step below compiles to a slower
+// schedule for DIM = 3: 41.1 ms against 40.0 ms per launch at 3 x 2^16, so the headline instantiation keeps its own text).
+template <bool SYM, int RT, int RS, typename F>
+__device__ __forceinline__ void sym_step3(const F (&px)[RT], const F (&py)[RT], const F (&pz)[RT],
+                                         const F (&gx)[RT], const F (&gy)[RT], const F (&gz)[RT],
+                                         const F (&wp)[RT], F (&ax)[RT], F (&ay)[RT],
+                                         F (&az)[RT], const F (&qx)[RS], const F (&qy)[RS],
+                                         const F (&qz)[RS], const F (&hx)[RS], const F (&hy)[RS],
+                                         const F (&hz)[RS], const F (&wq)[RS], F (&bx)[RS],
+                                         F (&by)[RS], F (&bz)[RS]) {
+#pragma unroll
+    for (int s = 0; s < RS; ++s) {
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const F zx = px[r] - qx[s], zy = py[r] - qy[s], zz = pz[r] - qz[s];
+            const F cx = gx[r] - hx[s], cy = gy[r] - hy[s], cz = gz[r] - hz[s];
+            const F r2 = sym_fma(zz, zz, sym_fma(zy, zy, zx * zx));
+            const F d = sym_fma(zz, cz, sym_fma(zy, cy, zx * cx));
+            const F yv = rsqrt_or_zero(r2);
+            const F h = d * (yv * yv);
+            const F ux = sym_fma(-zx, h, cx), uy = sym_fma(-zy, h, cy), uz = sym_fma(-zz, h, cz);
+            const F a = wq[s] * yv;
+            ax[r] = sym_fma(a, ux, ax[r]); ay[r] = sym_fma(a, uy, ay[r]); az[r] = sym_fma(a, uz, az[r]);
+            if (SYM) {
+                const F b = wp[r] * yv;
+                bx[s] = sym_fma(b, ux, bx[s]); by[s] = sym_fma(b, uy, by[s]); bz[s] = sym_fma(b, uz, bz[s]);
+            }
+        }
+    }
+}
+
 // What the detection variant of the kernel (first pass-2 evaluation of a step, stiff_pairs.cuh) hands to sym_step.
 struct StiffDetect {
     StiffCtrl* sc; int* mark;
@@ -299,6 +330,69 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         }
         for (int ph = 0; ph < W; ++ph) {
             const int base = ((wv + ph) % W) * C::SUB;
+            if (DIM == 3 && !DETECT) {
+#pragma unroll 1
+            for (int k = 0; k < 32; ++k) {
+                const int g = base + ((lane + k) & 31) * RS;
+                F qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS], bx[RS], by[RS], bz[RS];
+                if (RS % 2 == 0) {
+#pragma unroll
+                    for (int s = 0; s < RS; s += 2) {
+                        const F2 a0 = *reinterpret_cast<const F2*>(sx + 0 * C::BS + g + s);
+                        const F2 a1 = *reinterpret_cast<const F2*>(sx + 1 * C::BS + g + s);
+                        const F2 a2 = *reinterpret_cast<const F2*>(sx + 2 * C::BS + g + s);
+                        const F2 a3 = *reinterpret_cast<const F2*>(sx + 3 * C::BS + g + s);
+                        const F2 a4 = *reinterpret_cast<const F2*>(sx + 4 * C::BS + g + s);
+                        const F2 a5 = *reinterpret_cast<const F2*>(sx + 5 * C::BS + g + s);
+                        const F2 a6 = *reinterpret_cast<const F2*>(sx + 6 * C::BS + g + s);
+                        qx[s] = a0.x; qx[s + 1] = a0.y; qy[s] = a1.x; qy[s + 1] = a1.y; qz[s] = a2.x; qz[s + 1] = a2.y;
+                        qw[s] = a3.x * nu; qw[s + 1] = a3.y * nu;
+                        hx[s] = a4.x; hx[s + 1] = a4.y; hy[s] = a5.x; hy[s + 1] = a5.y; hz[s] = a6.x; hz[s + 1] = a6.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int s = 0; s < RS; ++s) {
+                        qx[s] = sx[0 * C::BS + g + s]; qy[s] = sx[1 * C::BS + g + s]; qz[s] = sx[2 * C::BS + g + s];
+                        qw[s] = sx[3 * C::BS + g + s] * nu;
+                        hx[s] = sx[4 * C::BS + g + s]; hy[s] = sx[5 * C::BS + g + s]; hz[s] = sx[6 * C::BS + g + s];
+                    }
+                }
+                if (diag) {
+                    sym_step3<false, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                } else {
+                    // the source-side sums live in shared memory next to their sources: in this phase the sub-tile is
+                    // this warp's alone and at step k every lane holds another group, so the read-modify-write is
+                    // conflict free and ordered by the warp's program order (no shuffles, no atomics)
+                    if (RS % 2 == 0) {
+#pragma unroll
+                        for (int s = 0; s < RS; s += 2) {
+                            const F2 b0 = *reinterpret_cast<const F2*>(s_acc + g + s);
+                            const F2 b1 = *reinterpret_cast<const F2*>(s_acc + C::BS + g + s);
+                            const F2 b2 = *reinterpret_cast<const F2*>(s_acc + 2 * C::BS + g + s);
+                            bx[s] = b0.x; bx[s + 1] = b0.y; by[s] = b1.x; by[s + 1] = b1.y; bz[s] = b2.x; bz[s + 1] = b2.y;
+                        }
+                    } else {
+#pragma unroll
+                        for (int s = 0; s < RS; ++s) { bx[s] = s_acc[g + s]; by[s] = s_acc[C::BS + g + s]; bz[s] = s_acc[2 * C::BS + g + s]; }
+                    }
+                    sym_step3<true, RT, RS, F>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    if (RS % 2 == 0) {
+#pragma unroll
+                        for (int s = 0; s < RS; s += 2) {
+                            F2 b0, b1, b2;
+                            b0.x = bx[s]; b0.y = bx[s + 1]; b1.x = by[s]; b1.y = by[s + 1]; b2.x = bz[s]; b2.y = bz[s + 1];
+                            *reinterpret_cast<F2*>(s_acc + g + s) = b0;
+                            *reinterpret_cast<F2*>(s_acc + C::BS + g + s) = b1;
+                            *reinterpret_cast<F2*>(s_acc + 2 * C::BS + g + s) = b2;
+                        }
+                    } else {
+#pragma unroll
+                        for (int s = 0; s < RS; ++s) { s_acc[g + s] = bx[s]; s_acc[C::BS + g + s] = by[s]; s_acc[2 * C::BS + g + s] = bz[s]; }
+                    }
+                    __syncwarp();
+                }
+            }
+            } else {
 #pragma unroll 1
             for (int k = 0; k < 32; ++k) {
                 const int g = base + ((lane + k) & 31) * RS;
@@ -377,6 +471,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
                     }
                     __syncwarp();
                 }
+            }
             }
             __syncthreads();
         }

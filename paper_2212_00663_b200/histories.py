@@ -35,8 +35,8 @@ def _kurtosis(mass, n, P, stress, m4):
 
 
 def run_history(config: int, n_per_species=None, steps=None, every_ext: int = 1, verbose: bool = False,
-                solver: int = 0, depth: int = 3, substep: int = 0, n_q=None, max_iter=None, stiff: float = 0.0):
-    wl = W.make(config, n_per_species=n_per_species)
+                solver: int = 0, depth: int = 3, substep: int = 0, n_q=None, max_iter=None, stiff: float = 0.0, eps_rule=None):
+    wl = W.make(config, n_per_species=n_per_species, **({} if eps_rule is None else {"eps_rule": float(eps_rule)}))
     if n_q is not None:
         wl.n_q = int(n_q)
     if max_iter is not None:
@@ -144,6 +144,7 @@ def main():
     ap.add_argument("--newton-restart", type=int, default=20)
     ap.add_argument("--n-q", type=int, default=None, help="Gauss-Hermite knots per axis (default: the workload's, 4)")
     ap.add_argument("--max-iter", type=int, default=None)
+    ap.add_argument("--eps-rule", type=float, default=None, help="eps_s = EPS_RULE * T_s/m_s (default 0.05, reading U2)")
     ap.add_argument("--stiff", type=float, default=0.0,
                     help="landau_set_stiff_pairs threshold (0 = off): stiff two-marker interactions solved implicitly")
     ap.add_argument("--substep", type=int, default=0, help="levels of step halving for unconverged steps")
@@ -152,7 +153,7 @@ def main():
     solver = {"jacobi": 0, "anderson": 1, "newton": 2}[args.solver]
     wl, H, summary = run_history(args.config, args.n_per_species, args.steps, verbose=True, solver=solver,
                                  depth=args.newton_restart if solver == 2 else args.anderson_depth,
-                                 substep=args.substep, n_q=args.n_q, max_iter=args.max_iter, stiff=args.stiff)
+                                 substep=args.substep, n_q=args.n_q, max_iter=args.max_iter, stiff=args.stiff, eps_rule=args.eps_rule)
     write(Path(args.out), f"{args.config}{args.tag}", H, summary)
     print(json.dumps(summary))
 
