@@ -39,8 +39,10 @@ struct CellRecord {          // mirrors landau_cell_info (host struct) field by 
 
 template <int NQ>
 struct CellsCfg {
-    // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / ux uy uz (pass 2)
-    static constexpr int DPM = 10 + 3 * NQ;
+    // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / one source record
+    // {ux uy uz w gx gy gz 0} (pass 2; 64 bytes: four LDS.128 per source instead of seven LDS.64)
+    static constexpr int TAB = 3 * NQ > 8 ? 3 * NQ : 8;
+    static constexpr int DPM = 10 + TAB;
     // x-node indices per register slice of the node sums: NI * NQ^2 <= 64 accumulators
     static constexpr int NI = NQ <= 4 ? NQ : 1;
     static_assert(NQ % NI == 0, "slices must tile the x-node indices");
@@ -141,20 +143,19 @@ __device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, doubl
     }
 }
 
-// Pass 2 of NT targets of one thread against every source of the cell (sources read once per NT targets:
-// NT = 2 halves the shared-memory traffic per pair).  t? = sum_s' nu_ss' sum_q w_q Q(u_p - u_q)(g_p - g_q).
+// Pass 2 of NT targets of one thread against every source of the cell (a source record is read once per NT targets:
+// NT = 4 quarters the shared-memory traffic per pair).  t? = sum_s' nu_ss' sum_q w_q Q(u_p - u_q)(g_p - g_q).
+// rec: [n][8] = {ux uy uz w gx gy gz 0}.
 template <int NT>
-__device__ __forceinline__ void cells_field(const double* __restrict__ ux, const double* __restrict__ uy,
-                                            const double* __restrict__ uz, const double* __restrict__ Gx,
-                                            const double* __restrict__ Gy, const double* __restrict__ Gz,
-                                            const double* __restrict__ ww, const int* __restrict__ s_off,
+__device__ __forceinline__ void cells_field(const double* __restrict__ rec, const int* __restrict__ s_off,
                                             const double* __restrict__ s_nu, int S, const int (&pc)[NT],
                                             const int (&sp)[NT], double (&tx)[NT], double (&ty)[NT], double (&tz)[NT]) {
     double px[NT], py[NT], pz[NT], hx[NT], hy[NT], hz[NT];
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
-        px[t] = ux[pc[t]]; py[t] = uy[pc[t]]; pz[t] = uz[pc[t]];
-        hx[t] = Gx[pc[t]]; hy[t] = Gy[pc[t]]; hz[t] = Gz[pc[t]];
+        const double* r = rec + (size_t)pc[t] * 8;
+        px[t] = r[0]; py[t] = r[1]; pz[t] = r[2];
+        hx[t] = r[4]; hy[t] = r[5]; hz[t] = r[6];
         tx[t] = ty[t] = tz[t] = 0.0;
     }
     for (int sb = 0; sb < S; ++sb) {
@@ -164,7 +165,9 @@ __device__ __forceinline__ void cells_field(const double* __restrict__ ux, const
         for (int t = 0; t < NT; ++t) ax[t] = ay[t] = az[t] = 0.0;
 #pragma unroll 4
         for (int q = q0; q < q1; ++q) {
-            const double qx = ux[q], qy = uy[q], qz = uz[q], gx = Gx[q], gy = Gy[q], gz = Gz[q], wq = ww[q];
+            const double2* r2 = reinterpret_cast<const double2*>(rec + (size_t)q * 8);
+            const double2 a = r2[0], b = r2[1], c = r2[2], d = r2[3];
+            const double qx = a.x, qy = a.y, qz = b.x, wq = b.y, gx = c.x, gy = c.y, gz = d.x;
 #pragma unroll
             for (int t = 0; t < NT; ++t)
                 pair_accumulate(px[t] - qx, py[t] - qy, pz[t] - qz, hx[t] - gx, hy[t] - gy, hz[t] - gz, wq, ax[t], ay[t],
@@ -189,9 +192,9 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
     double* yn = xn + cap; double* zn = yn + cap; double* ww = zn + cap;
     double* Gx = ww + cap; double* Gy = Gx + cap; double* Gz = Gy + cap;
     double* xk = Gz + cap; double* yk = xk + cap; double* zk = yk + cap;
-    double* tab = zk + cap;                               // [cap][3 NQ] in pass 1; ux uy uz in pass 2
-    double* ux = tab; double* uy = ux + cap; double* uz = uy + cap;
-    double* s_e2 = tab + (size_t)3 * NQ * cap;            // [64]
+    double* tab = zk + cap;                               // [cap][3 NQ] in pass 1; source records [cap][8] in pass 2
+    double* srec = tab;
+    double* s_e2 = tab + (size_t)CellsCfg<NQ>::TAB * cap; // [64]
     double* s_red = s_e2 + 64;                            // [32]
     double* s_part = s_red + 32;                          // [GF][3][TPG] partial sums of split targets (small cells)
     int* idx = reinterpret_cast<int*>(s_part + 3 * CELLS_THREADS);   // [cap] caller index (within the cell) of slot p
@@ -388,9 +391,12 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     int s = 0;
                     for (int t = 1; t < S; ++t) s += (p >= s_off[t]) ? 1 : 0;
                     sp[r] = s; im[r] = T->inv_mass[s]; wm[r] = ww[p] * T->mass[s];
-                    Gx[p] *= im[r]; Gy[p] *= im[r]; Gz[p] *= im[r];
                     xk[p] = xn[p]; yk[p] = yn[p]; zk[p] = zn[p];
-                    ux[p] = xn[p]; uy[p] = yn[p]; uz[p] = zn[p];
+                    double2* o = reinterpret_cast<double2*>(srec + (size_t)p * 8);
+                    o[0] = make_double2(xn[p], yn[p]);
+                    o[1] = make_double2(zn[p], ww[p]);
+                    o[2] = make_double2(Gx[p] * im[r], Gy[p] * im[r]);
+                    o[3] = make_double2(Gz[p] * im[r], 0.0);
                 }
             }
             __syncthreads();
@@ -417,16 +423,19 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     const int pc = min(tg, n - 1);
                     int spt = 0;
                     for (int t = 1; t < S; ++t) spt += (pc >= s_off[t]) ? 1 : 0;
-                    const double px = ux[pc], py = uy[pc], pz = uz[pc], hx = Gx[pc], hy = Gy[pc], hz = Gz[pc];
+                    const double* rp = srec + (size_t)pc * 8;
+                    const double px = rp[0], py = rp[1], pz = rp[2], hx = rp[4], hy = rp[5], hz = rp[6];
                     double tx = 0.0, ty = 0.0, tz = 0.0;
                     for (int sb = 0; sb < S; ++sb) {
                         const int q0 = s_off[sb], len = s_off[sb + 1] - q0;
                         const int qa = q0 + (len * part) / GF, qb = q0 + (len * (part + 1)) / GF;
                         double ax = 0.0, ay = 0.0, az = 0.0;
 #pragma unroll 4
-                        for (int q = qa; q < qb; ++q)
-                            pair_accumulate(px - ux[q], py - uy[q], pz - uz[q], hx - Gx[q], hy - Gy[q], hz - Gz[q], ww[q],
-                                            ax, ay, az);
+                        for (int q = qa; q < qb; ++q) {
+                            const double2* r2 = reinterpret_cast<const double2*>(srec + (size_t)q * 8);
+                            const double2 a = r2[0], b = r2[1], c = r2[2], d = r2[3];
+                            pair_accumulate(px - a.x, py - a.y, pz - b.x, hx - c.x, hy - c.y, hz - d.x, b.y, ax, ay, az);
+                        }
                         const double nu = s_nu[spt * S + sb];
                         tx = fma(nu, ax, tx); ty = fma(nu, ay, ty); tz = fma(nu, az, tz);
                     }
@@ -443,21 +452,35 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         finish_target(0, a, b, c);
                     }
                 } else
+                {
+                    // all rounds of targets of a thread share every source read (block-uniform branch on the cell size)
+                    static_assert(CELLS_ROUNDS == 4, "one branch per number of rounds");
+                    const int rounds = ceil_div(n, CELLS_THREADS);
+                    int pc4[4], sp4[4];
 #pragma unroll
-                for (int r = 0; r < CELLS_ROUNDS; r += 2) {
-                    if ((r + 1) * CELLS_THREADS < n) {                 // uniform: two rounds of targets share the sources
-                        const int pc[2] = {r * CELLS_THREADS + tid, min((r + 1) * CELLS_THREADS + tid, n - 1)};
-                        const int spc[2] = {sp[r], sp[r + 1]};
+                    for (int r = 0; r < 4; ++r) { pc4[r] = min(r * CELLS_THREADS + tid, n - 1); sp4[r] = sp[r]; }
+                    if (rounds == 4) {
+                        double tx[4], ty[4], tz[4];
+                        cells_field<4>(srec, s_off, s_nu, S, pc4, sp4, tx, ty, tz);
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) finish_target(r, tx[r], ty[r], tz[r]);
+                    } else if (rounds == 3) {
+                        const int pc[3] = {pc4[0], pc4[1], pc4[2]}, spc[3] = {sp4[0], sp4[1], sp4[2]};
+                        double tx[3], ty[3], tz[3];
+                        cells_field<3>(srec, s_off, s_nu, S, pc, spc, tx, ty, tz);
+#pragma unroll
+                        for (int r = 0; r < 3; ++r) finish_target(r, tx[r], ty[r], tz[r]);
+                    } else if (rounds == 2) {
+                        const int pc[2] = {pc4[0], pc4[1]}, spc[2] = {sp4[0], sp4[1]};
                         double tx[2], ty[2], tz[2];
-                        cells_field<2>(ux, uy, uz, Gx, Gy, Gz, ww, s_off, s_nu, S, pc, spc, tx, ty, tz);
-                        finish_target(r, tx[0], ty[0], tz[0]);
-                        finish_target(r + 1, tx[1], ty[1], tz[1]);
-                    } else if (r * CELLS_THREADS < n) {                // uniform: one (partial) round
-                        const int pc[1] = {min(r * CELLS_THREADS + tid, n - 1)};
-                        const int spc[1] = {sp[r]};
+                        cells_field<2>(srec, s_off, s_nu, S, pc, spc, tx, ty, tz);
+                        finish_target(0, tx[0], ty[0], tz[0]);
+                        finish_target(1, tx[1], ty[1], tz[1]);
+                    } else {
+                        const int pc[1] = {pc4[0]}, spc[1] = {sp4[0]};
                         double tx[1], ty[1], tz[1];
-                        cells_field<1>(ux, uy, uz, Gx, Gy, Gz, ww, s_off, s_nu, S, pc, spc, tx, ty, tz);
-                        finish_target(r, tx[0], ty[0], tz[0]);
+                        cells_field<1>(srec, s_off, s_nu, S, pc, spc, tx, ty, tz);
+                        finish_target(0, tx[0], ty[0], tz[0]);
                     }
                 }
                 cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
@@ -466,7 +489,8 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     const int p = r * CELLS_THREADS + tid;
                     if (p < n) {
                         xk[p] = nx[r]; yk[p] = ny[r]; zk[p] = nz[r];
-                        ux[p] = 0.5 * (xn[p] + nx[r]); uy[p] = 0.5 * (yn[p] + ny[r]); uz[p] = 0.5 * (zn[p] + nz[r]);
+                        double* o = srec + (size_t)p * 8;
+                        o[0] = 0.5 * (xn[p] + nx[r]); o[1] = 0.5 * (yn[p] + ny[r]); o[2] = 0.5 * (zn[p] + nz[r]);
                     }
                 }
                 __syncthreads();
