@@ -2,22 +2,25 @@
 //
 // The factorised node sums of entropy_fact.cuh (Eq. (22); 3-V restatement DESIGN.md
 // section 3 D1),
-//     F_p(n) = sum_{q in s} C_pq * P_q(n),   C_pq = w_q exp(-|p' - q'|^2),   P_q(n) = Tx_q(i) Ty_q(j) Tz_q(l),
+//     F_p(n) = sum_{q in s} C_pq * P_q(n),   C_pq = exp(-|p' - q'|^2),   P_q(n) = w_q Tx_q(i) Ty_q(j) Tz_q(l),
 // with n = (i,j,l) a tensor Gauss-Hermite node, ARE a matrix product  F[targets x nodes] = C[targets x sources]
 // * P[sources x nodes]  whose left factor is generated on the fly (one exponential per pair).  This kernel
 // issues it as  mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4):  a warp owns 8*MT targets x NL <= 64 nodes of
 // accumulators in registers; per k-step of 4 sources each lane computes the MT entries C[lane/4 + 8 mt][lane%4]
 // of the A fragments (its own exponentials), reads the NBG entries P[lane%4][8 nb + lane/4] of the B fragments
-// from a per-tile product table in shared memory, and issues MT*NBG DMMAs.  Per pair the FP64 pipe sees
-// 17 vector instructions (|d|^2, exponential, weight) + n_q^3 tensor FMAs, against 108 vector instructions in
+// from the product table in shared memory, and issues MT*NBG DMMAs.  Per pair the FP64 pipe sees
+// 16 vector instructions (|d|^2, exponential) + n_q^3 tensor FMAs, against 108 vector instructions in
 // entropy_fact_kernel; on B200 DMMA and DFMA share one pipe (profiles/r1_entropy_fact_v3_full.md), so the gain
 // is the removed product/issue overhead and DMMA's 12/12 (vs DFMA's 11/12) pipe efficiency, not overlap.
 //
-// Source records {x',y',z',w,Tx[NQ],Ty[NQ],Tz[NQ]} are those of entropy_fact_prep_kernel, staged by TMA bulk
-// copies (double buffered); the block turns each tile of 64 records into the product table
-// s_prod[q][0..NL) = P_q(node0 + .), s_prod[q][64..68) = {x',y',z',w}  (row stride 68 doubles: the B-fragment
-// reads of a half-warp fall into 16 distinct bank pairs), also double buffered, one __syncthreads per tile.
-// Nodes beyond n_q^3 (padding of the last 8-node block) have P = 0 and are not written.
+// The product table is the SAME for every target tile, so it is built once per pass 1 in global memory
+// (entropy_prod_kernel: row of slot q and node group g = { P_q(node0 + 0..NL), x', y', z', 0 }, ROW = NL + 4 doubles,
+// the weight folded into the products) and a tile of 64 rows arrives as ONE TMA bulk copy (double buffered, one
+// __syncthreads per tile).  Round 1-2 built the table inside every block from the per-marker factor records: a serial
+// LDS -> DMUL -> STS chain that took 20 % of every warp's time (profiles/r2_entropy_mma_full.md).  A species' table
+// (544 B per marker at n_q = 4) stays L2 resident while the co-resident blocks stream it.  ROW = NL + 4 is 4 or 12
+// mod 16, so the B-fragment reads of a half-warp fall into 16 distinct bank pairs.
+// Nodes beyond n_q^3 (padding of the last 8-node block) have P = 0.
 // Output layout as the other pass-1 kernels: part[((chunk * M + node) * npad_max) + slot].
 #pragma once
 #include "common.cuh"
@@ -29,7 +32,7 @@ namespace landau {
 constexpr int MMA_THREADS = 128;   // 4 warps, 32 targets each
 constexpr int MMA_TILE = 64;       // sources per stage
 constexpr int MMA_MT = 4;          // 8-target blocks per warp
-constexpr int MMA_ROW = 68;        // doubles per product-table row
+constexpr int MMA_STAGES = 2;      // product-table tiles in shared memory
 constexpr int MMA_LCAP = 1024;     // source tiles per segment of the active-tile list (Gaussian cutoff)
 
 // NZ = NQ: the 3-V tensor grid of n_q^3 nodes.  NZ = 1: the paper's own 2-V setting (landau_set_dimension(2), v_z = 0):
@@ -42,11 +45,42 @@ struct MmaCfg {
     static constexpr int NBG = NB <= 8 ? NB : (NQ == 6 ? 7 : 8);    // blocks per node group (gridDim.z)
     static constexpr int GROUPS = (NB + NBG - 1) / NBG;
     static constexpr int NL = NBG * 8;                              // nodes per group (<= 64)
+    static constexpr int ROW = NL + 4;                              // doubles per product-table row
     static constexpr int REC = FactCfg<NQ>::REC;
+    static constexpr uint32_t TILE_BYTES = MMA_TILE * ROW * (uint32_t)sizeof(double);
     static constexpr size_t SMEM =
-        sizeof(double) * (2 * MMA_TILE * MMA_ROW + 2 * MMA_TILE * REC + 64) + 2 * sizeof(uint64_t) +
+        sizeof(double) * (MMA_STAGES * MMA_TILE * ROW + 64) + MMA_STAGES * sizeof(uint64_t) +
         sizeof(int) * (MMA_LCAP + 8);
+    static size_t table_bytes(size_t npad_max) { return sizeof(double) * ROW * npad_max * GROUPS; }
 };
+
+// Product table of pass 1 (one launch per pass): tab[(g * npad_max + q) * ROW + c] = w_q Tx_q(i) Ty_q(j) Tz_q(l) for
+// node n = g * NL + c = (i, j, l), c < NL (0 beyond n_q^3), then {x', y', z', 0}; from the factor records of
+// entropy_fact_prep_kernel.  Dummies have all-zero rows: as sources they add exactly 0.
+template <int NQ, int NZ>
+__global__ void entropy_prod_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max,
+                                    const double* __restrict__ rec, double* __restrict__ tab,
+                                    const StepCtrl* __restrict__ stop) {
+    if (stop && stop->done) return;
+    using C = MmaCfg<NQ, NZ>;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)npad_max * C::ROW) return;
+    if (!fact_usable(T, L)) return;
+    const int q = (int)(idx / C::ROW), c = (int)(idx - (size_t)q * C::ROW);
+    const double* r = rec + (size_t)q * C::REC;
+    double v = 0.0;
+    if (c < C::NL) {
+        const int nd = blockIdx.y * C::NL + c;
+        if (nd < C::M) {
+            v = r[4 + nd / (NQ * NZ)] * r[4 + NQ + (nd / NZ) % NQ];
+            if (NZ != 1) v *= r[4 + 2 * NQ + nd % NZ];
+            v *= r[3];
+        }
+    } else if (c < C::NL + 3) {
+        v = r[c - C::NL];
+    }
+    tab[((size_t)blockIdx.y * npad_max + q) * C::ROW + c] = v;
+}
 
 // exp(-r2) for r2 >= 0, FP64, ~1.5 ulp, 10 FP64-pipe instructions: N = round(-r2 * 64/ln 2),
 // r = -r2 - N ln2/64 (two-term Cody-Waite, |r| <= ln2/128), exp(r) by its degree-5 Taylor polynomial
@@ -82,12 +116,12 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 template <int NQ, int NZ = NQ>
 __global__ void __launch_bounds__(MMA_THREADS, 2)
 entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L, int npad_max, int nchunks,
-                   const double* __restrict__ rec, const TileBox* __restrict__ box,
+                   const double* __restrict__ tab, const TileBox* __restrict__ box,
                    unsigned long long* __restrict__ cutstats, double* __restrict__ part,
                    const StepCtrl* __restrict__ stop) {
     if (stop && stop->done) return;
     using C = MmaCfg<NQ, NZ>;
-    constexpr int REC = C::REC, MT = MMA_MT, NBG = C::NBG, NL = C::NL, M = C::M;
+    constexpr int ROW = C::ROW, MT = MMA_MT, NBG = C::NBG, NL = C::NL, M = C::M;
     const int slot0 = blockIdx.x * MMA_THREADS;
     if (slot0 >= L->npad) return;
     if (!fact_usable(T, L)) return;
@@ -98,61 +132,41 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     const int tpc = ceil_div(ntiles, nchunks);
     const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
     const int node0 = blockIdx.z * NL;
+    const double* gtab = tab + (size_t)blockIdx.z * npad_max * ROW;   // this node group's table
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* s_prod = reinterpret_cast<double*>(smem_raw);            // [2][MMA_TILE][MMA_ROW]
-    double* s_rec = s_prod + 2 * MMA_TILE * MMA_ROW;                 // [2][MMA_TILE * REC]
-    double* s_e2 = s_rec + 2 * MMA_TILE * REC;                       // [64]  2^(j/64)
-    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_e2 + 64);        // [2]
-    int* s_list = reinterpret_cast<int*>(s_bar + 2);                 // [MMA_LCAP] active source tiles of a segment
+    double* s_prod = reinterpret_cast<double*>(smem_raw);            // [MMA_STAGES][MMA_TILE][ROW]
+    double* s_e2 = s_prod + MMA_STAGES * MMA_TILE * ROW;             // [64]  2^(j/64)
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_e2 + 64);        // [MMA_STAGES]
+    int* s_list = reinterpret_cast<int*>(s_bar + MMA_STAGES);        // [MMA_LCAP] active source tiles of a segment
     int* s_wcnt = s_list + MMA_LCAP;                                 // [4]
     const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
     const int lr = lane >> 2, lc = lane & 3;                         // fragment row / column of this lane
     if (tid < 64) s_e2[tid] = T->exp2_tab[tid];
     if (tid == 0) {
-        mbar_init(&s_bar[0], 1);
-        mbar_init(&s_bar[1], 1);
+#pragma unroll
+        for (int b = 0; b < MMA_STAGES; ++b) mbar_init(&s_bar[b], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    // gk counts the tiles loaded by this block so far (stage = gk & 1, mbarrier parity = (gk >> 1) & 1); li is the
-    // tile's position in the active list of the current segment
+    // gk counts the tiles loaded by this block so far (stage = gk % STAGES, mbarrier parity = (gk / STAGES) & 1);
+    // li is the tile's position in the active list of the current segment
     auto issue = [&](int gk, int li) {
         if (tid == 0) {
+            const int st = gk % MMA_STAGES;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            constexpr uint32_t BYTES = MMA_TILE * REC * (uint32_t)sizeof(double);
-            mbar_expect_tx(&s_bar[gk & 1], BYTES);
-            bulk_g2s(s_rec + (size_t)(gk & 1) * MMA_TILE * REC,
-                     rec + ((size_t)src0 + (size_t)s_list[li] * MMA_TILE) * REC, BYTES, &s_bar[gk & 1]);
-        }
-    };
-    // product-table builder: lane = node (conflict-free: a warp reads <= NQ distinct factors of ONE record per
-    // load and writes 32 consecutive doubles of one row), the block's two warp pairs take alternate sources
-    const int be = tid & 63, bq = tid >> 6;
-    const int bnd = node0 + be;
-    const bool bvalid = be < NL && bnd < M;
-    const int oi = 4 + (bvalid ? bnd / (NQ * NZ) : 0), oj = 4 + NQ + (bvalid ? (bnd / NZ) % NQ : 0),
-              ol = 4 + 2 * NQ + (bvalid ? bnd % NZ : 0);
-    auto build = [&](int k) {                                        // records of tile k -> product table k & 1
-        mbar_wait(&s_bar[k & 1], (uint32_t)(k >> 1) & 1u);
-        const double* r = s_rec + (size_t)(k & 1) * MMA_TILE * REC + bq * REC;
-        double* row = s_prod + ((size_t)(k & 1) * MMA_TILE + bq) * MMA_ROW;
-#pragma unroll 8
-        for (int qi = 0; qi < MMA_TILE / 2; ++qi) {
-            const double v = NZ == 1 ? r[oi] * r[oj] : r[oi] * r[oj] * r[ol];
-            if (be < NL) row[be] = bvalid ? v : 0.0;
-            if (be < 4) row[64 + be] = r[be];
-            r += 2 * REC;
-            row += 2 * MMA_ROW;
+            mbar_expect_tx(&s_bar[st], C::TILE_BYTES);
+            bulk_g2s(s_prod + (size_t)st * MMA_TILE * ROW,
+                     gtab + ((size_t)src0 + (size_t)s_list[li] * MMA_TILE) * ROW, C::TILE_BYTES, &s_bar[st]);
         }
     };
 
     double px[MT], py[MT], pz[MT];
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
-        const size_t p = (size_t)(slot0 + wv * 32 + mt * 8 + lr) * REC;
-        px[mt] = rec[p]; py[mt] = rec[p + 1]; pz[mt] = rec[p + 2];
+        const double* r = gtab + (size_t)(slot0 + wv * 32 + mt * 8 + lr) * ROW + NL;
+        px[mt] = r[0]; py[mt] = r[1]; pz[mt] = r[2];
     }
     double acc[MT][NBG][2];
 #pragma unroll
@@ -181,38 +195,34 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         __syncthreads();
     }
     nskip += (seg1 - seg0) - n;
-    if (n > 0) {
-        issue(gbase, 0);
-        if (n > 1) issue(gbase + 1, 1);
-        build(gbase);
-        __syncthreads();
-        if (n > 2) issue(gbase + 2, 2);
-    }
+#pragma unroll
+    for (int b = 0; b < MMA_STAGES; ++b)
+        if (b < n) issue(gbase + b, b);
     for (int kk = 0; kk < n; ++kk) {
         const int k = gbase + kk;
-        if (kk + 1 < n) build(k + 1);
-        const double* pr = s_prod + (size_t)(k & 1) * MMA_TILE * MMA_ROW;
+        mbar_wait(&s_bar[k % MMA_STAGES], (uint32_t)(k / MMA_STAGES) & 1u);
+        const double* pr = s_prod + (size_t)(k % MMA_STAGES) * MMA_TILE * ROW;
 #pragma unroll 2
         for (int ks = 0; ks < MMA_TILE / 4; ++ks) {
-            const double* row = pr + (ks * 4 + lc) * MMA_ROW;
-            const double2 a = *reinterpret_cast<const double2*>(row + 64);
-            const double2 b = *reinterpret_cast<const double2*>(row + 66);
+            const double* row = pr + (ks * 4 + lc) * ROW;
+            const double2 a = *reinterpret_cast<const double2*>(row + NL);
+            const double qz = row[NL + 2];
             double A[MT], Bf[NBG];
 #pragma unroll
             for (int nb = 0; nb < NBG; ++nb) Bf[nb] = row[nb * 8 + lr];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
-                const double dx = px[mt] - a.x, dy = py[mt] - a.y, dz = pz[mt] - b.x;
+                const double dx = px[mt] - a.x, dy = py[mt] - a.y, dz = pz[mt] - qz;
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                A[mt] = b.y * exp_neg_tab(r2, s_e2);
+                A[mt] = exp_neg_tab(r2, s_e2);
             }
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
                 for (int nb = 0; nb < NBG; ++nb) dmma884(acc[mt][nb][0], acc[mt][nb][1], A[mt], Bf[nb]);
         }
-        __syncthreads();
-        if (kk + 3 < n) issue(k + 3, kk + 3);
+        __syncthreads();                                              // every warp is done with this stage
+        if (kk + MMA_STAGES < n) issue(k + MMA_STAGES, kk + MMA_STAGES);
     }
     gbase += n;
     }

@@ -82,7 +82,7 @@ struct landau_ctx {
     void* h_pin = nullptr;                // pinned read-back area
     Cloud tmp, state;
     Buf blockcnt, blockoff, part, vpart, blockpart, vk, V, records, stage_v, stage_w, stage_s, stage_o;
-    Buf facttab, tilebox;
+    Buf facttab, prodtab, tilebox;
     Buf cellkey, cellrank, chunkcnt, binoff, spbox;   // Morton bucketing of pack (pack.cuh)
     int morton_on = 1;                                // landau_set_cutoff(.., morton)
     size_t attr_cellcount = 0;
@@ -458,8 +458,14 @@ template <int NQ, int NZ>
 int launch_entropy_mma_nz(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl* stop) {
     using M = MmaCfg<NQ, NZ>;
     RC(ensure(c, c->facttab, sizeof(double) * M::REC * (size_t)cl.npad_max));
+    RC(ensure(c, c->prodtab, M::table_bytes((size_t)cl.npad_max)));
     entropy_fact_prep_kernel<NQ><<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(), cl.z(), cl.w(), (double*)c->facttab.p, stop);
+    // the product table every block of the contraction streams (built once per pass, entropy_mma.cuh)
+    dim3 pgrid((unsigned)(((size_t)cl.npad_max * M::ROW + 255) / 256), M::GROUPS);
+    entropy_prod_kernel<NQ, NZ><<<pgrid, 256, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, (const double*)c->facttab.p,
+                                                             (double*)c->prodtab.p, stop);
+    c->launches += 1;
     auto kern = entropy_mma_kernel<NQ, NZ>;
     bool& attr = NZ == 1 ? c->attr_mma2v[NQ] : c->attr_mma[NQ];
     if (!attr) {
@@ -468,7 +474,7 @@ int launch_entropy_mma_nz(landau_ctx* c, Cloud& cl, int nchunks, const StepCtrl*
     }
     dim3 grid(cl.npad_max / MMA_THREADS, nchunks, M::GROUPS);
     kern<<<grid, MMA_THREADS, M::SMEM, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, nchunks,
-                                                    (const double*)c->facttab.p, (const TileBox*)c->tilebox.p,
+                                                    (const double*)c->prodtab.p, (const TileBox*)c->tilebox.p,
                                                     c->d_cutstats, (double*)c->part.p, stop);
     return 0;
 }
@@ -1157,7 +1163,7 @@ void landau_destroy(landau_ctx* c) {
         release(cl->lay); release(cl->xyzw); release(cl->perm); release(cl->G); release(cl->rec); release(cl->soa);
     }
     for (Buf* b : {&c->blockcnt, &c->blockoff, &c->part, &c->vpart, &c->blockpart, &c->vk, &c->V, &c->records,
-                   &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->dg_u, &c->dg_Gu,
+                   &c->stage_v, &c->stage_w, &c->stage_s, &c->stage_o, &c->facttab, &c->prodtab, &c->dg_u, &c->dg_Gu,
                    &c->dg_Gk, &c->dg_part, &c->aa_hist, &c->cells_off, &c->cells_rec, &c->soa32, &c->sym_acc,
                    &c->sym_tpart, &c->sym_ticket, &c->tilebox, &c->cellkey,
                    &c->cellrank, &c->chunkcnt, &c->binoff, &c->spbox, &c->stiff_mark, &c->stiff_scratch})
