@@ -30,6 +30,7 @@ struct DevTable {
     double knot[LD_MAX_NQ];           // Gauss-Hermite knots k_i (weight exp(-k^2))
     double gw[LD_MAX_NQ];             // Gauss-Hermite weights a_i
     double exp2_tab[64];              // 2^(j/64), j = 0..63 (table of exp_neg_tab, entropy_mma.cuh)
+    double exp2_tab256[256];          // 2^(j/256) (table of exp_neg_t256, entropy_mma.cuh)
 };
 
 // Per-pack layout, written on the device by the pack kernels (no host round trip needed).

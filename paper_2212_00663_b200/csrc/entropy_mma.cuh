@@ -49,7 +49,7 @@ struct MmaCfg {
     static constexpr int REC = FactCfg<NQ>::REC;
     static constexpr uint32_t TILE_BYTES = MMA_TILE * ROW * (uint32_t)sizeof(double);
     static constexpr size_t SMEM =
-        sizeof(double) * (MMA_STAGES * MMA_TILE * ROW + 64) + MMA_STAGES * sizeof(uint64_t) +
+        sizeof(double) * (MMA_STAGES * MMA_TILE * ROW + 256) + MMA_STAGES * sizeof(uint64_t) +
         sizeof(int) * (MMA_LCAP + 8);
     static size_t table_bytes(size_t npad_max) { return sizeof(double) * ROW * npad_max * GROUPS; }
 };
@@ -106,6 +106,31 @@ __device__ __forceinline__ double exp_neg_tab(double r2, const double* __restric
     return __hiloint2double(far ? 0 : hi, far ? 0 : __double2loint(p));
 }
 
+// exp(-r2) for r2 >= 0 as used by the contraction kernel: <= 1.5 ulp with 9 FP64-pipe instructions (exp_neg_tab: 10).
+// N = round(-r2 * 256/ln 2), r = -r2 - N ln2/256 (two-term Cody-Waite, |r| <= ln2/512 = 1.36e-3),
+// exp(r) - 1 = r (1 + r (1/2 + r (1/6 + r/24)))  (dropped r^5/120 < 4e-17), times 2^(j/256) from a 256-entry table
+// (j = N mod 256) and 2^(N div 256) through the exponent field.  Arguments beyond 708 return 0.
+// (Measured and dropped: the cubic part in FP32 through the bit patterns -- 7 FP64 instructions, but the longer
+// dependent chain FP64 -> integer -> FP32 -> FP64 costs more than the two FMAs: 68.0 against 62.8 ms per pass.)
+__device__ __forceinline__ double exp_neg_t256(double r2, const double* __restrict__ s_e2) {
+    const double x = -r2;
+    const double MAGIC = 6755399441055744.0;                       // 1.5 * 2^52
+    double t = fma(x, 369.32993046757462751, MAGIC);               // 256 / ln 2
+    const int N = __double2loint(t);
+    t -= MAGIC;
+    double r = fma(t, -1.08304246932675596327e-02 / 4.0, x);       // ln2_hi / 256 (33 significant bits)
+    r = fma(t, -2.98158582698529328128e-12 / 4.0, r);              // ln2_lo / 256
+    double p = fma(r, 4.1666666666666664354e-02, 1.6666666666666665741e-01);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p *= r;
+    const double tab = s_e2[N & 255];
+    p = fma(tab, p, tab);
+    const int hi = __double2hiint(p) + ((N >> 8) << 20);
+    const bool far = __double2hiint(r2) > 0x40862000;              // r2 > 708 (r2 >= 0: integer order)
+    return __hiloint2double(far ? 0 : hi, far ? 0 : __double2loint(p));
+}
+
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1)
@@ -136,13 +161,13 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* s_prod = reinterpret_cast<double*>(smem_raw);            // [MMA_STAGES][MMA_TILE][ROW]
-    double* s_e2 = s_prod + MMA_STAGES * MMA_TILE * ROW;             // [64]  2^(j/64)
-    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_e2 + 64);        // [MMA_STAGES]
+    double* s_e2 = s_prod + MMA_STAGES * MMA_TILE * ROW;             // [256]  2^(j/256)
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_e2 + 256);        // [MMA_STAGES]
     int* s_list = reinterpret_cast<int*>(s_bar + MMA_STAGES);        // [MMA_LCAP] active source tiles of a segment
     int* s_wcnt = s_list + MMA_LCAP;                                 // [4]
     const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
     const int lr = lane >> 2, lc = lane & 3;                         // fragment row / column of this lane
-    if (tid < 64) s_e2[tid] = T->exp2_tab[tid];
+    for (int i = tid; i < 256; i += MMA_THREADS) s_e2[i] = T->exp2_tab256[i];
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < MMA_STAGES; ++b) mbar_init(&s_bar[b], 1);
@@ -214,7 +239,7 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
             for (int mt = 0; mt < MT; ++mt) {
                 const double dx = px[mt] - a.x, dy = py[mt] - a.y, dz = pz[mt] - qz;
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                A[mt] = exp_neg_tab(r2, s_e2);
+                A[mt] = exp_neg_t256(r2, s_e2);
             }
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)

@@ -11,6 +11,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <cmath>
 #include <new>
 #include <vector>
 
@@ -510,6 +511,21 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / (c->S * 256))));   // >= 4 source tiles per chunk
     nchunks = std::min(nchunks, 64);
     while (nchunks > 1 && (size_t)nchunks * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) --nchunks;
+    if (use_mma && nchunks >= 3) {
+        // wave quantisation: 2 blocks are resident per SM, and a last wave that fills a few SMs costs a whole block
+        // time (3 x 2^16 markers: 4 chunks = 21.08 waves, the 22nd wave 4 % of the kernel).  Take the chunk count
+        // near the first guess whose block count is closest below a whole number of waves.
+        const int hi = std::min({64, 2 * nchunks, std::max(1, cl.npad_max / (c->S * 256))});
+        double best = 1e30;
+        int pick = nchunks;
+        for (int k = std::max(2, nchunks - 1); k <= hi; ++k) {
+            if ((size_t)k * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) break;
+            const double waves = (double)ttiles * mma_groups(nq) * k / (2.0 * c->sm_count);
+            const double cost = std::ceil(waves) / waves + 0.002 * k;      // larger k: more partial sums to store
+            if (cost < best) { best = cost; pick = k; }
+        }
+        nchunks = pick;
+    }
     RC(ensure(c, c->part, (size_t)nchunks * M * cl.npad_max * sizeof(double)));
     RC(ensure(c, c->tilebox, sizeof(TileBox) * ((size_t)cl.npad_max / ENT_SRC_TILE + 2)));
     {
@@ -1123,6 +1139,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     for (int i = 0; i < S * S; ++i) t.nu[i] = c->nu[i];
     for (int i = 0; i < c->n_q; ++i) { t.knot[i] = c->knot[i]; t.gw[i] = c->gw[i]; }
     for (int j = 0; j < 64; ++j) t.exp2_tab[j] = exp2((double)j / 64.0);
+    for (int j = 0; j < 256; ++j) t.exp2_tab256[j] = exp2((double)j / 256.0);
     if (cudaMalloc(&c->d_tab, sizeof(DevTable)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);
