@@ -190,7 +190,13 @@ entropy_literal_kernel(const DevTable* __restrict__ T, const DevLayout* __restri
 //   sum_l a_l k_l [1 + ln rho_ijl] = 0,   sum_l a_l [1 + ln rho_ijl] = (sum_l a_l)(1 + ln rho_ij0) - sum_l a_l k_l^2,
 // the last term dropping out of G by the antisymmetry of the knots in i and j -- which gives the paper's 2-V Eq. (22)
 // exactly and the same s_p as the n_q^3-node evaluation.
-__global__ void __launch_bounds__(128)
+// One block = FIN_MARKERS consecutive slots; warp w takes the nodes w, w + FIN_SLICES, ... of all of them (coalesced reads
+// of the node sums, n_q^3 / FIN_SLICES logarithms per thread), the slices meet in shared memory and are added in slice
+// order (deterministic).  Round 1: one thread per marker walked all n_q^3 nodes x chunks serially -- 178 us for the
+// 8192 markers of BASELINE config 1, as long as the contraction itself.
+constexpr int FIN_MARKERS = 32, FIN_SLICES = 8, FIN_THREADS = FIN_MARKERS * FIN_SLICES;
+
+__global__ void __launch_bounds__(FIN_THREADS)
 entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, int npad_max,
                         int nchunks, const int* __restrict__ perm, const double* __restrict__ part,
                         const double* __restrict__ px, const double* __restrict__ py,
@@ -198,34 +204,34 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
                         double* __restrict__ Gx, double* __restrict__ Gy, double* __restrict__ Gz,
                         double* __restrict__ snode, const StepCtrl* __restrict__ stop) {
     if (stop && stop->done) return;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= npad_max || p >= L->npad) return;
+    const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;
+    const int p = blockIdx.x * FIN_MARKERS + lane;
+    if (blockIdx.x * FIN_MARKERS >= L->npad) return;                 // block-uniform
     const bool factorised = fact_mode != 0 && fact_usable(T, L);
-    if (p == 0) L->used_fact = factorised ? 1 : 0;
-    if (fact_mode == 2 && !factorised) { if (p == 0) atomicMin(&L->err, -5); return; }
-    if (perm[p] < 0) { Gx[p] = 0.0; Gy[p] = 0.0; Gz[p] = 0.0; snode[p] = 0.0; return; }
+    if (p == 0 && slice == 0) L->used_fact = factorised ? 1 : 0;
+    if (fact_mode == 2 && !factorised) { if (p == 0 && slice == 0) atomicMin(&L->err, -5); return; }
+    const bool real = p < L->npad && perm[p] >= 0;
     const int S = T->S, nq = T->n_q;
-    const int s = species_of_slot(L, S, p);
+    const int s = species_of_slot(L, S, min(p, L->npad - 1));
     const double eps = T->eps[s];
     const double PI = 3.14159265358979323846;
     const double lognorm = -1.5 * log(2.0 * PI * eps);
-    const size_t M = (size_t)nq * nq * nq;
     // factorised form: ln A_p(k) = -|k|^2 - 2 k.(p - c) + ln(sum); (p - c) in mollifier units
     double cx = 0.0, cy = 0.0, cz = 0.0;
-    if (factorised) {
+    if (factorised && real) {
         const double inv = T->inv_sqrt_2eps[s];
         cx = (px[p] - L->center[s][0]) * inv;
         cy = (py[p] - L->center[s][1]) * inv;
         cz = (pz[p] - L->center[s][2]) * inv;
     }
     double gx = 0.0, gy = 0.0, gz = 0.0, sn = 0.0;
-    if (planar && factorised) {
-        double az = 0.0, azk2 = 0.0, axy = 0.0;
-        for (int l = 0; l < nq; ++l) { az += T->gw[l]; azk2 = fma(T->gw[l], T->knot[l] * T->knot[l], azk2); }
-        const size_t M2 = (size_t)nq * nq;
-        for (int i = 0; i < nq; ++i)
-            for (int j = 0; j < nq; ++j) {
-                const size_t node = (size_t)i * nq + j;
+    if (real) {
+        if (planar && factorised) {
+            double az = 0.0, azk2 = 0.0, axy = 0.0;
+            for (int l = 0; l < nq; ++l) { az += T->gw[l]; azk2 = fma(T->gw[l], T->knot[l] * T->knot[l], azk2); }
+            const int M2 = nq * nq;
+            for (int node = slice; node < M2; node += FIN_SLICES) {
+                const int i = node / nq, j = node - i * nq;
                 double a = 0.0;
                 for (int c = 0; c < nchunks; ++c) a += part[((size_t)c * M2 + node) * (size_t)npad_max + p];
                 const double ki = T->knot[i], kj = T->knot[j];
@@ -236,12 +242,11 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
                 sn = fma(aa * az, lnrho, sn);
                 axy += aa;
             }
-        sn -= axy * azk2;
-    } else
-    for (int i = 0; i < nq; ++i)
-        for (int j = 0; j < nq; ++j)
-            for (int l = 0; l < nq; ++l) {
-                const size_t node = ((size_t)i * nq + j) * nq + l;
+            sn -= axy * azk2;
+        } else {
+            const int M = nq * nq * nq;
+            for (int node = slice; node < M; node += FIN_SLICES) {
+                const int i = node / (nq * nq), j = (node / nq) % nq, l = node % nq;
                 double a = 0.0;
                 for (int c = 0; c < nchunks; ++c) a += part[((size_t)c * M + node) * (size_t)npad_max + p];
                 const double ki = T->knot[i], kj = T->knot[j], kl = T->knot[l];
@@ -253,6 +258,16 @@ entropy_finalize_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ 
                 gx = fma(t, ki, gx); gy = fma(t, kj, gy); gz = fma(t, kl, gz);
                 sn = fma(aaa, lnrho, sn);
             }
+        }
+    }
+    __shared__ double s_red[FIN_SLICES][4][FIN_MARKERS];
+    s_red[slice][0][lane] = gx; s_red[slice][1][lane] = gy; s_red[slice][2][lane] = gz; s_red[slice][3][lane] = sn;
+    __syncthreads();
+    if (slice != 0 || p >= L->npad) return;
+    gx = gy = gz = sn = 0.0;
+#pragma unroll
+    for (int k = 0; k < FIN_SLICES; ++k) { gx += s_red[k][0][lane]; gy += s_red[k][1][lane]; gz += s_red[k][2][lane]; sn += s_red[k][3][lane]; }
+    if (!real) { Gx[p] = 0.0; Gy[p] = 0.0; Gz[p] = 0.0; snode[p] = 0.0; return; }
     const double pref = -sqrt(2.0 / eps) / (PI * sqrt(PI));
     gx *= pref; gy *= pref; gz *= pref;
     if (!(isfinite(gx) && isfinite(gy) && isfinite(gz) && isfinite(sn))) atomicMin(&L->err, -4);

@@ -574,7 +574,7 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
         c->launches += 1;
     }
     }
-    entropy_finalize_kernel<<<ceil_div(cl.npad_max, 128), 128, 0, c->stream>>>(
+    entropy_finalize_kernel<<<ceil_div(cl.npad_max, FIN_MARKERS), FIN_THREADS, 0, c->stream>>>(
         c->d_tab, cl.L(), cl.npad_max, nchunks, cl.prm(), (const double*)c->part.p, cl.x(), cl.y(), cl.z(),
         mode == 1 ? 0 : (mode >= 2 ? 2 : 1), (c->dim == 2 && use_mma) ? 1 : 0, cl.Gx(), cl.Gy(), cl.Gz(), cl.snode(), stop);
     c->launches += 1;
