@@ -11,7 +11,7 @@
 //   -> write back in caller order.
 // No global-memory traffic, no kernel launch and no host synchronisation inside a step.  Cells are dealt to the
 // CTAs through an atomic counter (cells are independent, so results do not depend on the assignment).
-// Limits: markers per cell <= CellsCfg<NQ>::max_cap() (shared memory: 1024 for n_q <= 5, 984 / 890 / 812 for
+// Limits: markers per cell <= CellsCfg<NQ>::max_cap() (shared memory: 1024 for n_q <= 5, 970 / 878 / 802 for
 // n_q = 6 / 7 / 8).  A cell that is too wide for the factorised pass 1 (reading N3) takes the literal-separable form
 // of Eq. (22) (3 n_q exponentials per pair, every factor <= 1), as the single-cell path does.  n_q > 4: the n_q^3 node
 // sums of a target are accumulated in slices of x-node indices (registers), the per-pair exponential recomputed per
@@ -22,6 +22,7 @@
 #include "entropy.cuh"
 #include "entropy_mma.cuh"   // exp_neg_tab
 #include "pair.cuh"          // pair_accumulate
+#include "pair_sym.cuh"      // sym_step3
 
 namespace landau {
 
@@ -40,8 +41,9 @@ struct CellRecord {          // mirrors landau_cell_info (host struct) field by 
 template <int NQ>
 struct CellsCfg {
     // doubles per marker: xn yn zn w | Gx Gy Gz | xk yk zk | 3 NQ table entries (pass 1) / one source record
-    // {ux uy uz w gx gy gz 0} (pass 2; 64 bytes: four LDS.128 per source instead of seven LDS.64)
-    static constexpr int TAB = 3 * NQ > 8 ? 3 * NQ : 8;
+    // {ux uy uz w gx gy gz 0} (pass 2, one-sided loop; 64 bytes: four LDS.128 per source instead of seven LDS.64) /
+    // seven source arrays + three source-side accumulator arrays (pass 2, symmetric evaluation)
+    static constexpr int TAB = 3 * NQ > 10 ? 3 * NQ : 10;
     static constexpr int DPM = 10 + TAB;
     // x-node indices per register slice of the node sums: NI * NQ^2 <= 64 accumulators
     static constexpr int NI = NQ <= 4 ? NQ : 1;
@@ -51,7 +53,7 @@ struct CellsCfg {
     }
     static int max_cap() {                  // largest even cap whose state fits the 227 KB of a CTA
         int cap = CELLS_CAP;
-        while (cap > 32 && smem(cap) > 227 * 1024 - 1024) cap -= 2;
+        while (cap > 32 && smem(cap) > 227 * 1024 - 4096) cap -= 2;   // the kernel's static shared memory is ~2.2 KB
         return cap;
     }
 };
@@ -178,6 +180,121 @@ __device__ __forceinline__ void cells_field(const double* __restrict__ rec, cons
             const double nu = s_nu[sp[t] * S + sb];
             tx[t] = fma(nu, ax[t], tx[t]); ty[t] = fma(nu, ay[t], ty[t]); tz[t] = fma(nu, az[t], tz[t]);
         }
+    }
+}
+
+// Pass 2 of a whole cell in the symmetric (action-reaction) form of pair_sym.cuh: Q(z)(g_p - g_q)/|z| once per
+// unordered pair, applied to both markers -- 15 instead of 26 FP64 instructions per ordered pair.  Needs
+// nu_ss' = c_s c_s' (DevTable::nu_rank1; c_s is folded into the weights, W = w c_s, and applied to the target at the
+// end).  Thread tid owns R = ceil(n / 256) slots of its warp's sub-tile (cells_sym_slot; registers: position, g, W,
+// target-side sums); warp w's 32 R slots are also "sub-tile" w of the sources.  Phase 0: every warp its own sub-tile, one-sided.
+// Phases 1..3: warp w against sub-tile (w + ph) % 8, both sides.  Phase 4: the pairs {w, w + 4} are split between the
+// two warps (steps 0..15 / 1..16 of the lane rotation).  Inside a phase lane l visits source group (l + k) % 32 at
+// step k -- R consecutive slots, read as 16-byte vectors -- and adds the source-side sums into the shared-memory
+// accumulators next to the sources: in a phase a sub-tile belongs to one warp and at a step every lane holds another
+// group, so there are no conflicts, no atomics, and the order is the program's (deterministic).
+// sx: seven arrays [cap] {ux uy uz W gx gy gz}; sa: [3][cap]; slots n .. n2 (n2 even, <= cap) hold zero dummies.
+// Slot of a thread's r-th target in the symmetric evaluation: warp w owns the 32 R slots of sub-tile w, stored as
+// R / RS blocks of 32 groups of RS consecutive slots, so that the lanes of a warp read consecutive 8 RS-byte vectors
+// whatever R is (R = 4 as two blocks of pairs: four consecutive slots per lane would be a 2-way bank conflict).
+__device__ __forceinline__ int cells_sym_slot(int R, int RS, int wv, int lane, int r) {
+    return wv * 32 * R + (r / RS) * 32 * RS + lane * RS + (r % RS);
+}
+
+template <int R, int RS>
+__device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, double* __restrict__ sa, int cap, int n,
+                                                int n2, double (&tx)[R], double (&ty)[R], double (&tz)[R]) {
+    static_assert(R % RS == 0, "sources of a group are taken RS at a time");
+    const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+    const double* X = sx; const double* Y = sx + cap; const double* Z = sx + 2 * (size_t)cap;
+    const double* Wt = sx + 3 * (size_t)cap;
+    const double* HX = sx + 4 * (size_t)cap; const double* HY = sx + 5 * (size_t)cap; const double* HZ = sx + 6 * (size_t)cap;
+    double* AX = sa; double* AY = sa + cap; double* AZ = sa + 2 * (size_t)cap;
+    double px[R], py[R], pz[R], gx[R], gy[R], gz[R], wp[R], ax[R], ay[R], az[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int p = cells_sym_slot(R, RS, wv, lane, r);
+        const bool ok = p < n2;
+        px[r] = ok ? X[p] : 0.0; py[r] = ok ? Y[p] : 0.0; pz[r] = ok ? Z[p] : 0.0;
+        gx[r] = ok ? HX[p] : 0.0; gy[r] = ok ? HY[p] : 0.0; gz[r] = ok ? HZ[p] : 0.0;
+        wp[r] = ok ? Wt[p] : 0.0;
+        ax[r] = ay[r] = az[r] = 0.0;
+        if (ok) { AX[p] = 0.0; AY[p] = 0.0; AZ[p] = 0.0; }
+    }
+    __syncthreads();
+    constexpr int NW = CELLS_THREADS / 32;
+#pragma unroll 1
+    for (int ph = 0; ph <= NW / 2; ++ph) {
+        const int u = (wv + ph) & (NW - 1);
+        int k0 = 0, k1 = 32;
+        if (ph == NW / 2) { if (wv < NW / 2) k1 = 16; else { k0 = 1; k1 = 17; } }
+#pragma unroll 1
+        for (int k = k0; k < k1; ++k) {
+            const int gl = (lane + k) & 31;                            // the group this lane visits
+#pragma unroll
+            for (int h = 0; h < R; h += RS) {
+                double qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS], bx[RS], by[RS], bz[RS];
+                const int q = cells_sym_slot(R, RS, u, gl, h);
+                if (RS == 2) {
+                    // q and n2 are even: both slots exist or neither
+                    const bool ok = q < n2;
+                    const double2 zero = make_double2(0.0, 0.0);
+                    const double2 a0 = ok ? *reinterpret_cast<const double2*>(X + q) : zero;
+                    const double2 a1 = ok ? *reinterpret_cast<const double2*>(Y + q) : zero;
+                    const double2 a2 = ok ? *reinterpret_cast<const double2*>(Z + q) : zero;
+                    const double2 a3 = ok ? *reinterpret_cast<const double2*>(Wt + q) : zero;
+                    const double2 a4 = ok ? *reinterpret_cast<const double2*>(HX + q) : zero;
+                    const double2 a5 = ok ? *reinterpret_cast<const double2*>(HY + q) : zero;
+                    const double2 a6 = ok ? *reinterpret_cast<const double2*>(HZ + q) : zero;
+                    qx[0] = a0.x; qx[RS - 1] = a0.y; qy[0] = a1.x; qy[RS - 1] = a1.y; qz[0] = a2.x; qz[RS - 1] = a2.y;
+                    qw[0] = a3.x; qw[RS - 1] = a3.y;
+                    hx[0] = a4.x; hx[RS - 1] = a4.y; hy[0] = a5.x; hy[RS - 1] = a5.y; hz[0] = a6.x; hz[RS - 1] = a6.y;
+                    if (ph == 0) {
+                        sym_step3<false, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    } else {
+                        const double2 b0 = ok ? *reinterpret_cast<const double2*>(AX + q) : zero;
+                        const double2 b1 = ok ? *reinterpret_cast<const double2*>(AY + q) : zero;
+                        const double2 b2 = ok ? *reinterpret_cast<const double2*>(AZ + q) : zero;
+                        bx[0] = b0.x; bx[RS - 1] = b0.y; by[0] = b1.x; by[RS - 1] = b1.y; bz[0] = b2.x; bz[RS - 1] = b2.y;
+                        sym_step3<true, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                        if (ok) {
+                            *reinterpret_cast<double2*>(AX + q) = make_double2(bx[0], bx[RS - 1]);
+                            *reinterpret_cast<double2*>(AY + q) = make_double2(by[0], by[RS - 1]);
+                            *reinterpret_cast<double2*>(AZ + q) = make_double2(bz[0], bz[RS - 1]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int s2 = 0; s2 < RS; ++s2) {
+                        const bool ok = q + s2 < n2;
+                        qx[s2] = ok ? X[q + s2] : 0.0; qy[s2] = ok ? Y[q + s2] : 0.0; qz[s2] = ok ? Z[q + s2] : 0.0;
+                        qw[s2] = ok ? Wt[q + s2] : 0.0;
+                        hx[s2] = ok ? HX[q + s2] : 0.0; hy[s2] = ok ? HY[q + s2] : 0.0; hz[s2] = ok ? HZ[q + s2] : 0.0;
+                    }
+                    if (ph == 0) {
+                        sym_step3<false, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+                    } else {
+#pragma unroll
+                        for (int s2 = 0; s2 < RS; ++s2) {
+                            const bool ok = q + s2 < n2;
+                            bx[s2] = ok ? AX[q + s2] : 0.0; by[s2] = ok ? AY[q + s2] : 0.0; bz[s2] = ok ? AZ[q + s2] : 0.0;
+                        }
+                        sym_step3<true, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
+#pragma unroll
+                        for (int s2 = 0; s2 < RS; ++s2)
+                            if (q + s2 < n2) { AX[q + s2] = bx[s2]; AY[q + s2] = by[s2]; AZ[q + s2] = bz[s2]; }
+                    }
+                }
+            }
+            if (ph != 0) __syncwarp();
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int p = cells_sym_slot(R, RS, wv, lane, r);
+        const bool ok = p < n2;
+        tx[r] = ax[r] - (ok ? AX[p] : 0.0); ty[r] = ay[r] - (ok ? AY[p] : 0.0); tz[r] = az[r] - (ok ? AZ[p] : 0.0);
     }
 }
 
@@ -381,24 +498,55 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             __syncthreads();
             if (s_status != 0) break;
             // ---- Eq. (24): Jacobi fixed point, G^n frozen (g = G/m in place), v^(0) = v^n
+            // symmetric in-cell evaluation (cells_field_sym) when nu_ss' = c_s c_s' and the cell has >= 448 markers (measured:
+            // below that the idle lanes of the last round cost more than the 26 -> 15 instructions per pair save)
+            const int rounds = ceil_div(n, CELLS_THREADS);
+#ifndef LANDAU_CELLS_SYM_MIN     // tuning knob (build.py: LANDAU_NVCC_EXTRA): smallest cell taking the symmetric evaluation
+#define LANDAU_CELLS_SYM_MIN 448
+#endif
+            const bool use_sym = GF == 1 && T->nu_rank1 != 0 && n >= LANDAU_CELLS_SYM_MIN;
+            const int n2 = min(rounds * CELLS_THREADS, cap);          // cap is even: pairs of slots exist or not together
+            double* const sxa = tab;                                   // [7][cap] sources, then [3][cap] source-side sums
+            double* const saa = tab + 7 * (size_t)cap;
+            // slot of this thread's r-th target: consecutive slots in the symmetric evaluation, strided otherwise
+            auto slot_of = [&](int r) {
+                return use_sym ? (r < rounds ? cells_sym_slot(rounds, rounds == 3 ? 3 : 2, wv, lane, r) : n) : r * CELLS_THREADS + tid;
+            };
             int sp[CELLS_ROUNDS];
             double im[CELLS_ROUNDS], wm[CELLS_ROUNDS];
 #pragma unroll
             for (int r = 0; r < CELLS_ROUNDS; ++r) {
-                const int p = r * CELLS_THREADS + tid;
+                const int p = slot_of(r);
                 sp[r] = 0; im[r] = 0.0; wm[r] = 0.0;
                 if (p < n) {
                     int s = 0;
                     for (int t = 1; t < S; ++t) s += (p >= s_off[t]) ? 1 : 0;
                     sp[r] = s; im[r] = T->inv_mass[s]; wm[r] = ww[p] * T->mass[s];
                     xk[p] = xn[p]; yk[p] = yn[p]; zk[p] = zn[p];
-                    double2* o = reinterpret_cast<double2*>(srec + (size_t)p * 8);
-                    o[0] = make_double2(xn[p], yn[p]);
-                    o[1] = make_double2(zn[p], ww[p]);
-                    o[2] = make_double2(Gx[p] * im[r], Gy[p] * im[r]);
-                    o[3] = make_double2(Gz[p] * im[r], 0.0);
                 }
             }
+            __syncthreads();                                           // pass 1 has read its tables: the region is free
+#pragma unroll
+            for (int r = 0; r < CELLS_ROUNDS; ++r) {
+                const int p = slot_of(r);
+                if (p < n) {
+                    if (use_sym) {
+                        sxa[p] = xn[p]; sxa[cap + p] = yn[p]; sxa[2 * (size_t)cap + p] = zn[p];
+                        sxa[3 * (size_t)cap + p] = ww[p] * T->nu_fac[sp[r]];
+                        sxa[4 * (size_t)cap + p] = Gx[p] * im[r]; sxa[5 * (size_t)cap + p] = Gy[p] * im[r];
+                        sxa[6 * (size_t)cap + p] = Gz[p] * im[r];
+                    } else {
+                        double2* o = reinterpret_cast<double2*>(srec + (size_t)p * 8);
+                        o[0] = make_double2(xn[p], yn[p]);
+                        o[1] = make_double2(zn[p], ww[p]);
+                        o[2] = make_double2(Gx[p] * im[r], Gy[p] * im[r]);
+                        o[3] = make_double2(Gz[p] * im[r], 0.0);
+                    }
+                }
+            }
+            if (use_sym)                                               // zero dummies behind the cell's last marker
+                for (int p = n + tid; p < n2; p += CELLS_THREADS)
+                    for (int c = 0; c < 7; ++c) sxa[(size_t)c * cap + p] = 0.0;
             __syncthreads();
             int it = 0, conv = 0;
             double res = 0.0;
@@ -408,7 +556,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
 #pragma unroll
                 for (int r = 0; r < CELLS_ROUNDS; ++r) nx[r] = ny[r] = nz[r] = 0.0;
                 auto finish_target = [&](int r, double tx, double ty, double tz) {
-                    const int p = r * CELLS_THREADS + tid;
+                    const int p = slot_of(r);
                     if (p < n) {
                         const double a = fma(dt, tx * im[r], xn[p]), b = fma(dt, ty * im[r], yn[p]),
                                      c = fma(dt, tz * im[r], zn[p]);
@@ -451,11 +599,28 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         }
                         finish_target(0, a, b, c);
                     }
+                } else if (use_sym) {
+                    // block-uniform branch on the cell size: R slots per thread
+                    if (rounds == 4) {
+                        double tx[4], ty[4], tz[4];
+                        cells_field_sym<4, 2>(sxa, saa, cap, n, n2, tx, ty, tz);
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
+                    } else if (rounds == 3) {
+                        double tx[3], ty[3], tz[3];
+                        cells_field_sym<3, 3>(sxa, saa, cap, n, n2, tx, ty, tz);
+#pragma unroll
+                        for (int r = 0; r < 3; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
+                    } else {
+                        double tx[2], ty[2], tz[2];
+                        cells_field_sym<2, 2>(sxa, saa, cap, n, n2, tx, ty, tz);
+#pragma unroll
+                        for (int r = 0; r < 2; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
+                    }
                 } else
                 {
                     // all rounds of targets of a thread share every source read (block-uniform branch on the cell size)
                     static_assert(CELLS_ROUNDS == 4, "one branch per number of rounds");
-                    const int rounds = ceil_div(n, CELLS_THREADS);
                     int pc4[4], sp4[4];
 #pragma unroll
                     for (int r = 0; r < 4; ++r) { pc4[r] = min(r * CELLS_THREADS + tid, n - 1); sp4[r] = sp[r]; }
@@ -486,11 +651,12 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
 #pragma unroll
                 for (int r = 0; r < CELLS_ROUNDS; ++r) {
-                    const int p = r * CELLS_THREADS + tid;
+                    const int p = slot_of(r);
                     if (p < n) {
                         xk[p] = nx[r]; yk[p] = ny[r]; zk[p] = nz[r];
-                        double* o = srec + (size_t)p * 8;
-                        o[0] = 0.5 * (xn[p] + nx[r]); o[1] = 0.5 * (yn[p] + ny[r]); o[2] = 0.5 * (zn[p] + nz[r]);
+                        const double ux = 0.5 * (xn[p] + nx[r]), uy = 0.5 * (yn[p] + ny[r]), uz = 0.5 * (zn[p] + nz[r]);
+                        if (use_sym) { sxa[p] = ux; sxa[cap + p] = uy; sxa[2 * (size_t)cap + p] = uz; }
+                        else { double* o = srec + (size_t)p * 8; o[0] = ux; o[1] = uy; o[2] = uz; }
                     }
                 }
                 __syncthreads();

@@ -31,6 +31,9 @@ struct DevTable {
     double gw[LD_MAX_NQ];             // Gauss-Hermite weights a_i
     double exp2_tab[64];              // 2^(j/64), j = 0..63 (table of exp_neg_tab, entropy_mma.cuh)
     double exp2_tab256[256];          // 2^(j/256) (table of exp_neg_t256, entropy_mma.cuh)
+    double nu_fac[LD_MAX_SPECIES];    // nu_ss' = nu_fac[s] nu_fac[s'] when nu_rank1 (the default nu0 q_s^2 q_s'^2 is)
+    int nu_rank1;
+    int _r0;
 };
 
 // Per-pack layout, written on the device by the pack kernels (no host round trip needed).

@@ -1137,6 +1137,13 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
         t.inv_sqrt_2eps[s] = 1.0 / sqrt(2.0 * eps[s]);
     }
     for (int i = 0; i < S * S; ++i) t.nu[i] = c->nu[i];
+    // nu_ss' = c_s c_s' (true of the default nu0 q_s^2 q_s'^2): the symmetric in-cell pair evaluation of
+    // cells.cuh folds c_s into the weights; any other table keeps the one-sided loop
+    t.nu_rank1 = 1;
+    for (int a = 0; a < S; ++a) { t.nu_fac[a] = sqrt(c->nu[a * S + a]); if (!(c->nu[a * S + a] > 0.0)) t.nu_rank1 = 0; }
+    for (int a = 0; a < S && t.nu_rank1; ++a)
+        for (int b = 0; b < S; ++b)
+            if (fabs(t.nu_fac[a] * t.nu_fac[b] - c->nu[a * S + b]) > 4e-16 * fabs(c->nu[a * S + b])) t.nu_rank1 = 0;
     for (int i = 0; i < c->n_q; ++i) { t.knot[i] = c->knot[i]; t.gw[i] = c->gw[i]; }
     for (int j = 0; j < 64; ++j) t.exp2_tab[j] = exp2((double)j / 64.0);
     for (int j = 0; j < 256; ++j) t.exp2_tab256[j] = exp2((double)j / 256.0);

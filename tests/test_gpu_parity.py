@@ -914,6 +914,49 @@ def test_cells_run_higher_quadrature_orders_match_oracle(B, oracle_mod, n_q):
         assert rel_l2(vout[a:b] - v[a:b], o.get_markers() - v[a:b]) <= 1e-8, (n_q, k)
 
 
+@pytest.mark.parametrize("case", ["rank1", "general_nu", "n_q6_cap"])
+def test_cells_symmetric_in_cell_evaluation_matches_oracle(B, oracle_mod, case):
+    """Cells of >= 448 markers evaluate pass 2 in the symmetric (action-reaction) form inside the fused kernel
+    (cells_field_sym: 2, 3 or 4 slots per thread, ragged tails, a cell at the shared-memory capacity of n_q = 6) when
+    nu_ss' = c_s c_s'; a general symmetric nu table keeps the one-sided loop.  Every cell equals the oracle's step."""
+    if case == "n_q6_cap":
+        specs, n_q, nu = [(0, 485), (0, 230)], 6, None                      # 970 markers: the capacity at n_q = 6
+    else:
+        specs, n_q = [(0, 225), (0, 256), (4, 200), (0, 384), (4, 300), (0, 512), (0, 100)], 4
+        nu = None if case == "rank1" else np.array([[1.0, 0.5, 2.0], [0.5, 1.0, 3.0], [2.0, 3.0, 36.0]])
+    ref4 = W.make(4, n_per_species=8)
+    mass, charge = ref4.mass, ref4.charge
+    eps = np.array([0.05, 0.05 / 3671.0, 0.05 / 22032.0])
+    vs, ws, ss, off = [], [], [], [0]
+    for k, (cfg, n) in enumerate(specs):
+        wl = W.make(cfg, n_per_species=n, seed=300 + k, shuffled=True)
+        v = wl.v.copy()
+        if wl.n_species == 2:
+            v[wl.species_id == 1] *= np.sqrt(1836.0 / 3671.0)
+        vs.append(v); ws.append(wl.w); ss.append(wl.species_id)
+        off.append(off[-1] + wl.n_markers)
+    v, w, sid, off = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss), np.array(off, dtype=np.int64)
+    g = B.Landau(mass, charge, eps, n_q=n_q, nu=nu)
+    dt = 5e-4
+    rc, vout, info = g.cells_run(off, v, w, sid, 1, dt, 1e-12, 60)
+    vout = vout.cpu().numpy()
+    assert rc == 0 and (info["status"] == 0).all()
+    o = oracle_mod.LandauRef(mass, charge, eps, n_q=n_q, nu=nu)
+    mw = (mass[sid] * w)[:, None]
+    for k in range(len(off) - 1):
+        a, b = off[k], off[k + 1]
+        o.set_markers(v[a:b], w[a:b], sid[a:b])
+        rco, ito, reso, convo = o.step(dt, 1e-12, 60)
+        assert rco == 0 and convo
+        assert abs(int(info["iterations"][k]) - ito) <= 1, (case, k)
+        assert rel_l2(vout[a:b], o.get_markers()) <= 1e-11, (case, k)
+        assert rel_l2(vout[a:b] - v[a:b], o.get_markers() - v[a:b]) <= 1e-8, (case, k)
+        # Eqs. 27, 29 per cell: momentum and energy of the committed step
+        dP = np.abs((mw[a:b] * (vout[a:b] - v[a:b])).sum(0)).max() / (mw[a:b] * np.abs(v[a:b])).sum()
+        K0, K1 = 0.5 * (mw[a:b] * v[a:b] ** 2).sum(), 0.5 * (mw[a:b] * vout[a:b] ** 2).sum()
+        assert dP <= 1e-12 and abs(K1 - K0) / K0 <= 1e-12, (case, k, dP, K1 - K0)
+
+
 def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
     """landau_moments(S_eps) evaluates pass 1 at the current state; the next landau_step starts from exactly that
     state and reuses it (one pass 1 per step instead of two in history runs).  Results must be identical to a run
