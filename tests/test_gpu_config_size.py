@@ -101,6 +101,38 @@ def test_entropy_grad_config_size_sampled_rows(B, oracle_mod, cfg, nps):
     assert np.all(np.isfinite(G)) and max(err.values()) <= TOL_FIELD, err
 
 
+def test_both_passes_at_one_million_markers_sampled_rows(B, oracle_mod):
+    """Beyond BASELINE's largest config (393 216 markers): 3 x 349 525 = 1 048 575 markers, species sizes that are not
+    multiples of any tile (ragged tails everywhere), 64-bit offsets in every partial-sum array.  Pass 2 (1.1e12 ordered
+    pairs) and pass 1 (3.7e11 same-species pairs) against the oracle's literal Eqs. (23), (22) on sampled rows, plus
+    Eqs. 27 and 29, which hold at any size."""
+    nps = 349525
+    wl = W.make(4, n_per_species=nps, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    rng = np.random.default_rng(77)
+    G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+    got = g.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
+    assert "pair=sym" in g.last_kernels()
+    rows = sample_rows(wl, 12, 78)
+    err = per_species_errors(got[rows], o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows), wl.species_id[rows],
+                             wl.n_species)
+    REPORT[f"pair_field c4 3x{nps}"] = dict(err, rows=len(rows), kernels=g.last_kernels())
+    print(f"pass 2 c4 3 x {nps}: {err}")
+    assert np.all(np.isfinite(got)) and max(err.values()) <= TOL_FIELD, err
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    assert np.abs((wm * got).sum(axis=0)).max() <= 1e-13 * np.abs(wm * got).sum()          # Eq. 27
+    assert abs((wm * wl.v * got).sum()) <= 1e-13 * np.abs(wm * wl.v * got).sum()             # Eq. 29
+    Gg = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert "entropy=mma" in g.last_kernels()
+    rows = sample_rows(wl, 4, 79)
+    errG = per_species_errors(Gg[rows], o.entropy_grad_rows(wl.v, wl.w, wl.species_id, rows), wl.species_id[rows],
+                              wl.n_species)
+    REPORT[f"entropy_grad c4 3x{nps}"] = dict(errG, rows=len(rows), kernels=g.last_kernels())
+    print(f"pass 1 c4 3 x {nps}: {errG}")
+    assert np.all(np.isfinite(Gg)) and max(errG.values()) <= TOL_FIELD, errG
+
+
 @pytest.mark.parametrize("cfg,nps", [(4, 1 << 16), (3, 32768)])
 def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod, cfg, nps):
     """One converged landau_step at the bench workload (3 x 2^16 markers, symmetric kernel, the launch sequence
