@@ -145,6 +145,94 @@ __device__ __forceinline__ void cells_pass1_target(int i0, int o0, int o1, doubl
     }
 }
 
+// Pass 1 of one species of a cell as an FP64 tensor contraction (n_q = 4, factorised form; the in-cell version of
+// entropy_mma.cuh): F[targets x 64 nodes] = C[targets x sources] * P[sources x nodes], C_pq = exp(-|p' - q'|^2),
+// P_q(n) = w_q Tx_q(i) Ty_q(j) Tz_q(l).  A warp owns 32 targets x 64 nodes of accumulators (mma.sync.m8n8k4.f64, SASS
+// DMMA.8x8x4); per k-step of 4 sources a lane computes its 4 exponentials (A fragments) and builds its 8 B-fragment
+// entries P[source lane%4][node 8 nb + lane/4] from the source's factor table in shared memory (10 multiplies: the
+// node index splits as i = nb/2, j = 2 (nb%2) + (lane/4)/4, l = (lane/4)%4) -- there is no room for a product table next
+// to the cell's state.  64 + 10 vector instructions and 32 DMMAs per 128 pairs, against 101 vector instructions per
+// pair in cells_pass1_target.  The logarithms and the node sum of Eq. (22) are taken in the accumulator layout (a lane
+// holds 16 nodes of each of its 4 targets) and the 4 lanes of a target are added by two shuffles (fixed order).
+__device__ __forceinline__ void cells_pass1_dmma4(int o0, int o1, const double* __restrict__ xk,
+                                                  const double* __restrict__ yk, const double* __restrict__ zk,
+                                                  const double* __restrict__ ww, const double* __restrict__ tab,
+                                                  const double* __restrict__ s_e2, const double (&kn)[4],
+                                                  const double (&ga)[4], double lognorm, double pref, bool planar,
+                                                  double* __restrict__ Gx, double* __restrict__ Gy,
+                                                  double* __restrict__ Gz, int* s_status) {
+    constexpr int MT = 4, NBG = 8;
+    const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
+    const int lr = lane >> 2, lc = lane & 3;
+    const int nks = (o1 - o0 + 3) >> 2;
+    const int j0 = lr >> 2, l0 = lr & 3;                     // B fragment: j = 2 (nb & 1) + j0, l = l0
+    for (int base = o0; base < o1; base += CELLS_THREADS) {
+        const int t0 = base + wv * 32;
+        if (t0 >= o1) continue;                              // warp-uniform; no block barrier inside this function
+        double px[MT], py[MT], pz[MT];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            const int p = min(t0 + mt * 8 + lr, o1 - 1);     // clamped duplicate; not written
+            px[mt] = xk[p]; py[mt] = yk[p]; pz[mt] = zk[p];
+        }
+        double acc[MT][NBG][2];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nb = 0; nb < NBG; ++nb) acc[mt][nb][0] = acc[mt][nb][1] = 0.0;
+#pragma unroll 1
+        for (int ks = 0; ks < nks; ++ks) {
+            const int q = o0 + ks * 4 + lc;
+            const bool ok = q < o1;
+            const int qq = ok ? q : o1 - 1;
+            const double qx = xk[qq], qy = yk[qq], qz = zk[qq];
+            const double* t = tab + (size_t)qq * 12;
+            const double2 ta = *reinterpret_cast<const double2*>(t), tb = *reinterpret_cast<const double2*>(t + 2);
+            const double tzw = ok ? t[8 + l0] * ww[qq] : 0.0;  // a source beyond the species adds exactly 0
+            const double u0 = t[4 + j0] * tzw, u1 = t[6 + j0] * tzw;
+            double A[MT], Bf[NBG];
+            Bf[0] = ta.x * u0; Bf[1] = ta.x * u1; Bf[2] = ta.y * u0; Bf[3] = ta.y * u1;
+            Bf[4] = tb.x * u0; Bf[5] = tb.x * u1; Bf[6] = tb.y * u0; Bf[7] = tb.y * u1;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const double dx = px[mt] - qx, dy = py[mt] - qy, dz = pz[mt] - qz;
+                A[mt] = exp_neg_tab(fma(dz, dz, fma(dy, dy, dx * dx)), s_e2);
+            }
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int nb = 0; nb < NBG; ++nb) dmma884(acc[mt][nb][0], acc[mt][nb][1], A[mt], Bf[nb]);
+        }
+        // accumulator layout: acc[mt][nb][e] = F[target 8 mt + lr][node 8 nb + 2 lc + e], node = 16 i + 4 j + l
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            double gx = 0.0, gy = 0.0, gz = 0.0;
+#pragma unroll
+            for (int nb = 0; nb < NBG; ++nb) {
+                const double ki = kn[nb >> 1], gi = ga[nb >> 1];
+                const double kj = (lc & 2) ? kn[2 * (nb & 1) + 1] : kn[2 * (nb & 1)];
+                const double gj = (lc & 2) ? ga[2 * (nb & 1) + 1] : ga[2 * (nb & 1)];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double kl = (lc & 1) ? kn[2 + e] : kn[e], gl = (lc & 1) ? ga[2 + e] : ga[e];
+                    const double lnrho = lognorm + log(acc[mt][nb][e]) -
+                                         ((ki * ki + kj * kj + kl * kl) + 2.0 * (ki * px[mt] + kj * py[mt] + kl * pz[mt]));
+                    const double tt = gi * gj * gl * (1.0 + lnrho);
+                    gx = fma(tt, ki, gx); gy = fma(tt, kj, gy); gz = fma(tt, kl, gz);
+                }
+            }
+            gx += __shfl_xor_sync(0xffffffffu, gx, 1); gy += __shfl_xor_sync(0xffffffffu, gy, 1); gz += __shfl_xor_sync(0xffffffffu, gz, 1);
+            gx += __shfl_xor_sync(0xffffffffu, gx, 2); gy += __shfl_xor_sync(0xffffffffu, gy, 2); gz += __shfl_xor_sync(0xffffffffu, gz, 2);
+            const int p = t0 + mt * 8 + lr;
+            if (lc == 0 && p < o1) {
+                gx *= pref; gy *= pref; gz *= pref;
+                if (!(isfinite(gx) && isfinite(gy) && isfinite(gz))) *s_status = -4;
+                Gx[p] = gx; Gy[p] = gy; Gz[p] = planar ? 0.0 : gz;
+            }
+        }
+    }
+}
+
 // Pass 2 of NT targets of one thread against every source of the cell (a source record is read once per NT targets:
 // NT = 4 quarters the shared-memory traffic per pair).  t? = sum_s' nu_ss' sum_q w_q Q(u_p - u_q)(g_p - g_q).
 // rec: [n][8] = {ux uy uz w gx gy gz 0}.
@@ -468,6 +556,10 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         if (!(isfinite(a) && isfinite(b) && isfinite(c))) s_status = -4;
                         Gx[p] = a; Gy[p] = b; Gz[p] = (T->dim == 2) ? 0.0 : c;
                     }
+                } else if (NQ == 4 && !literal) {
+                    if constexpr (NQ == 4)
+                        cells_pass1_dmma4(o0, o1, xk, yk, zk, ww, tab, s_e2, kn, ga, lognorm, pref, T->dim == 2, Gx, Gy, Gz,
+                                          &s_status);
                 } else {
                     for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
                         const int pt = r0 + tid;
