@@ -227,7 +227,11 @@ entropy_mma_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         const int k = gbase + kk;
         mbar_wait(&s_bar[k % MMA_STAGES], (uint32_t)(k / MMA_STAGES) & 1u);
         const double* pr = s_prod + (size_t)(k % MMA_STAGES) * MMA_TILE * ROW;
-#pragma unroll 2
+#ifndef LANDAU_MMA_UNROLL            // tuning knob (build.py: LANDAU_NVCC_EXTRA)
+#define LANDAU_MMA_UNROLL 2
+#endif
+        constexpr int KS_UNROLL = LANDAU_MMA_UNROLL;
+#pragma unroll KS_UNROLL
         for (int ks = 0; ks < MMA_TILE / 4; ++ks) {
             const double* row = pr + (ks * 4 + lc) * ROW;
             const double2 a = *reinterpret_cast<const double2*>(row + NL);
