@@ -271,17 +271,6 @@ __device__ __forceinline__ void cells_field(const double* __restrict__ rec, cons
     }
 }
 
-// Pass 2 of a whole cell in the symmetric (action-reaction) form of pair_sym.cuh: Q(z)(g_p - g_q)/|z| once per
-// unordered pair, applied to both markers -- 15 instead of 26 FP64 instructions per ordered pair.  Needs
-// nu_ss' = c_s c_s' (DevTable::nu_rank1; c_s is folded into the weights, W = w c_s, and applied to the target at the
-// end).  Thread tid owns R = ceil(n / 256) slots of its warp's sub-tile (cells_sym_slot; registers: position, g, W,
-// target-side sums); warp w's 32 R slots are also "sub-tile" w of the sources.  Phase 0: every warp its own sub-tile, one-sided.
-// Phases 1..3: warp w against sub-tile (w + ph) % 8, both sides.  Phase 4: the pairs {w, w + 4} are split between the
-// two warps (steps 0..15 / 1..16 of the lane rotation).  Inside a phase lane l visits source group (l + k) % 32 at
-// step k -- R consecutive slots, read as 16-byte vectors -- and adds the source-side sums into the shared-memory
-// accumulators next to the sources: in a phase a sub-tile belongs to one warp and at a step every lane holds another
-// group, so there are no conflicts, no atomics, and the order is the program's (deterministic).
-// sx: seven arrays [cap] {ux uy uz W gx gy gz}; sa: [3][cap]; slots n .. n2 (n2 even, <= cap) hold zero dummies.
 // Slot of a thread's r-th target in the symmetric evaluation: warp w owns the 32 R slots of sub-tile w, stored as
 // R / RS blocks of 32 groups of RS consecutive slots, so that the lanes of a warp read consecutive 8 RS-byte vectors
 // whatever R is (R = 4 as two blocks of pairs: four consecutive slots per lane would be a 2-way bank conflict).
@@ -289,6 +278,18 @@ __device__ __forceinline__ int cells_sym_slot(int R, int RS, int wv, int lane, i
     return wv * 32 * R + (r / RS) * 32 * RS + lane * RS + (r % RS);
 }
 
+// Pass 2 of a whole cell in the symmetric (action-reaction) form of pair_sym.cuh: Q(z)(g_p - g_q)/|z| once per
+// unordered pair, applied to both markers -- 15 instead of 26 FP64 instructions per ordered pair.  Needs
+// nu_ss' = c_s c_s' (DevTable::nu_rank1; c_s is folded into the weights, W = w c_s, and applied to the target at the
+// end).  Thread tid owns R = ceil(n / 256) slots of its warp's sub-tile (cells_sym_slot; registers: position, g, W,
+// target-side sums); warp w's 32 R slots are also "sub-tile" w of the sources.  Phase 0: every warp its own sub-tile (the
+// lane's own group one-sided, every unordered pair of different groups once, both sides).
+// Phases 1..3: warp w against sub-tile (w + ph) % 8, both sides.  Phase 4: the pairs {w, w + 4} are split between the
+// two warps (steps 0..15 / 1..16 of the lane rotation).  Inside a phase lane l visits source group (l + k) % 32 at
+// step k -- R consecutive slots, read as 16-byte vectors -- and adds the source-side sums into the shared-memory
+// accumulators next to the sources: in a phase a sub-tile belongs to one warp and at a step every lane holds another
+// group, so there are no conflicts, no atomics, and the order is the program's (deterministic).
+// sx: seven arrays [cap] {ux uy uz W gx gy gz}; sa: [3][cap]; slots n .. n2 (n2 even, <= cap) hold zero dummies.
 template <int R, int RS>
 __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, double* __restrict__ sa, int cap, int n,
                                                 int n2, double (&tx)[R], double (&ty)[R], double (&tz)[R]) {
@@ -314,18 +315,23 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
 #pragma unroll 1
     for (int ph = 0; ph <= NW / 2; ++ph) {
         const int u = (wv + ph) & (NW - 1);
+        // phase 0 (own sub-tile): step 0 = the lane's own group, one-sided; steps 1..15 both sides; step 16 both sides
+        // by the lower half of the lanes only (the pair of groups {l, l + 16} is seen from both ends)
         int k0 = 0, k1 = 32;
+        if (ph == 0) k1 = 17;
         if (ph == NW / 2) { if (wv < NW / 2) k1 = 16; else { k0 = 1; k1 = 17; } }
 #pragma unroll 1
         for (int k = k0; k < k1; ++k) {
             const int gl = (lane + k) & 31;                            // the group this lane visits
+            const bool one = ph == 0 && k == 0;
+            const bool act = !(ph == 0 && k == 16 && lane >= 16);
 #pragma unroll
             for (int h = 0; h < R; h += RS) {
                 double qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS], bx[RS], by[RS], bz[RS];
                 const int q = cells_sym_slot(R, RS, u, gl, h);
                 if (RS == 2) {
                     // q and n2 are even: both slots exist or neither
-                    const bool ok = q < n2;
+                    const bool ok = q < n2 && act;
                     const double2 zero = make_double2(0.0, 0.0);
                     const double2 a0 = ok ? *reinterpret_cast<const double2*>(X + q) : zero;
                     const double2 a1 = ok ? *reinterpret_cast<const double2*>(Y + q) : zero;
@@ -337,7 +343,7 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
                     qx[0] = a0.x; qx[RS - 1] = a0.y; qy[0] = a1.x; qy[RS - 1] = a1.y; qz[0] = a2.x; qz[RS - 1] = a2.y;
                     qw[0] = a3.x; qw[RS - 1] = a3.y;
                     hx[0] = a4.x; hx[RS - 1] = a4.y; hy[0] = a5.x; hy[RS - 1] = a5.y; hz[0] = a6.x; hz[RS - 1] = a6.y;
-                    if (ph == 0) {
+                    if (one) {
                         sym_step3<false, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                     } else {
                         const double2 b0 = ok ? *reinterpret_cast<const double2*>(AX + q) : zero;
@@ -354,27 +360,27 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
                 } else {
 #pragma unroll
                     for (int s2 = 0; s2 < RS; ++s2) {
-                        const bool ok = q + s2 < n2;
+                        const bool ok = q + s2 < n2 && act;
                         qx[s2] = ok ? X[q + s2] : 0.0; qy[s2] = ok ? Y[q + s2] : 0.0; qz[s2] = ok ? Z[q + s2] : 0.0;
                         qw[s2] = ok ? Wt[q + s2] : 0.0;
                         hx[s2] = ok ? HX[q + s2] : 0.0; hy[s2] = ok ? HY[q + s2] : 0.0; hz[s2] = ok ? HZ[q + s2] : 0.0;
                     }
-                    if (ph == 0) {
+                    if (one) {
                         sym_step3<false, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
                     } else {
 #pragma unroll
                         for (int s2 = 0; s2 < RS; ++s2) {
-                            const bool ok = q + s2 < n2;
+                            const bool ok = q + s2 < n2 && act;
                             bx[s2] = ok ? AX[q + s2] : 0.0; by[s2] = ok ? AY[q + s2] : 0.0; bz[s2] = ok ? AZ[q + s2] : 0.0;
                         }
                         sym_step3<true, R, RS, double>(px, py, pz, gx, gy, gz, wp, ax, ay, az, qx, qy, qz, hx, hy, hz, qw, bx, by, bz);
 #pragma unroll
                         for (int s2 = 0; s2 < RS; ++s2)
-                            if (q + s2 < n2) { AX[q + s2] = bx[s2]; AY[q + s2] = by[s2]; AZ[q + s2] = bz[s2]; }
+                            if (q + s2 < n2 && act) { AX[q + s2] = bx[s2]; AY[q + s2] = by[s2]; AZ[q + s2] = bz[s2]; }
                     }
                 }
             }
-            if (ph != 0) __syncwarp();
+            if (!one) __syncwarp();
         }
         __syncthreads();
     }
