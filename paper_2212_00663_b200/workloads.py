@@ -281,3 +281,27 @@ def paper_test(test: int, n_grid: int = 32, dt_seconds: float = 1e-8, n_steps: O
                     n_steps=int(n_steps if n_steps is not None else round(1e-3 / dt_seconds)), tol=1e-12, max_iter=30,
                     notes={"t0_seconds": t0, "v0_m_per_s": float(v0), "T0_eV": T0, "lnLambda": lnL, "n_grid": n_grid,
                            "two_v": True, "species": species})
+
+
+def shard_cells(cell_offset, rank: int, world: int):
+    """Contiguous range [c0, c1) of collision cells for `rank` of `world` (cells are
+    independent, so a batch shards over GPUs with no data-path collective).  The cut points balance the pairwise work
+    sum_c n_c^2 (pass 2 dominates a cell's cost), every cell belongs to exactly one rank, order is preserved.
+    Pure index arithmetic on the host: none of the method's arithmetic lives here."""
+    off = np.ascontiguousarray(cell_offset, dtype=np.int64)
+    n = np.diff(off).astype(np.float64)
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("shard_cells: need 0 <= rank < world")
+    if n.size == 0:
+        return 0, 0
+    cum = np.concatenate([[0.0], np.cumsum(n * n)])
+    total = cum[-1]
+    if total == 0.0:                                   # only empty cells: split by count
+        cuts = [(n.size * r) // world for r in range(world + 1)]
+    else:
+        # cell c goes to the rank whose share contains the midpoint of its work interval
+        mid = 0.5 * (cum[:-1] + cum[1:])
+        owner = np.minimum((mid * world / total).astype(np.int64), world - 1)
+        owner = np.maximum.accumulate(owner)
+        cuts = [int(np.searchsorted(owner, r, side="left")) for r in range(world)] + [int(n.size)]
+    return cuts[rank], cuts[rank + 1]

@@ -8,6 +8,7 @@ import sys
 from pathlib import Path
 
 import numpy as np
+import pytest
 import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
@@ -66,3 +67,61 @@ def test_replicas_differ_by_seed_only():
     b = W.make(4, n_per_species=64, seed=4 + 1000)
     assert np.array_equal(a.mass, b.mass) and np.array_equal(a.charge, b.charge) and a.n_markers == b.n_markers
     assert not np.array_equal(a.v, b.v)
+
+
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, str(ROOT))
+    from paper_2212_00663_b200 import workloads as W
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    rng = np.random.default_rng(7)                                  # the same ragged batch on every rank
+    n = rng.integers(0, 1025, size=301)
+    off = np.concatenate([[0], np.cumsum(n)]).astype(np.int64)
+    c0, c1 = W.shard_cells(off, rank, world)
+    mine = torch.tensor([c0, c1, int((n[c0:c1].astype(np.int64) ** 2).sum())], dtype=torch.int64)
+    allr = [torch.zeros(3, dtype=torch.int64) for _ in range(world)]
+    dist.all_gather(allr, mine)
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, [t.tolist() for t in allr], int((n.astype(np.int64) ** 2).sum()), int(n.size), int(n.max())))
+
+
+def test_cells_shard_over_ranks_is_a_balanced_partition_over_gloo():
+    """NEXT-3 multi-GPU path (cells_bench under torchrun): workloads.shard_cells gives every rank a contiguous range of
+    cells, every cell exactly once, pairwise work balanced to within one cell -- no data-path collective is needed."""
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_shard_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res[0][1] == res[1][1]                                   # every rank sees the same table
+    _, table, total, ncells, nmax = res[0]
+    assert table[0][0] == 0 and table[-1][1] == ncells
+    assert all(table[r][1] == table[r + 1][0] for r in range(world - 1))
+    assert sum(t[2] for t in table) == total
+    assert max(t[2] for t in table) <= total / world + nmax * nmax
+
+
+def test_shard_cells_edge_cases():
+    sys.path.insert(0, str(ROOT))
+    from paper_2212_00663_b200 import workloads as W
+    assert W.shard_cells(np.array([0]), 0, 4) == (0, 0)                                  # no cells
+    off = np.array([0, 0, 0, 0], dtype=np.int64)                                          # only empty cells
+    assert [W.shard_cells(off, r, 2) for r in range(2)] == [(0, 1), (1, 3)]
+    off = np.array([0, 1000], dtype=np.int64)                                             # fewer cells than ranks
+    got = [W.shard_cells(off, r, 3) for r in range(3)]
+    assert sorted(b - a for a, b in got) == [0, 0, 1] and got[0][0] == 0 and got[-1][1] == 1
+    assert all(got[r][1] == got[r + 1][0] for r in range(2))
+    for world in (1, 2, 3, 5, 8):
+        rng = np.random.default_rng(world)
+        n = rng.integers(1, 600, size=97)
+        off = np.concatenate([[0], np.cumsum(n)])
+        cuts = [W.shard_cells(off, r, world) for r in range(world)]
+        assert cuts[0][0] == 0 and cuts[-1][1] == 97 and all(cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))
+    with pytest.raises(ValueError):
+        W.shard_cells(off, 2, 2)
