@@ -392,8 +392,14 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
     }
 }
 
-template <int NQ>
-__global__ void __launch_bounds__(CELLS_THREADS, 1)
+// MINB = 1: any cell up to the shared-memory capacity, one CTA per SM (255 registers: register-tiled pair loops, DMMA
+// accumulators).  MINB = 2 (n_q = 4, every cell of the batch <= CELLS_SMALL markers): only the small-cell paths (2 or 4
+// threads per target) are compiled, 128 registers, two CTAs per SM -- such cells are bound by the latencies of their
+// barriers and reductions, not by the FP64 pipe, and a second resident cell fills the gaps.
+constexpr int CELLS_SMALL = CELLS_THREADS / 2;
+
+template <int NQ, int MINB = 1>
+__global__ void __launch_bounds__(CELLS_THREADS, MINB)
 cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const long long* __restrict__ cell_off,
                  const double* __restrict__ v, const double* __restrict__ w, const int32_t* __restrict__ sid,
                  double* __restrict__ v_out, int n_steps, double dt, double tol, int max_iter,
@@ -438,7 +444,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             if (v_out != v && n > 0)
                 for (long long i = tid; i < 3LL * n; i += CELLS_THREADS) v_out[3 * g0 + i] = v[3 * g0 + i];
         };
-        if (n < 1 || n > cap) {
+        if (n < 1 || n > cap || (MINB > 1 && n > CELLS_SMALL)) {
             pass_through();
             if (tid == 0) { rec.status = n == 0 ? 0 : -1; records[cell] = rec; }
             continue;
@@ -562,11 +568,11 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         if (!(isfinite(a) && isfinite(b) && isfinite(c))) s_status = -4;
                         Gx[p] = a; Gy[p] = b; Gz[p] = (T->dim == 2) ? 0.0 : c;
                     }
-                } else if (NQ == 4 && !literal) {
-                    if constexpr (NQ == 4)
+                } else if (MINB == 1 && NQ == 4 && !literal) {
+                    if constexpr (NQ == 4 && MINB == 1)
                         cells_pass1_dmma4(o0, o1, xk, yk, zk, ww, tab, s_e2, kn, ga, lognorm, pref, T->dim == 2, Gx, Gy, Gz,
                                           &s_status);
-                } else {
+                } else if constexpr (MINB == 1) {
                     for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
                         const int pt = r0 + tid;
                         const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
@@ -697,7 +703,8 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         }
                         finish_target(0, a, b, c);
                     }
-                } else if (use_sym) {
+                } else if constexpr (MINB == 1) {
+                if (use_sym) {
                     // block-uniform branch on the cell size: R slots per thread
                     if (rounds == 4) {
                         double tx[4], ty[4], tz[4];
@@ -746,6 +753,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         finish_target(0, tx[0], ty[0], tz[0]);
                     }
                 }
+                }   // MINB == 1
                 cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
 #pragma unroll
                 for (int r = 0; r < CELLS_ROUNDS; ++r) {

@@ -99,7 +99,7 @@ struct landau_ctx {
     // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
     bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {}, attr_mma2v[LD_MAX_NQ + 1] = {};
     bool attr_sym64_2v = false;
-    size_t attr_cells[LD_MAX_NQ + 1] = {};
+    size_t attr_cells[LD_MAX_NQ + 1] = {}, attr_cells_small = 0;
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson, 2 Newton-Krylov (NEXT-4)
@@ -1054,22 +1054,32 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
 
 namespace {
 // NEXT-3: many collision cells, one persistent CTA per cell, whole run in one launch (cells.cuh).
-template <int NQ>
-int launch_cells(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
-                 double* v_out, int n_steps, double dt, double tol, int max_iter) {
-    auto kern = cells_run_kernel<NQ>;
+template <int NQ, int MINB>
+int launch_cells_v(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
+                   double* v_out, int n_steps, double dt, double tol, int max_iter) {
+    auto kern = cells_run_kernel<NQ, MINB>;
     const size_t smem = CellsCfg<NQ>::smem(cap);
-    if (smem > c->attr_cells[NQ]) {
+    size_t& attr = MINB == 1 ? c->attr_cells[NQ] : c->attr_cells_small;
+    if (smem > attr) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        c->attr_cells[NQ] = smem;
+        attr = smem;
     }
     int* counter = (int*)((char*)c->cells_off.p + sizeof(long long) * ((size_t)n_cells + 1));
-    const int grid = std::min(n_cells, c->sm_count);
+    const int grid = std::min(n_cells, MINB * c->sm_count);
     kern<<<grid, CELLS_THREADS, smem, c->stream>>>(c->d_tab, n_cells, cap, (const long long*)c->cells_off.p, v, w, sid,
                                                    v_out, n_steps, dt, tol, max_iter, counter,
                                                    (CellRecord*)c->cells_rec.p);
     c->launches += 1;
     return 0;
+}
+
+template <int NQ>
+int launch_cells(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
+                 double* v_out, int n_steps, double dt, double tol, int max_iter) {
+    // a batch of small cells (n_q = 4, every cell <= 128 markers): the two-CTAs-per-SM build of the kernel
+    if (NQ == 4 && cap <= CELLS_SMALL && n_cells > c->sm_count)
+        return launch_cells_v<4, 2>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
+    return launch_cells_v<NQ, 1>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
 }
 
 }  // namespace

@@ -957,6 +957,46 @@ def test_cells_symmetric_in_cell_evaluation_matches_oracle(B, oracle_mod, case):
         assert dP <= 1e-12 and abs(K1 - K0) / K0 <= 1e-12, (case, k, dP, K1 - K0)
 
 
+def test_cells_batch_of_small_cells_two_ctas_per_sm_matches_oracle(B, oracle_mod):
+    """A batch of more cells than SMs whose cells all have <= 128 markers (n_q = 4) runs the two-CTAs-per-SM build of the
+    fused kernel (cells_run_kernel<4, 2>: only the 2- and 4-threads-per-target paths, 128 registers).  170 ragged cells
+    of 1 .. 128 markers, two steps; every cell equals the oracle's steps on that cell alone."""
+    rng = np.random.default_rng(12)
+    sizes = list(rng.integers(1, 65, size=168)) + [64, 1]             # markers per species
+    wl0 = W.make(0, n_per_species=8)
+    vs, ws, ss, off = [], [], [], [0]
+    for k, n in enumerate(sizes):
+        wl = W.make(0, n_per_species=int(n), seed=500 + k, shuffled=True)
+        vs.append(wl.v); ws.append(wl.w); ss.append(wl.species_id)
+        off.append(off[-1] + wl.n_markers)
+    v, w, sid, off = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss), np.array(off, dtype=np.int64)
+    assert np.diff(off).max() == 128 and len(sizes) > 148
+    g = B.Landau(wl0.mass, wl0.charge, wl0.eps)
+    dt, n_steps = 1e-3, 2
+    rc, vout, info = g.cells_run(off, v, w, sid, n_steps, dt, 1e-12, 60)
+    vout = vout.cpu().numpy()
+    assert rc in (0, 1)
+    o = oracle_mod.LandauRef(wl0.mass, wl0.charge, wl0.eps)
+    worst = 0.0
+    for k in range(len(sizes)):
+        a, b = off[k], off[k + 1]
+        o.set_markers(v[a:b], w[a:b], sid[a:b])
+        its, conv_all = 0, True
+        for _ in range(n_steps):
+            rco, ito, reso, convo = o.step(dt, 1e-12, 60)
+            its += ito; conv_all = conv_all and bool(convo)
+        if not conv_all:                                              # a stalled tiny cell: compared at equal max_iter
+            assert info["status"][k] == 1
+            continue
+        assert info["status"][k] == 0 and abs(int(info["iterations"][k]) - its) <= 2, k
+        e = rel_l2(vout[a:b], o.get_markers())
+        worst = max(worst, e)
+        assert e <= 1e-11, (k, e)
+        if b - a > 2:
+            assert rel_l2(vout[a:b] - v[a:b], o.get_markers() - v[a:b]) <= 1e-8, k
+    print(f"small-cell batch: worst state error {worst:.2e}")
+
+
 def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
     """landau_moments(S_eps) evaluates pass 1 at the current state; the next landau_step starts from exactly that
     state and reuses it (one pass 1 per step instead of two in history runs).  Results must be identical to a run
