@@ -997,6 +997,34 @@ def test_cells_batch_of_small_cells_two_ctas_per_sm_matches_oracle(B, oracle_mod
     print(f"small-cell batch: worst state error {worst:.2e}")
 
 
+def test_cells_in_two_v_mode_keep_vz_zero_and_match_oracle(B, oracle_mod):
+    """landau_set_dimension(2) inside landau_cells_run (the paper's 2-V setting): on v_z = 0 data every
+    in-cell path (2 threads per target; DMMA pass 1 + one-sided pass 2; DMMA pass 1 + symmetric pass 2) stores G_z as an
+    exact zero, so v_z stays exactly 0, and v_x, v_y equal the oracle's 3-V step on the same data."""
+    cells = [W.make(0, n_per_species=n, seed=70 + n, shuffled=True) for n in (50, 150, 300)]
+    v = np.concatenate([c.v for c in cells]); w = np.concatenate([c.w for c in cells])
+    sid = np.concatenate([c.species_id for c in cells])
+    v[:, 2] = 0.0
+    off = np.cumsum([0] + [c.n_markers for c in cells]).astype(np.int64)
+    wl = cells[0]
+    g = B.Landau(wl.mass, wl.charge, wl.eps)
+    g.set_dimension(2)
+    rc, vout, info = g.cells_run(off, v, w, sid, 2, 2e-3, 1e-12, 60)
+    vout = vout.cpu().numpy()
+    assert rc == 0 and (info["status"] == 0).all()
+    assert np.all(vout[:, 2] == 0.0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps)
+    for k in range(3):
+        a, b = off[k], off[k + 1]
+        o.set_markers(v[a:b], w[a:b], sid[a:b])
+        for _ in range(2):
+            assert o.step(2e-3, 1e-12, 60)[0] == 0
+        ref = o.get_markers()
+        assert np.abs(ref[:, 2]).max() <= 1e-13 * np.abs(ref[:, :2]).max()       # the oracle's v_z is round-off
+        assert rel_l2(vout[a:b, :2], ref[:, :2]) <= 1e-11, k
+        assert rel_l2(vout[a:b, :2] - v[a:b, :2], ref[:, :2] - v[a:b, :2]) <= 1e-8, k
+
+
 def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
     """landau_moments(S_eps) evaluates pass 1 at the current state; the next landau_step starts from exactly that
     state and reuses it (one pass 1 per step instead of two in history runs).  Results must be identical to a run
