@@ -133,6 +133,49 @@ def test_both_passes_at_one_million_markers_sampled_rows(B, oracle_mod):
     assert np.all(np.isfinite(Gg)) and max(errG.values()) <= TOL_FIELD, errG
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_fuzz_mid_size_clouds_sampled_rows(B, oracle_mod, seed):
+    """Randomised clouds of 1e3 .. 5e4 markers: 1-4 species with random masses, charges, temperatures, drifts and ragged
+    counts (no count a multiple of any tile), n_q 2..8 (one to eight node groups of the DMMA contraction), 3-V and
+    native 2-V, whatever pair kernel the size selects.  Pass 1 and the whole field on sampled rows against the oracle's
+    literal Eqs. (22), (23)."""
+    rng = np.random.default_rng(9000 + seed)
+    S = int(rng.integers(1, 5))
+    mass = np.exp(rng.uniform(0.0, 9.0, S)); mass[0] = 1.0
+    charge = rng.choice([-1.0, 1.0, 2.0], S)
+    counts = rng.integers(1, 9000, S)
+    if seed % 5 == 0:
+        counts[0] = int(rng.integers(16000, 40000))
+    T = rng.uniform(0.3, 2.0, S)
+    vs, ws, ss = [], [], []
+    for s in range(S):
+        vs.append(rng.standard_normal((counts[s], 3)) * np.sqrt(T[s] / mass[s])
+                  + rng.normal(0, 0.3, 3) * np.sqrt(T[s] / mass[s]))
+        ws.append((0.2 + rng.random(counts[s])) / counts[s])
+        ss.append(np.full(counts[s], s, dtype=np.int32))
+    v, w, sid = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss)
+    perm = rng.permutation(len(w))
+    v, w, sid = v[perm], w[perm], sid[perm]
+    eps = rng.uniform(0.03, 0.2, S) * T / mass
+    n_q = int(rng.integers(2, 9))
+    two_v = seed % 7 == 3
+    if two_v:
+        v[:, 2] = 0.0
+    g = B.Landau(mass, charge, eps, n_q=n_q)
+    o = oracle_mod.LandauRef(mass, charge, eps, n_q=n_q)
+    if two_v:
+        g.set_dimension(2)
+    G = g.entropy_grad(v, w, sid).cpu().numpy()
+    rows = np.sort(rng.choice(len(w), min(24, len(w)), replace=False)).astype(np.int64)
+    eG = rel_l2(G[rows], o.entropy_grad_rows(v, w, sid, rows))
+    V = g.eval_field(v, w, sid).cpu().numpy()
+    eV = rel_l2(V[rows], o.pair_field_rows(v, w, sid, G, rows))
+    print(f"fuzz {seed}: S={S} N={len(w)} n_q={n_q} {'2-V' if two_v else '3-V'} [{g.last_kernels()}] G {eG:.1e} V {eV:.1e}")
+    assert np.all(np.isfinite(V)) and eG <= TOL_FIELD and eV <= 10 * TOL_FIELD, (seed, eG, eV)
+    if two_v:
+        assert np.all(G[:, 2] == 0.0) and np.all(V[:, 2] == 0.0)
+
+
 @pytest.mark.parametrize("cfg,nps", [(4, 1 << 16), (3, 32768)])
 def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod, cfg, nps):
     """One converged landau_step at the bench workload (3 x 2^16 markers, symmetric kernel, the launch sequence
