@@ -147,13 +147,15 @@ int landau_set_cutoff(landau_ctx* ctx, int on, int morton);
 int landau_cutoff_stats(landau_ctx* ctx, int64_t* tiles_considered, int64_t* tiles_skipped);
 
 /* How landau_step / landau_run issue a step whose cost is launch latency (small clouds).  mode 1 (default,
- * automatic): clouds of <= 65536 padded slots replay the whole step as ONE CUDA graph whose fixed-point body is a
- * conditional WHILE node kept alive from the device (cudaGraphSetConditional in the update kernel) -- no launch
- * per iteration, no pre-enqueued iterations that exit at once.  mode 0: always the plain launch sequence
- * (max_iter iterations enqueued up front, early exit on the device flag).  mode 2: graph at any size.  Same
- * kernels and bit-identical results either way (for every solver of landau_set_solver); the graph is captured
- * after the first ordinary step, is reused while shapes and parameters stay the same, and is not used while
- * landau_profile_enable is on. */
+ * automatic): clouds of <= 32768 padded slots on the one-sided pair kernel with the paper's Jacobi iteration (no stiff-
+ * pair treatment) run ALL iterations of a step inside one persistent kernel with grid-wide barriers (cooperative
+ * launch; step_small.cuh); other clouds of <= 65536 padded slots replay the whole step as ONE CUDA graph whose fixed-
+ * point body is a conditional WHILE node kept alive from the device (cudaGraphSetConditional in the update kernel) --
+ * no launch per iteration, no pre-enqueued iterations that exit at once.  mode 0: always the plain launch sequence
+ * (max_iter iterations enqueued up front, early exit on the device flag).  mode 2: the graph at any size (never the
+ * persistent kernel).  The same kernel bodies in the same summation orders and bit-identical results in every mode
+ * (for every solver of landau_set_solver); the graph is captured after the first ordinary step, is reused while shapes
+ * and parameters stay the same, and neither graph nor persistent kernel is used while landau_profile_enable is on. */
 int landau_set_step_graph(landau_ctx* ctx, int mode);
 
 /* SURVEY.md NEXT-4 (robustness): what landau_step / landau_run do with a step whose fixed point does not converge

@@ -24,6 +24,7 @@
 #include "pair.cuh"
 #include "pair_sym.cuh"
 #include "step.cuh"
+#include "step_small.cuh"
 #include "step_dg.cuh"
 #include "step_anderson.cuh"
 #include "step_newton.cuh"
@@ -100,6 +101,8 @@ struct landau_ctx {
     bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {}, attr_mma2v[LD_MAX_NQ + 1] = {};
     bool attr_sym64_2v = false;
     size_t attr_cells[LD_MAX_NQ + 1] = {}, attr_cells_small = 0;
+    int small_occ[2][2] = {};                    // resident CTAs per SM of step_small_kernel<R, DIM> (0 = not asked yet)
+    bool coop_ok = false;                        // the device supports cooperative launches
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson, 2 Newton-Krylov (NEXT-4)
@@ -584,6 +587,21 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     return 0;
 }
 
+#ifndef LANDAU_ONESIDED_WAVES  // tuning knob (build.py: LANDAU_NVCC_EXTRA): blocks per SM the source chunking aims at
+#define LANDAU_ONESIDED_WAVES 8
+#endif
+// Grid of the one-sided pair kernel for a cloud: targets per thread, target tiles, source chunks.
+void onesided_grid(const landau_ctx* c, const Cloud& cl, int* R, int* ttiles, int* nchunks) {
+    // targets per thread: 2, or 1 for the smallest clouds (more blocks matter more than source reuse there)
+#ifndef LANDAU_ONESIDED_R1_MAX   // tuning knob (build.py: LANDAU_NVCC_EXTRA)
+#define LANDAU_ONESIDED_R1_MAX 4096
+#endif
+    *R = cl.npad_max <= LANDAU_ONESIDED_R1_MAX ? 1 : 2;
+    *ttiles = ceil_div(cl.npad_max, PAIR_THREADS * *R);
+    const int stiles = cl.npad_max / PAIR_SRC_TILE;
+    *nchunks = std::min(32, std::max(1, std::min(stiles, ceil_div(LANDAU_ONESIDED_WAVES * c->sm_count, *ttiles))));
+}
+
 // ---- a3: pairwise field of source records -> partial fields ---------------------------------
 // Returns the number of partial slices written to c->vpart (to be summed in index order).
 // detect: 0 = plain evaluation; 1 = this is the first evaluation of a step with the stiff-pair treatment on (find
@@ -648,15 +666,8 @@ int pair(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, int* nparts_out, int de
         *nparts_out = nchunks;
         return 0;
     }
-#ifndef LANDAU_ONESIDED_WAVES  // tuning knob (build.py: LANDAU_NVCC_EXTRA): blocks per SM the source chunking aims at
-#define LANDAU_ONESIDED_WAVES 8
-#endif
-    // targets per thread: 2, or 1 for the smallest clouds (more blocks matter more than source reuse there)
-    const int R = cl.npad_max <= 1024 ? 1 : 2;
-    const int ttiles = ceil_div(cl.npad_max, PAIR_THREADS * R);
-    const int stiles = cl.npad_max / PAIR_SRC_TILE;
-    int nchunks = std::max(1, std::min(stiles, ceil_div(LANDAU_ONESIDED_WAVES * c->sm_count, ttiles)));
-    nchunks = std::min(nchunks, 32);
+    int R, ttiles, nchunks;
+    onesided_grid(c, cl, &R, &ttiles, &nchunks);
     RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
     dim3 grid(ttiles, nchunks);
     if (detect) {
@@ -1053,6 +1064,57 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
 }  // namespace
 
 namespace {
+// Launch-bound clouds (step_small.cuh): all Jacobi iterations of a step in one persistent kernel.  Returns 1 if the
+// kernel was launched, 0 if this cloud / configuration does not qualify (the caller takes the graph or the launch
+// sequence), < 0 on error.
+template <int R, int DIM>
+int launch_step_small_rd(landau_ctx* c, Cloud& cl, const StepBufs& b, int ttiles, int nchunks, double dt, double tol,
+                                int max_iter) {
+    auto kern = step_small_kernel<R, DIM>;
+    int& occ = c->small_occ[R - 1][DIM - 2];
+    if (!occ) {
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, PAIR_THREADS, 0));
+        if (occ < 1) occ = -1;
+    }
+    const int G = ttiles * nchunks;
+    if (occ < 0 || G > occ * c->sm_count) return 0;               // every CTA must be resident (grid-wide barriers)
+    const DevTable* T = c->d_tab; DevLayout* L = cl.L(); StepCtrl* ctrl = c->d_ctrl;
+    int npm = b.npm;
+    double* rec = cl.recs(); double* vpart = (double*)c->vpart.p;
+    const double *xn = cl.x(), *yn = cl.y(), *zn = cl.z(), *w = cl.w();
+    double *xk = b.xk, *yk = b.yk, *zk = b.zk, *bp = (double*)c->blockpart.p;
+    unsigned int* bar = &c->d_ctrl->ticket;                        // zeroed by step_begin_kernel
+    void* args[] = {&T, &L, &ctrl, &npm, &ttiles, &nchunks, &dt, &tol, &max_iter, &rec, &vpart, &xn, &yn, &zn, &w,
+                    &xk, &yk, &zk, &bp, &bar};
+    CU(cudaLaunchCooperativeKernel((const void*)kern, dim3(G), dim3(PAIR_THREADS), args, 0, c->stream));
+    c->launches += 1;
+    return 1;
+}
+
+bool step_small_eligible(const landau_ctx* c, const Cloud& cl) {
+    return c->graph_mode == 1 && !c->prof_on && c->solver == 0 && !stiff_active(c) && !cl.sym && c->precision == 0 &&
+           c->coop_ok && cl.npad_max <= PAIR_THREADS * UPD_THREADS;
+}
+
+int launch_step_small(landau_ctx* c, Cloud& cl, const StepBufs& b, double dt, double tol, int max_iter) {
+    int R, ttiles, nchunks;
+    onesided_grid(c, cl, &R, &ttiles, &nchunks);
+    RC(ensure(c, c->vpart, sizeof(double) * 3 * (size_t)nchunks * cl.npad_max));
+    int rc;
+    if (c->dim == 2) rc = R == 1 ? launch_step_small_rd<1, 2>(c, cl, b, ttiles, nchunks, dt, tol, max_iter)
+                                 : launch_step_small_rd<2, 2>(c, cl, b, ttiles, nchunks, dt, tol, max_iter);
+    else             rc = R == 1 ? launch_step_small_rd<1, 3>(c, cl, b, ttiles, nchunks, dt, tol, max_iter)
+                                 : launch_step_small_rd<2, 3>(c, cl, b, ttiles, nchunks, dt, tol, max_iter);
+    if (rc == 1) {
+        c->k_pair = c->dim == 2 ? "onesided2v" : "onesided";
+        snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
+    }
+    return rc;
+}
+
+}  // namespace
+
+namespace {
 // NEXT-3: many collision cells, one persistent CTA per cell, whole run in one launch (cells.cuh).
 template <int NQ, int MINB>
 int launch_cells_v(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
@@ -1139,6 +1201,7 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     DevGuard dev_guard(c);                 // the caller's current device is left untouched
     { int cur = -1; if (cudaGetDevice(&cur) != cudaSuccess || cur != c->device) { delete c; return LANDAU_ECUDA; } }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
+    { int coop = 0; cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device); c->coop_ok = coop != 0; }
     DevTable t;
     memset(&t, 0, sizeof(t));
     t.S = S; t.n_q = c->n_q; t.pad = 128; t.dim = 3;
@@ -1351,11 +1414,20 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
     }
     const bool graph_ok = !hold && c->graph_mode != 0 && !c->sg.failed && !c->prof_on &&
                           (c->graph_mode == 2 || npm <= 65536);
-    std::vector<char> via_graph(n_steps, 0);
+    std::vector<char> via_graph(n_steps, 0), via_small(n_steps, 0);
+    bool small_ok = step_small_eligible(c, cl);
     for (int n = 0; n < n_steps; ++n) {
         c->prof_step = n; c->prof_iter = 0;
         if (!cl.G_valid) RC(entropy(c, cl));     // a preceding landau_moments(S_eps) already evaluated pass 1 here
         cl.G_valid = false;                      // the step moves the markers
+        if (small_ok) {
+            // vpart must have its final size before step_begin (nothing else allocates in a fused step)
+            RC(enqueue_step_begin(c, cl, sb));
+            const int rs = launch_step_small(c, cl, sb, dt, tol, max_iter);
+            if (rs < 0) return rs;
+            if (rs == 1) { enqueue_step_commit(c, cl, sb); via_small[n] = 1; continue; }
+            small_ok = false;                    // not resident: the graph / launch sequence from here on (begin is idempotent)
+        }
         if (graph_ok && step_graph_matches(c, cl, dt, tol, max_iter)) {
             CU(cudaGraphLaunch(c->sg.exec, st));
             c->launches += c->sg.fixed_nodes;
@@ -1387,7 +1459,7 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
         for (int n = 0; n < n_steps; ++n) its[n] = h[n].iterations;
         prof_resolve(c, its.data(), n_steps);
     }
-    c->k_step = via_graph[n_steps - 1] ? "graph" : "launch";
+    c->k_step = via_small[n_steps - 1] ? "fused" : (via_graph[n_steps - 1] ? "graph" : "launch");
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s step=%s", c->k_pair, c->k_entropy, c->k_step);
     int any_unconverged = 0;
     for (int n = 0; n < n_steps; ++n) {

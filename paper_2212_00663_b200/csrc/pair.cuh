@@ -44,25 +44,22 @@ __device__ __forceinline__ void pair_accumulate2(double zx, double zy, double cx
     ay = fma(a, fma(-zy, h, cy), ay);
 }
 
-// grid = (target tiles, source chunks).  Each thread owns R targets (slots tile*128R + r*128 + tid).
-// Partial fields are written chunk-major: vpart[((chunk*3 + d) * npad_max) + slot], already scaled
-// by nu_ss'/m_s, so that the combine step is a fixed-order sum over chunks.
-template <int R, int DIM = 3, bool DETECT = false>
-__global__ void __launch_bounds__(PAIR_THREADS)
-pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
-                     const StepCtrl* __restrict__ ctrl, int npad_max, int nchunks,
-                     const double* __restrict__ rec, double* __restrict__ vpart, int gate = GATE_NONE,
-                     StiffCtrl* stiff = nullptr, int* stiff_mark = nullptr) {
-    if (ctrl && ctrl->done) return;
-    if (gate_closed(ctrl, gate)) return;
+// Loads of data another CTA of the SAME launch may have written (the fused small-cloud step, step_small.cuh) bypass L1.
+template <bool COH>
+__device__ __forceinline__ double2 ld_d2(const double2* p) { return COH ? __ldcg(p) : *p; }
+
+// Body of the one-sided kernel for target tile bx and source chunk by.  Each thread owns R targets (slots
+// bx*128R + r*128 + tid).  Partial fields are written chunk-major: vpart[((chunk*3 + d) * npad_max) + slot], already
+// scaled by nu_ss'/m_s, so that the combine step is a fixed-order sum over chunks.  sm: [PAIR_SRC_TILE * 8] doubles.
+template <int R, int DIM, bool DETECT, bool COH>
+__device__ __forceinline__ void pair_onesided_body(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
+                                                   int npad_max, int nchunks, const double* rec, double* vpart,
+                                                   StiffCtrl* stiff, int* stiff_mark, int bx, int by, double* sm,
+                                                   const double* s_nu) {
     const int npad = L->npad;
-    const int slot0 = blockIdx.x * (PAIR_THREADS * R);
+    const int slot0 = bx * (PAIR_THREADS * R);
     if (slot0 >= npad) return;
     const int S = T->S;
-    __shared__ __align__(16) double sm[PAIR_SRC_TILE * 8];
-    __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
-    for (int i = threadIdx.x; i < S * S; i += PAIR_THREADS) s_nu[i] = T->nu[i];
-
     double px[R], py[R], pz[R], gx[R], gy[R], gz[R];
     double tx[R], ty[R], tz[R], pw[R];
     int sp[R], ps[R];
@@ -72,7 +69,7 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
         ps[r] = p < npad ? p : -1;
         if (p >= npad) p = npad - 1;              // clamped duplicate; its result is not written
         const double2* rp = reinterpret_cast<const double2*>(rec + (size_t)p * 8);
-        const double2 a = rp[0], b = rp[1], c = rp[2], d = rp[3];
+        const double2 a = ld_d2<COH>(rp), b = ld_d2<COH>(rp + 1), c = ld_d2<COH>(rp + 2), d = ld_d2<COH>(rp + 3);
         px[r] = a.x; py[r] = a.y; pz[r] = b.x; pw[r] = b.y;   // (the weight is only used by the stiff-pair detection)
         gx[r] = c.x; gy[r] = c.y; gz[r] = d.x;
         tx[r] = ty[r] = tz[r] = 0.0;
@@ -81,14 +78,14 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
 
     const int ntiles = npad / PAIR_SRC_TILE;
     const int tpc = ceil_div(ntiles, nchunks);
-    const int t0 = blockIdx.y * tpc, t1 = min(ntiles, t0 + tpc);
+    const int t0 = by * tpc, t1 = min(ntiles, t0 + tpc);
     for (int t = t0; t < t1; ++t) {
         __syncthreads();
         {
             const double2* src = reinterpret_cast<const double2*>(rec + (size_t)t * PAIR_SRC_TILE * 8);
             double2* dst = reinterpret_cast<double2*>(sm);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) dst[threadIdx.x + k * PAIR_THREADS] = src[threadIdx.x + k * PAIR_THREADS];
+            for (int k = 0; k < 4; ++k) dst[threadIdx.x + k * PAIR_THREADS] = ld_d2<COH>(src + threadIdx.x + k * PAIR_THREADS);
         }
         __syncthreads();
         const int sb = species_of_slot(L, S, t * PAIR_SRC_TILE);
@@ -130,12 +127,28 @@ pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict
         const int p = slot0 + r * PAIR_THREADS + threadIdx.x;
         if (p < npad) {
             const double im = T->inv_mass[sp[r]];
-            double* o = vpart + (size_t)blockIdx.y * 3 * (size_t)npad_max + p;
+            double* o = vpart + (size_t)by * 3 * (size_t)npad_max + p;
             o[0] = tx[r] * im;
             o[(size_t)npad_max] = ty[r] * im;
             o[2 * (size_t)npad_max] = tz[r] * im;
         }
     }
+}
+
+// grid = (target tiles, source chunks).
+template <int R, int DIM = 3, bool DETECT = false>
+__global__ void __launch_bounds__(PAIR_THREADS)
+pair_onesided_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
+                     const StepCtrl* __restrict__ ctrl, int npad_max, int nchunks,
+                     const double* __restrict__ rec, double* __restrict__ vpart, int gate = GATE_NONE,
+                     StiffCtrl* stiff = nullptr, int* stiff_mark = nullptr) {
+    if (ctrl && ctrl->done) return;
+    if (gate_closed(ctrl, gate)) return;
+    __shared__ __align__(16) double sm[PAIR_SRC_TILE * 8];
+    __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
+    for (int i = threadIdx.x; i < T->S * T->S; i += PAIR_THREADS) s_nu[i] = T->nu[i];
+    pair_onesided_body<R, DIM, DETECT, false>(T, L, npad_max, nchunks, rec, vpart, stiff, stiff_mark, blockIdx.x, blockIdx.y,
+                                              sm, s_nu);
 }
 
 // FP32 variant of the one-sided kernel (BASELINE config 4, "plus an FP32 field variant"; landau_opts.precision = 1,

@@ -56,6 +56,40 @@ __global__ void step_begin_kernel(const DevTable* __restrict__ T, const DevLayou
     }
 }
 
+// Slot p of the Jacobi update: v^(k+1) = v^n + dt * (fixed-order sum of the partial fields), its share of the residual
+// sums, the next midpoint into the source records.  COH: the partial fields and the iterate were written by other CTAs
+// of the same launch (step_small.cuh) and are read past L1.
+template <bool COH>
+__device__ __forceinline__ void step_update_slot(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
+                                                 int p, int npad_max, int nparts, double dt, const double* vpart,
+                                                 const double* __restrict__ xn, const double* __restrict__ yn,
+                                                 const double* __restrict__ zn, const double* __restrict__ w, double* xk,
+                                                 double* yk, double* zk, double* rec, double* soa, double& num,
+                                                 double& den) {
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int k = 0; k < nparts; ++k) {
+        const double* o = vpart + (size_t)k * 3 * (size_t)npad_max + p;
+        if (COH) { a += __ldcg(o); b += __ldcg(o + (size_t)npad_max); c += __ldcg(o + 2 * (size_t)npad_max); }
+        else { a += o[0]; b += o[(size_t)npad_max]; c += o[2 * (size_t)npad_max]; }
+    }
+    const double wp = w[p];
+    if (wp == 0.0) { a = 0.0; b = 0.0; c = 0.0; }          // dummies stay at the origin
+    const double x0 = xn[p], y0 = yn[p], z0 = zn[p];
+    const double x1 = fma(dt, a, x0), y1 = fma(dt, b, y0), z1 = fma(dt, c, z0);
+    const double dx = x1 - xk[p], dy = y1 - yk[p], dz = z1 - zk[p];      // xk[p] is only ever touched by p's own thread
+    const double wm = wp * T->mass[species_of_slot(L, T->S, p)];
+    num = wm * (dx * dx + dy * dy + dz * dz);
+    den = wm * (x1 * x1 + y1 * y1 + z1 * z1);
+    xk[p] = x1; yk[p] = y1; zk[p] = z1;
+    const double ux = 0.5 * (x0 + x1), uy = 0.5 * (y0 + y1), uz = 0.5 * (z0 + z1);   // Eq. (25)
+    if (rec) {
+        double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
+        o[0] = make_double2(ux, uy);
+        reinterpret_cast<double*>(o + 1)[0] = uz;
+    }
+    if (soa) { soa[p] = ux; soa[(size_t)npad_max + p] = uy; soa[2 * (size_t)npad_max + p] = uz; }
+}
+
 // v^(k+1) = v^n + dt * (fixed-order sum of the partial fields); residual; next midpoint records.
 __global__ void __launch_bounds__(UPD_THREADS)
 step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
@@ -70,29 +104,8 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
     __shared__ int s_last;
     const int p = blockIdx.x * UPD_THREADS + threadIdx.x;
     double num = 0.0, den = 0.0;
-    if (p < npad_max && p < L->npad) {
-        double a = 0.0, b = 0.0, c = 0.0;
-        for (int k = 0; k < nparts; ++k) {
-            const double* o = vpart + (size_t)k * 3 * (size_t)npad_max + p;
-            a += o[0]; b += o[(size_t)npad_max]; c += o[2 * (size_t)npad_max];
-        }
-        const double wp = w[p];
-        if (wp == 0.0) { a = 0.0; b = 0.0; c = 0.0; }          // dummies stay at the origin
-        const double x0 = xn[p], y0 = yn[p], z0 = zn[p];
-        const double x1 = fma(dt, a, x0), y1 = fma(dt, b, y0), z1 = fma(dt, c, z0);
-        const double dx = x1 - xk[p], dy = y1 - yk[p], dz = z1 - zk[p];
-        const double wm = wp * T->mass[species_of_slot(L, T->S, p)];
-        num = wm * (dx * dx + dy * dy + dz * dz);
-        den = wm * (x1 * x1 + y1 * y1 + z1 * z1);
-        xk[p] = x1; yk[p] = y1; zk[p] = z1;
-        const double ux = 0.5 * (x0 + x1), uy = 0.5 * (y0 + y1), uz = 0.5 * (z0 + z1);   // Eq. (25)
-        if (rec) {
-            double2* o = reinterpret_cast<double2*>(rec + (size_t)p * 8);
-            o[0] = make_double2(ux, uy);
-            reinterpret_cast<double*>(o + 1)[0] = uz;
-        }
-        if (soa) { soa[p] = ux; soa[(size_t)npad_max + p] = uy; soa[2 * (size_t)npad_max + p] = uz; }
-    }
+    if (p < npad_max && p < L->npad)
+        step_update_slot<false>(T, L, p, npad_max, nparts, dt, vpart, xn, yn, zn, w, xk, yk, zk, rec, soa, num, den);
     num = warp_sum(num); den = warp_sum(den);
     const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
     if (lane == 0) { s_num[wv] = num; s_den[wv] = den; }

@@ -1047,6 +1047,43 @@ def test_step_reuses_the_pass1_of_moments(B, oracle_mod):
     np.testing.assert_array_equal(ga.moments()["S_eps"], gb.moments()["S_eps"])
 
 
+@pytest.mark.parametrize("cfg,n,dim", [(0, 256, 3), (4, 300, 3), (0, 1000, 2), (1, 1900, 3), (4, 37, 3)])
+def test_fused_small_cloud_step_is_bit_identical_to_the_launch_sequence(B, cfg, n, dim):
+    """Launch-bound clouds (default mode of landau_set_step_graph) run every Jacobi iteration of a step inside ONE
+    persistent kernel with grid-wide barriers (step_small.cuh).  It executes the bodies of the pair and update kernels
+    in their own summation orders, so states, iteration counts and residuals are bit-identical to the plain launch
+    sequence -- 3-V and 2-V, one and two targets per thread, steps that end at max_iter included."""
+    wl = W.make(cfg, n_per_species=n, shuffled=True)
+    v = wl.v.copy()
+    if dim == 2:
+        v[:, 2] = 0.0
+    ga = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gb = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    if dim == 2:
+        ga.set_dimension(2); gb.set_dimension(2)
+    ga.set_step_graph(1)
+    gb.set_step_graph(0)
+    for rep in range(2):
+        ga.set_markers(v, wl.w, wl.species_id)
+        gb.set_markers(v, wl.w, wl.species_id)
+        ra = [ga.step(wl.dt, wl.tol, wl.max_iter) for _ in range(3)]
+        rb = [gb.step(wl.dt, wl.tol, wl.max_iter) for _ in range(3)]
+        assert ra == rb
+        assert "step=fused" in ga.last_kernels() and "step=launch" in gb.last_kernels()
+        rca, ia = ga.run(4, wl.dt, wl.tol, wl.max_iter)
+        rcb, ib = gb.run(4, wl.dt, wl.tol, wl.max_iter)
+        assert rca == rcb and ia == ib
+        assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+    ga.set_markers(v, wl.w, wl.species_id); gb.set_markers(v, wl.w, wl.species_id)
+    assert ga.step(wl.dt, 1e-15, 3) == gb.step(wl.dt, 1e-15, 3)    # ends at max_iter
+    assert np.array_equal(ga.get_markers().cpu().numpy(), gb.get_markers().cpu().numpy())
+    # other solvers and the stiff-pair treatment keep the graph / launch sequence
+    ga.set_solver(1, 3)
+    ga.set_markers(v, wl.w, wl.species_id)
+    ga.step(wl.dt, wl.tol, wl.max_iter); ga.step(wl.dt, wl.tol, wl.max_iter)
+    assert "step=fused" not in ga.last_kernels()
+
+
 @pytest.mark.parametrize("cfg,n", [(0, 256), (4, 300), (1, 4096), (4, 8000)])
 def test_graph_step_is_bit_identical_to_the_launch_sequence(B, cfg, n):
     """Small clouds replay the step as a CUDA graph with a device-driven WHILE node (landau_set_step_graph);
