@@ -511,14 +511,20 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
                              : std::min(literal_groups(nq), use_mma ? mma_groups(nq) : fact_groups(nq));
     // enough blocks for >= ~20 waves of 2 resident blocks per SM, so that the last wave costs < 5 %
     int nchunks = ceil_div(40 * c->sm_count, ttiles * ig);
-    nchunks = std::max(1, std::min(nchunks, std::max(1, cl.npad_max / (c->S * 256))));   // >= 4 source tiles per chunk
+#ifndef LANDAU_PASS1_MIN_TILES   // tuning knob (build.py: LANDAU_NVCC_EXTRA): source tiles of 64 per chunk, at least
+#define LANDAU_PASS1_MIN_TILES 4
+#endif
+    // (launch-bound clouds of <= 4096 slots: half of that -- more, smaller blocks; measured on the paper's 2048-marker tests)
+    const int min_tiles = cl.npad_max <= 4096 ? std::max(1, LANDAU_PASS1_MIN_TILES / 2) : LANDAU_PASS1_MIN_TILES;
+    const int chunk_cap = std::max(1, cl.npad_max / (c->S * 64 * min_tiles));
+    nchunks = std::max(1, std::min(nchunks, chunk_cap));
     nchunks = std::min(nchunks, 64);
     while (nchunks > 1 && (size_t)nchunks * M * cl.npad_max * sizeof(double) > ((size_t)2 << 30)) --nchunks;
     if (use_mma && nchunks >= 3) {
         // wave quantisation: 2 blocks are resident per SM, and a last wave that fills a few SMs costs a whole block
         // time (3 x 2^16 markers: 4 chunks = 21.08 waves, the 22nd wave 4 % of the kernel).  Take the chunk count
         // near the first guess whose block count is closest below a whole number of waves.
-        const int hi = std::min({64, 2 * nchunks, std::max(1, cl.npad_max / (c->S * 256))});
+        const int hi = std::min({64, 2 * nchunks, chunk_cap});
         double best = 1e30;
         int pick = nchunks;
         for (int k = std::max(2, nchunks - 1); k <= hi; ++k) {
