@@ -648,7 +648,10 @@ def test_stiff_pairs_are_solved_where_the_plain_iteration_cycles(B, oracle_mod, 
     wm = (wl.w * wl.mass[wl.species_id])[:, None]
     assert np.sqrt((wm * defect ** 2).sum() / (wm * v1 ** 2).sum()) <= 2e-12
     e = np.flatnonzero(wl.species_id == 0)[:len(offsets) + 1]
-    assert np.abs(defect[e]).max() <= 1e-9 * np.abs(v1[e] - wl.v[e]).max()    # the eliminated markers themselves
+    # the eliminated markers themselves: 1e-9 of their displacement, plus what the stopping rule itself resolves (the
+    # iteration ends at a residual of tol = 1e-12 RELATIVE TO THE STATE, reading S7: tol |v| is 2.7e-12 here, twice the
+    # first term; which side of 1e-9 x displacement a run lands on depends on the summation order of pass 1)
+    assert np.abs(defect[e]).max() <= 1e-9 * np.abs(v1[e] - wl.v[e]).max() + 1e-12 * np.abs(v1[e]).max()
     m1 = g.moments(with_entropy=False)
     wm_abs = (wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(1)).sum()
     assert np.abs(m1["P"].sum(0) - m0["P"].sum(0)).max() <= TOL_DRIFT * wm_abs
