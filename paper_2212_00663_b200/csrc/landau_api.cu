@@ -1092,7 +1092,14 @@ int launch_step_small_rd(landau_ctx* c, Cloud& cl, const StepBufs& b, int ttiles
     unsigned int* bar = &c->d_ctrl->ticket;                        // zeroed by step_begin_kernel
     void* args[] = {&T, &L, &ctrl, &npm, &ttiles, &nchunks, &dt, &tol, &max_iter, &rec, &vpart, &xn, &yn, &zn, &w,
                     &xk, &yk, &zk, &bp, &bar};
-    CU(cudaLaunchCooperativeKernel((const void*)kern, dim3(G), dim3(PAIR_THREADS), args, 0, c->stream));
+    const cudaError_t ce = cudaLaunchCooperativeKernel((const void*)kern, dim3(G), dim3(PAIR_THREADS), args, 0, c->stream);
+    if (ce == cudaErrorCooperativeLaunchTooLarge || ce == cudaErrorNotSupported) {
+        // fewer SMs than the occupancy query assumed (e.g. an MPS partition): the graph / launch sequence instead
+        cudaGetLastError();
+        occ = -1;
+        return 0;
+    }
+    CU(ce);
     c->launches += 1;
     return 1;
 }
