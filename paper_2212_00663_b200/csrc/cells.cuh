@@ -59,6 +59,7 @@ struct CellsCfg {
 };
 
 // Fixed-order block sum of two values (warp shuffles, then warp 0 adds the warp totals in index order).
+template <int NT = CELLS_THREADS>
 __device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_red) {
     a = warp_sum(a); b = warp_sum(b);
     const int lane = threadIdx.x & 31, wv = threadIdx.x >> 5;
@@ -66,7 +67,7 @@ __device__ __forceinline__ void cells_reduce2(double& a, double& b, double* s_re
     if (lane == 0) { s_red[2 * wv] = a; s_red[2 * wv + 1] = b; }
     __syncthreads();
     double x = 0.0, y = 0.0;
-    for (int k = 0; k < CELLS_THREADS / 32; ++k) { x += s_red[2 * k]; y += s_red[2 * k + 1]; }
+    for (int k = 0; k < NT / 32; ++k) { x += s_red[2 * k]; y += s_red[2 * k + 1]; }
     a = x; b = y;
 }
 
@@ -392,18 +393,20 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
     }
 }
 
-// MINB = 1: any cell up to the shared-memory capacity, one CTA per SM (255 registers: register-tiled pair loops, DMMA
-// accumulators).  MINB = 2 (n_q = 4, every cell of the batch <= CELLS_SMALL markers): only the small-cell paths (2 or 4
-// threads per target) are compiled, 128 registers, two CTAs per SM -- such cells are bound by the latencies of their
-// barriers and reductions, not by the FP64 pipe, and a second resident cell fills the gaps.
+// MINB = 1: any cell up to the shared-memory capacity, one CTA of 256 threads per SM (255 registers: register-tiled pair
+// loops, DMMA accumulators).  MINB > 1 (n_q = 4, every cell of the batch <= NT / 2 markers): only the small-cell paths (2
+// or 4 threads per target) are compiled, 128 registers; <4, 2, 256>: cells of <= 128 markers, two CTAs per SM;
+// <4, 4, 128>: cells of <= 64 markers, four CTAs of 128 threads per SM -- such cells are bound by the latencies of their
+// barriers and reductions, not by the FP64 pipe, and more resident cells fill the gaps.
 constexpr int CELLS_SMALL = CELLS_THREADS / 2;
 
-template <int NQ, int MINB = 1>
-__global__ void __launch_bounds__(CELLS_THREADS, MINB)
+template <int NQ, int MINB = 1, int NT = CELLS_THREADS>
+__global__ void __launch_bounds__(NT, MINB)
 cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const long long* __restrict__ cell_off,
                  const double* __restrict__ v, const double* __restrict__ w, const int32_t* __restrict__ sid,
                  double* __restrict__ v_out, int n_steps, double dt, double tol, int max_iter,
                  int* __restrict__ next_cell, CellRecord* __restrict__ records) {
+    static_assert(MINB > 1 || NT == CELLS_THREADS, "the register-tiled paths are written for 256 threads");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* xn = reinterpret_cast<double*>(smem_raw);
     double* yn = xn + cap; double* zn = yn + cap; double* ww = zn + cap;
@@ -414,16 +417,16 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
     double* s_e2 = tab + (size_t)CellsCfg<NQ>::TAB * cap; // [64]
     double* s_red = s_e2 + 64;                            // [32]
     double* s_part = s_red + 32;                          // [GF][3][TPG] partial sums of split targets (small cells)
-    int* idx = reinterpret_cast<int*>(s_part + 3 * CELLS_THREADS);   // [cap] caller index (within the cell) of slot p
+    int* idx = reinterpret_cast<int*>(s_part + 3 * NT);   // [cap] caller index (within the cell) of slot p
     __shared__ int s_off[LD_MAX_SPECIES + 1];
-    __shared__ int s_wcnt[CELLS_THREADS / 32];
+    __shared__ int s_wcnt[NT / 32];
     __shared__ int s_cell, s_status;
     __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
 
     const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
     const int S = T->S;
     if (tid < 64) s_e2[tid] = T->exp2_tab[tid];
-    for (int i = tid; i < S * S; i += CELLS_THREADS) s_nu[i] = T->nu[i];
+    for (int i = tid; i < S * S; i += NT) s_nu[i] = T->nu[i];
     double kn[NQ], ga[NQ];
 #pragma unroll
     for (int i = 0; i < NQ; ++i) { kn[i] = T->knot[i]; ga[i] = T->gw[i]; }
@@ -442,9 +445,9 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
         rec.status = 0; rec.iterations = 0; rec.max_iterations = 0; rec.steps_not_converged = 0; rec.residual = 0.0;
         auto pass_through = [&]() {                                    // failed cell: output = input
             if (v_out != v && n > 0)
-                for (long long i = tid; i < 3LL * n; i += CELLS_THREADS) v_out[3 * g0 + i] = v[3 * g0 + i];
+                for (long long i = tid; i < 3LL * n; i += NT) v_out[3 * g0 + i] = v[3 * g0 + i];
         };
-        if (n < 1 || n > cap || (MINB > 1 && n > CELLS_SMALL)) {
+        if (n < 1 || n > cap || (MINB > 1 && n > NT / 2)) {
             pass_through();
             if (tid == 0) { rec.status = n == 0 ? 0 : -1; records[cell] = rec; }
             continue;
@@ -453,7 +456,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
         int base = 0;
         for (int s = 0; s < S; ++s) {
             if (tid == 0) s_off[s] = base;
-            for (int c0 = 0; c0 < n; c0 += CELLS_THREADS) {
+            for (int c0 = 0; c0 < n; c0 += NT) {
                 const int i = c0 + tid;
                 int si = -2;
                 if (i < n) { si = sid[g0 + i]; if (si < 0 || si >= S) { si = -2; s_status = -1; } }
@@ -462,7 +465,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 if (lane == 0) s_wcnt[wv] = __popc(m);
                 __syncthreads();
                 int before = 0, total = 0;
-                for (int k = 0; k < CELLS_THREADS / 32; ++k) { if (k < wv) before += s_wcnt[k]; total += s_wcnt[k]; }
+                for (int k = 0; k < NT / 32; ++k) { if (k < wv) before += s_wcnt[k]; total += s_wcnt[k]; }
                 if (mine) {
                     const int p = base + before + __popc(m & ((1u << lane) - 1u));
                     const double a = v[3 * (g0 + i)], b = v[3 * (g0 + i) + 1], c = v[3 * (g0 + i) + 2], wi = w[g0 + i];
@@ -482,8 +485,8 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             continue;
         }
         // threads per target: small cells (NQ = 4 only) put 2 or 4 threads on every target
-        const int GF = (NQ == 4) ? (n <= CELLS_THREADS / 4 ? 4 : (n <= CELLS_THREADS / 2 ? 2 : 1)) : 1;
-        const int TPG = CELLS_THREADS / GF, part = tid / TPG, tg = tid % TPG;
+        const int GF = (NQ == 4) ? (n <= NT / 4 ? 4 : (n <= NT / 2 ? 2 : 1)) : 1;
+        const int TPG = NT / GF, part = tid / TPG, tg = tid % TPG;
         for (int step = 0; step < n_steps && s_status == 0; ++step) {
             // ---- pass 1 (Eq. 22, factorised): G_p for every species, sources = same species of this cell
             for (int s = 0; s < S; ++s) {
@@ -493,7 +496,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 // bounding box -> centre and half-width in mollifier units
                 double lo[3] = {1.7976931348623157e308, 1.7976931348623157e308, 1.7976931348623157e308};
                 double hi[3] = {-1.7976931348623157e308, -1.7976931348623157e308, -1.7976931348623157e308};
-                for (int p = o0 + tid; p < o1; p += CELLS_THREADS) {
+                for (int p = o0 + tid; p < o1; p += NT) {
                     lo[0] = fmin(lo[0], xn[p]); hi[0] = fmax(hi[0], xn[p]);
                     lo[1] = fmin(lo[1], yn[p]); hi[1] = fmax(hi[1], yn[p]);
                     lo[2] = fmin(lo[2], zn[p]); hi[2] = fmax(hi[2], zn[p]);
@@ -510,14 +513,14 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     if (lane == 0) { s_red[2 * wv] = lo[d]; s_red[2 * wv + 1] = hi[d]; }
                     __syncthreads();
                     double a = s_red[0], b = s_red[1];
-                    for (int k = 1; k < CELLS_THREADS / 32; ++k) { a = fmin(a, s_red[2 * k]); b = fmax(b, s_red[2 * k + 1]); }
+                    for (int k = 1; k < NT / 32; ++k) { a = fmin(a, s_red[2 * k]); b = fmax(b, s_red[2 * k + 1]); }
                     cen[d] = 0.5 * a + 0.5 * b;
                     hw = fmax(hw, 0.5 * b - 0.5 * a);
                 }
                 // a cell too wide for the factorised form (reading N3) takes the literal-separable one
                 const bool literal = !(6.0 * kmax * hw * inv <= FACT_EXP_LIMIT);
                 // scaled coordinates (alias of xk..zk) and the per-marker exponential tables
-                for (int p = o0 + tid; p < o1; p += CELLS_THREADS) {
+                for (int p = o0 + tid; p < o1; p += NT) {
                     const double a = (xn[p] - cen[0]) * inv, b = (yn[p] - cen[1]) * inv, c = (zn[p] - cen[2]) * inv;
                     xk[p] = a; yk[p] = b; zk[p] = c;
                     if (!literal) {
@@ -573,7 +576,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                         cells_pass1_dmma4(o0, o1, xk, yk, zk, ww, tab, s_e2, kn, ga, lognorm, pref, T->dim == 2, Gx, Gy, Gz,
                                           &s_status);
                 } else if constexpr (MINB == 1) {
-                    for (int r0 = o0; r0 < o1; r0 += CELLS_THREADS) {
+                    for (int r0 = o0; r0 < o1; r0 += NT) {
                         const int pt = r0 + tid;
                         const int p = min(pt, o1 - 1);                 // clamped duplicate; not written
                         const double px = xk[p], py = yk[p], pz = zk[p];
@@ -604,17 +607,17 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             // ---- Eq. (24): Jacobi fixed point, G^n frozen (g = G/m in place), v^(0) = v^n
             // symmetric in-cell evaluation (cells_field_sym) when nu_ss' = c_s c_s' and the cell has >= 448 markers (measured:
             // below that the idle lanes of the last round cost more than the 26 -> 15 instructions per pair save)
-            const int rounds = ceil_div(n, CELLS_THREADS);
+            const int rounds = ceil_div(n, NT);
 #ifndef LANDAU_CELLS_SYM_MIN     // tuning knob (build.py: LANDAU_NVCC_EXTRA): smallest cell taking the symmetric evaluation
 #define LANDAU_CELLS_SYM_MIN 448
 #endif
             const bool use_sym = GF == 1 && T->nu_rank1 != 0 && n >= LANDAU_CELLS_SYM_MIN;
-            const int n2 = min(rounds * CELLS_THREADS, cap);          // cap is even: pairs of slots exist or not together
+            const int n2 = min(rounds * NT, cap);          // cap is even: pairs of slots exist or not together
             double* const sxa = tab;                                   // [7][cap] sources, then [3][cap] source-side sums
             double* const saa = tab + 7 * (size_t)cap;
             // slot of this thread's r-th target: consecutive slots in the symmetric evaluation, strided otherwise
             auto slot_of = [&](int r) {
-                return use_sym ? (r < rounds ? cells_sym_slot(rounds, rounds == 3 ? 3 : 2, wv, lane, r) : n) : r * CELLS_THREADS + tid;
+                return use_sym ? (r < rounds ? cells_sym_slot(rounds, rounds == 3 ? 3 : 2, wv, lane, r) : n) : r * NT + tid;
             };
             int sp[CELLS_ROUNDS];
             double im[CELLS_ROUNDS], wm[CELLS_ROUNDS];
@@ -649,7 +652,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                 }
             }
             if (use_sym)                                               // zero dummies behind the cell's last marker
-                for (int p = n + tid; p < n2; p += CELLS_THREADS)
+                for (int p = n + tid; p < n2; p += NT)
                     for (int c = 0; c < 7; ++c) sxa[(size_t)c * cap + p] = 0.0;
             __syncthreads();
             int it = 0, conv = 0;
@@ -728,7 +731,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     static_assert(CELLS_ROUNDS == 4, "one branch per number of rounds");
                     int pc4[4], sp4[4];
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) { pc4[r] = min(r * CELLS_THREADS + tid, n - 1); sp4[r] = sp[r]; }
+                    for (int r = 0; r < 4; ++r) { pc4[r] = min(r * NT + tid, n - 1); sp4[r] = sp[r]; }
                     if (rounds == 4) {
                         double tx[4], ty[4], tz[4];
                         cells_field<4>(srec, s_off, s_nu, S, pc4, sp4, tx, ty, tz);
@@ -754,7 +757,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     }
                 }
                 }   // MINB == 1
-                cells_reduce2(num, den, s_red);                        // also the barrier after all reads of u
+                cells_reduce2<NT>(num, den, s_red);                        // also the barrier after all reads of u
 #pragma unroll
                 for (int r = 0; r < CELLS_ROUNDS; ++r) {
                     const int p = slot_of(r);
@@ -774,7 +777,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             __syncthreads();
             if (s_status != 0) break;
             // commit (also when not converged, reading S8)
-            for (int p = tid; p < n; p += CELLS_THREADS) { xn[p] = xk[p]; yn[p] = yk[p]; zn[p] = zk[p]; }
+            for (int p = tid; p < n; p += NT) { xn[p] = xk[p]; yn[p] = yk[p]; zn[p] = zk[p]; }
             rec.iterations += it;
             rec.max_iterations = max(rec.max_iterations, it);
             rec.steps_not_converged += conv ? 0 : 1;
@@ -787,7 +790,7 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             if (tid == 0) { rec.status = s_status; records[cell] = rec; }
             continue;
         }
-        for (int p = tid; p < n; p += CELLS_THREADS) {
+        for (int p = tid; p < n; p += NT) {
             double* o = v_out + 3 * (g0 + idx[p]);
             o[0] = xn[p]; o[1] = yn[p]; o[2] = zn[p];
         }

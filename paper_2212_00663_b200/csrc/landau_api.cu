@@ -100,7 +100,7 @@ struct landau_ctx {
     // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per context (= per device)
     bool attr_sym64 = false, attr_sym32 = false, attr_mma[LD_MAX_NQ + 1] = {}, attr_mma2v[LD_MAX_NQ + 1] = {};
     bool attr_sym64_2v = false;
-    size_t attr_cells[LD_MAX_NQ + 1] = {}, attr_cells_small = 0;
+    size_t attr_cells[LD_MAX_NQ + 1] = {}, attr_cells_small[2] = {};
     int small_occ[2][2] = {};                    // resident CTAs per SM of step_small_kernel<R, DIM> (0 = not asked yet)
     bool coop_ok = false;                        // the device supports cooperative launches
     int dim = 3;                          // landau_set_dimension
@@ -1129,21 +1129,20 @@ int launch_step_small(landau_ctx* c, Cloud& cl, const StepBufs& b, double dt, do
 
 namespace {
 // NEXT-3: many collision cells, one persistent CTA per cell, whole run in one launch (cells.cuh).
-template <int NQ, int MINB>
+template <int NQ, int MINB, int NT>
 int launch_cells_v(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
                    double* v_out, int n_steps, double dt, double tol, int max_iter) {
-    auto kern = cells_run_kernel<NQ, MINB>;
+    auto kern = cells_run_kernel<NQ, MINB, NT>;
     const size_t smem = CellsCfg<NQ>::smem(cap);
-    size_t& attr = MINB == 1 ? c->attr_cells[NQ] : c->attr_cells_small;
+    size_t& attr = MINB == 1 ? c->attr_cells[NQ] : c->attr_cells_small[MINB == 2 ? 0 : 1];
     if (smem > attr) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr = smem;
     }
     int* counter = (int*)((char*)c->cells_off.p + sizeof(long long) * ((size_t)n_cells + 1));
     const int grid = std::min(n_cells, MINB * c->sm_count);
-    kern<<<grid, CELLS_THREADS, smem, c->stream>>>(c->d_tab, n_cells, cap, (const long long*)c->cells_off.p, v, w, sid,
-                                                   v_out, n_steps, dt, tol, max_iter, counter,
-                                                   (CellRecord*)c->cells_rec.p);
+    kern<<<grid, NT, smem, c->stream>>>(c->d_tab, n_cells, cap, (const long long*)c->cells_off.p, v, w, sid,
+                                        v_out, n_steps, dt, tol, max_iter, counter, (CellRecord*)c->cells_rec.p);
     c->launches += 1;
     return 0;
 }
@@ -1151,10 +1150,12 @@ int launch_cells_v(landau_ctx* c, int n_cells, int cap, const double* v, const d
 template <int NQ>
 int launch_cells(landau_ctx* c, int n_cells, int cap, const double* v, const double* w, const int32_t* sid,
                  double* v_out, int n_steps, double dt, double tol, int max_iter) {
-    // a batch of small cells (n_q = 4, every cell <= 128 markers): the two-CTAs-per-SM build of the kernel
+    // batches of small cells (n_q = 4): builds of the kernel with only the small-cell paths and several CTAs per SM
+    if (NQ == 4 && cap <= CELLS_THREADS / 4 && n_cells > 2 * c->sm_count)
+        return launch_cells_v<4, 4, CELLS_THREADS / 2>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
     if (NQ == 4 && cap <= CELLS_SMALL && n_cells > c->sm_count)
-        return launch_cells_v<4, 2>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
-    return launch_cells_v<NQ, 1>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
+        return launch_cells_v<4, 2, CELLS_THREADS>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
+    return launch_cells_v<NQ, 1, CELLS_THREADS>(c, n_cells, cap, v, w, sid, v_out, n_steps, dt, tol, max_iter);
 }
 
 }  // namespace

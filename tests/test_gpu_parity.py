@@ -960,12 +960,14 @@ def test_cells_symmetric_in_cell_evaluation_matches_oracle(B, oracle_mod, case):
         assert dP <= 1e-12 and abs(K1 - K0) / K0 <= 1e-12, (case, k, dP, K1 - K0)
 
 
-def test_cells_batch_of_small_cells_two_ctas_per_sm_matches_oracle(B, oracle_mod):
+@pytest.mark.parametrize("nmax,ncells", [(64, 170), (32, 310)])
+def test_cells_batch_of_small_cells_two_ctas_per_sm_matches_oracle(B, oracle_mod, nmax, ncells):
     """A batch of more cells than SMs whose cells all have <= 128 markers (n_q = 4) runs the two-CTAs-per-SM build of the
-    fused kernel (cells_run_kernel<4, 2>: only the 2- and 4-threads-per-target paths, 128 registers).  170 ragged cells
-    of 1 .. 128 markers, two steps; every cell equals the oracle's steps on that cell alone."""
-    rng = np.random.default_rng(12)
-    sizes = list(rng.integers(1, 65, size=168)) + [64, 1]             # markers per species
+    fused kernel (cells_run_kernel<4, 2, 256>: only the 2- and 4-threads-per-target paths, 128 registers); more than two
+    cells per SM with <= 64 markers each the four-CTAs-per-SM build with 128 threads (<4, 4, 128>).  Ragged cells of
+    1 .. 2 nmax markers, two steps; every cell equals the oracle's steps on that cell alone."""
+    rng = np.random.default_rng(12 + nmax)
+    sizes = list(rng.integers(1, nmax + 1, size=ncells - 2)) + [nmax, 1]   # markers per species
     wl0 = W.make(0, n_per_species=8)
     vs, ws, ss, off = [], [], [], [0]
     for k, n in enumerate(sizes):
@@ -973,7 +975,7 @@ def test_cells_batch_of_small_cells_two_ctas_per_sm_matches_oracle(B, oracle_mod
         vs.append(wl.v); ws.append(wl.w); ss.append(wl.species_id)
         off.append(off[-1] + wl.n_markers)
     v, w, sid, off = np.concatenate(vs), np.concatenate(ws), np.concatenate(ss), np.array(off, dtype=np.int64)
-    assert np.diff(off).max() == 128 and len(sizes) > 148
+    assert np.diff(off).max() == 2 * nmax and len(sizes) > (148 if nmax == 64 else 296)
     g = B.Landau(wl0.mass, wl0.charge, wl0.eps)
     dt, n_steps = 1e-3, 2
     rc, vout, info = g.cells_run(off, v, w, sid, n_steps, dt, 1e-12, 60)
