@@ -36,9 +36,10 @@ struct FactCfg {
 __global__ void __launch_bounds__(1024)
 entropy_bounds_kernel(const DevTable* __restrict__ T, DevLayout* __restrict__ L, const double* __restrict__ x,
                       const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ w,
-                      int cutoff_on, const StepCtrl* __restrict__ stop) {
+                      int cutoff_on, const StepCtrl* __restrict__ stop, unsigned long long* __restrict__ cutstats) {
     if (stop && stop->done) return;
     const int s = blockIdx.x;
+    if (s == 0 && threadIdx.x == 0) { cutstats[0] = 0ull; cutstats[1] = 0ull; }   // counters of this pass (Gaussian cutoff)
     const int p0 = L->off[s], p1 = L->off[s + 1];
     const double BIG = 1.7976931348623157e308;
     double lo[3] = {BIG, BIG, BIG}, hi[3] = {-BIG, -BIG, -BIG};

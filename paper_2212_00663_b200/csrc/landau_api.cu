@@ -540,8 +540,8 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     {
     ProfScope prof(c, 1);
     // species extents (range guard of the factorised forms) and weights (Gaussian cutoff threshold); tile boxes
-    CU(cudaMemsetAsync(c->d_cutstats, 0, 2 * sizeof(unsigned long long), c->stream));
-    entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), c->cutoff_on, stop);
+    entropy_bounds_kernel<<<c->S, 1024, 0, c->stream>>>(c->d_tab, cl.L(), cl.x(), cl.y(), cl.z(), cl.w(), c->cutoff_on, stop,
+                                                         c->d_cutstats);
     entropy_tilebox_kernel<<<cl.npad_max / ENT_SRC_TILE, 64, 0, c->stream>>>(c->d_tab, cl.L(), cl.npad_max, cl.x(), cl.y(),
                                                                              cl.z(), cl.w(), (TileBox*)c->tilebox.p, stop);
     c->launches += 2;
