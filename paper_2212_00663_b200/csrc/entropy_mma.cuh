@@ -32,7 +32,10 @@ namespace landau {
 constexpr int MMA_THREADS = 128;   // 4 warps, 32 targets each
 constexpr int MMA_TILE = 64;       // sources per stage
 constexpr int MMA_MT = 4;          // 8-target blocks per warp
-constexpr int MMA_STAGES = 2;      // product-table tiles in shared memory
+#ifndef LANDAU_MMA_STAGES            // tuning knob (build.py: LANDAU_NVCC_EXTRA); 3 measured: no gain
+#define LANDAU_MMA_STAGES 2
+#endif
+constexpr int MMA_STAGES = LANDAU_MMA_STAGES;      // product-table tiles in shared memory
 constexpr int MMA_LCAP = 1024;     // source tiles per segment of the active-tile list (Gaussian cutoff)
 
 // NZ = NQ: the 3-V tensor grid of n_q^3 nodes.  NZ = 1: the paper's own 2-V setting (landau_set_dimension(2), v_z = 0):
