@@ -279,7 +279,8 @@ class Landau:
         return rc, out, info
 
     def set_step_graph(self, mode: int = 1):
-        """0 = plain launch sequence, 1 = CUDA-graph step for small clouds (default), 2 = CUDA-graph step always."""
+        """0 = plain launch sequence; 1 (default) = launch-bound clouds run all iterations of a step in one persistent
+        kernel, other small clouds replay the step as a CUDA graph; 2 = CUDA-graph step always."""
         self._check(self._lib.landau_set_step_graph(self._h, int(mode)), "landau_set_step_graph")
 
     def set_substep(self, max_halvings: int = 0):
