@@ -83,7 +83,9 @@ def integrate_isotropisation(m, n, T_par0, T_perp0, coupling, t_end, n_sub=20000
 def thermalisation_rate(m_s, m_sb, n_sb, T_s, T_sb, coupling) -> float:
     """1/tau-bar^{s\\s'} of Eq. (45), as printed, with the field-species density
     n_s' (reading U6).  Reading G1: the caption value of Fig. 3 (1.6e-3 s) is this formula's
-    2.83e-3 s divided by sqrt(pi); the normalisation beyond that factor is "parity unpinned".
+    2.83e-3 s divided by sqrt(pi).  The formula, not the caption, is right: a Monte Carlo estimate of the
+    Landau operator's energy-exchange integral for two Maxwellians equals it to 0.1 %
+    (tests/test_analytic.py::test_thermalisation_rate_equals_the_landau_energy_exchange_integral).
     """
     return ((8.0 / 3.0) * math.sqrt(2.0 * math.pi * m_s * m_sb) * coupling * n_sb
             / (m_s * T_sb + m_sb * T_s) ** 1.5)

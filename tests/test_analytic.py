@@ -69,3 +69,44 @@ def test_fit_and_temperatures():
     T = A.temperatures_from_moments([2.0], [0.5], [[0.2, 0.0, 0.0]], [0.77])
     # K = n(3T/2) + |P|^2/(2 m n)
     assert abs(T["T"][0] - (2 / 3) * (0.77 - 0.04 / 2.0) / 0.5) < 1e-15
+
+
+def _mc(n, seed):
+    return np.random.default_rng(seed), n
+
+
+def test_thermalisation_rate_equals_the_landau_energy_exchange_integral():
+    """Pin of Eq. (45) that does not come from the paper: for two drift-free Maxwellians the weak form of
+    the operator (Eqs. 3-4, 16-17 with G = -grad f / f) gives, with Q(z) z = 0,
+        dK_a/dt = -nu_ab (1/T_b - 1/T_a) n_a n_b E[ v . Q(v - v') . v ],   v ~ N(0, T_a/m_a), v' ~ N(0, T_b/m_b),
+    i.e. 1/tau^{a\\b} = 2 nu_ab n_b E[...] / (3 T_a T_b).  A Monte Carlo estimate of that expectation (1e6 samples,
+    ~0.2 % noise) equals the helper to 1 %: Eq. (45) as printed is right (the Fig. 3 caption differs by sqrt(pi) = 77 %)."""
+    rng = np.random.default_rng(45)
+    n = 1_000_000
+    for ma, mb, nb, Ta, Tb, nu in [(1.0, 1836.0, 1.0, 2.0, 1.0, 1.0), (1836.0, 1.0, 1.0, 1.0, 2.0, 1.0),
+                                   (1.0, 3.0, 0.7, 1.0, 1.5, 2.5), (2.0, 2.0, 1.3, 0.5, 0.8, 1.0)]:
+        v = rng.standard_normal((n, 3)) * math.sqrt(Ta / ma)
+        vp = rng.standard_normal((n, 3)) * math.sqrt(Tb / mb)
+        z = v - vp
+        r2, zv, v2 = (z * z).sum(1), (z * v).sum(1), (v * v).sum(1)
+        mc = 2.0 * nu * nb * ((r2 * v2 - zv * zv) / r2 ** 1.5).mean() / (3.0 * Ta * Tb)
+        an = A.thermalisation_rate(ma, mb, nb, Ta, Tb, A.coupling_from_nu(nu))
+        assert abs(mc / an - 1.0) < 0.01, (ma, mb, mc, an)
+
+
+def test_isotropisation_rate_equals_the_landau_moment_integral_both_signs_of_A():
+    """Pin of Eq. (41) and of its continuation to T_par > T_perp (reading U5): for a bi-Maxwellian the
+    same weak form gives  dT_par/dt = (nu n/m) E[ z_z (Q(z) M z)_z ],  z = v - v',  M = diag(m/T_perp, m/T_perp, m/T_par),
+    and Eq. (40) says dT_par/dt = 2 (T_perp - T_par)/tau.  Monte Carlo (1e6 samples) against the helper, 1 %."""
+    rng = np.random.default_rng(41)
+    n = 1_000_000
+    for m, dens, Tpar, Tperp, nu in [(1.0, 1.0, 1.0, 2.0, 1.0), (1.0, 1.0, 2.0, 1.0, 1.0), (3.0, 0.7, 1.0, 1.3, 2.0)]:
+        s = np.sqrt(np.array([Tperp, Tperp, Tpar]) / m)
+        z = rng.standard_normal((n, 3)) * s - rng.standard_normal((n, 3)) * s
+        M = np.array([m / Tperp, m / Tperp, m / Tpar])
+        Mz = z * M
+        r2, zMz = (z * z).sum(1), (z * Mz).sum(1)
+        e = z[:, 2] * (r2 * Mz[:, 2] - z[:, 2] * zMz) / r2 ** 1.5
+        mc = (nu * dens / m) * e.mean() / (2.0 * (Tperp - Tpar))
+        an = A.isotropisation_rate(m, dens, Tpar, Tperp, A.coupling_from_nu(nu))
+        assert abs(mc / an - 1.0) < 0.01, (Tpar, Tperp, mc, an)
