@@ -333,3 +333,43 @@ def test_config0_matches_survey_prototype_values(oracle_mod):
     m1 = o.moments()
     assert abs(m1["K"].sum() - K0) / K0 < 1e-14
     assert abs((m1["S_eps"].sum() - S.sum()) - g["delta_S_eps"][0]) < 6e-6
+
+
+def test_field_reproduces_the_analytic_relaxation_rates_of_maxwellians(oracle_mod):
+    """Physics pin of O3 that comes from neither the oracle nor the paper's printed numbers (north_star: "e-i temperature-
+    relaxation and isotropization rates matching the analytic estimates").  For Maxwellian samples the entropy gradient
+    is known in closed form, G_p = -grad ln f = M v_p with M = m/T (per axis for a bi-Maxwellian), so Eq. (23)
+     alone must reproduce, up to sampling noise ~ N^(-1/2),
+      * the energy exchange of two species, dK_a/dt = -(3/2) n_a (T_a - T_b)/tau^{a\\b}, Eqs. (44)-(45) PAPER.md:271-275
+        (the helper is itself pinned by a Monte Carlo of the operator's weak form, tests/test_analytic.py), with
+        dK_a/dt + dK_b/dt = 0 exactly (Eq. 29);
+      * the isotropisation of one bi-Maxwellian species, dT_par/dt = 2 (T_perp - T_par)/tau, Eqs. (40)-(41) PAPER.md:251-255.
+    A wrong sign, a misplaced 1/m_s, a missing weight or charge factor changes these by O(1); tolerance 5 %."""
+    from paper_2212_00663_b200 import analytic as A
+    rng = np.random.default_rng(23)
+    mass, charge = np.array([1.0, 3.0]), np.array([-1.0, 2.0])
+    T, dens, N = np.array([1.0, 1.5]), np.array([1.0, 0.7]), 3000
+    o = oracle_mod.LandauRef(mass, charge, 0.05 * T / mass)
+    v = np.concatenate([rng.standard_normal((N, 3)) * math.sqrt(T[s] / mass[s]) for s in range(2)])
+    sid = np.repeat(np.arange(2, dtype=np.int32), N)
+    w = np.repeat(dens / N, N)
+    V = o.pair_field(v, w, sid, (mass[sid] / T[sid])[:, None] * v)
+    nu = charge[0] ** 2 * charge[1] ** 2
+    dK = [float((w[sid == a] * mass[a] * (v[sid == a] * V[sid == a]).sum(1)).sum()) for a in range(2)]
+    for a, b in ((0, 1), (1, 0)):
+        want = -1.5 * dens[a] * (T[a] - T[b]) * A.thermalisation_rate(mass[a], mass[b], dens[b], T[a], T[b],
+                                                                     A.coupling_from_nu(nu))
+        assert abs(dK[a] / want - 1.0) < 0.05, (a, dK[a], want)
+    assert dK[0] > 0.0 > dK[1] and abs(dK[0] + dK[1]) <= 1e-13 * abs(dK[0])       # the colder species gains what the other loses
+    # one bi-Maxwellian species
+    m1, n1, Tpar, Tperp, N1 = 2.0, 1.3, 2.0, 1.0, 4000
+    o1 = oracle_mod.LandauRef(np.array([m1]), np.array([1.0]), np.array([0.05]))
+    s = np.sqrt(np.array([Tperp, Tperp, Tpar]) / m1)
+    v1 = rng.standard_normal((N1, 3)) * s
+    w1 = np.full(N1, n1 / N1)
+    V1 = o1.pair_field(v1, w1, np.zeros(N1, dtype=np.int32), v1 * (m1 / np.array([Tperp, Tperp, Tpar])))
+    dTpar = 2.0 * float((w1 * m1 * v1[:, 2] * V1[:, 2]).sum()) / n1
+    want = 2.0 * (Tperp - Tpar) * A.isotropisation_rate(m1, n1, Tpar, Tperp, A.coupling_from_nu(1.0))
+    assert dTpar < 0.0 and abs(dTpar / want - 1.0) < 0.05, (dTpar, want)
+    dTperp = float((w1 * m1 * (v1[:, :2] * V1[:, :2]).sum(1)).sum()) / n1         # mean of the two perpendicular axes
+    assert abs(dTperp + 0.5 * dTpar) <= 1e-12 * abs(dTpar)                        # Eq. (40): energy is conserved
