@@ -272,11 +272,13 @@ __device__ __forceinline__ void cells_field(const double* __restrict__ rec, cons
     }
 }
 
-// Slot of a thread's r-th target in the symmetric evaluation: warp w owns the 32 R slots of sub-tile w, stored as
-// R / RS blocks of 32 groups of RS consecutive slots, so that the lanes of a warp read consecutive 8 RS-byte vectors
-// whatever R is (R = 4 as two blocks of pairs: four consecutive slots per lane would be a 2-way bank conflict).
-__device__ __forceinline__ int cells_sym_slot(int R, int RS, int wv, int lane, int r) {
-    return wv * 32 * R + (r / RS) * 32 * RS + lane * RS + (r % RS);
+// Slot of a thread's r-th target in the symmetric evaluation: warp w owns the G R slots of sub-tile w (G <= 32 groups,
+// lanes >= G idle), stored as R / RS blocks of G groups of RS consecutive slots, so that the lanes of a warp read
+// consecutive 8 RS-byte vectors whatever R is (R = 4 as two blocks of pairs: four consecutive slots per lane would be a
+// 2-way bank conflict).  G = the even number of groups per warp that just covers the cell: a cell of 320 markers walks
+// 20 lane steps per phase, not 32.
+__device__ __forceinline__ int cells_sym_slot(int R, int RS, int G, int wv, int lane, int r) {
+    return wv * G * R + (r / RS) * G * RS + lane * RS + (r % RS);
 }
 
 // Pass 2 of a whole cell in the symmetric (action-reaction) form of pair_sym.cuh: Q(z)(g_p - g_q)/|z| once per
@@ -286,14 +288,14 @@ __device__ __forceinline__ int cells_sym_slot(int R, int RS, int wv, int lane, i
 // target-side sums); warp w's 32 R slots are also "sub-tile" w of the sources.  Phase 0: every warp its own sub-tile (the
 // lane's own group one-sided, every unordered pair of different groups once, both sides).
 // Phases 1..3: warp w against sub-tile (w + ph) % 8, both sides.  Phase 4: the pairs {w, w + 4} are split between the
-// two warps (steps 0..15 / 1..16 of the lane rotation).  Inside a phase lane l visits source group (l + k) % 32 at
+// two warps (steps 0..G/2-1 / 1..G/2 of the lane rotation).  Inside a phase lane l visits source group (l + k) % G at
 // step k -- R consecutive slots, read as 16-byte vectors -- and adds the source-side sums into the shared-memory
 // accumulators next to the sources: in a phase a sub-tile belongs to one warp and at a step every lane holds another
 // group, so there are no conflicts, no atomics, and the order is the program's (deterministic).
 // sx: seven arrays [cap] {ux uy uz W gx gy gz}; sa: [3][cap]; slots n .. n2 (n2 even, <= cap) hold zero dummies.
 template <int R, int RS>
 __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, double* __restrict__ sa, int cap, int n,
-                                                int n2, double (&tx)[R], double (&ty)[R], double (&tz)[R]) {
+                                                int n2, int G, double (&tx)[R], double (&ty)[R], double (&tz)[R]) {
     static_assert(R % RS == 0, "sources of a group are taken RS at a time");
     const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
     const double* X = sx; const double* Y = sx + cap; const double* Z = sx + 2 * (size_t)cap;
@@ -303,8 +305,8 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
     double px[R], py[R], pz[R], gx[R], gy[R], gz[R], wp[R], ax[R], ay[R], az[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int p = cells_sym_slot(R, RS, wv, lane, r);
-        const bool ok = p < n2;
+        const int p = cells_sym_slot(R, RS, G, wv, lane, r);
+        const bool ok = lane < G && p < n2;
         px[r] = ok ? X[p] : 0.0; py[r] = ok ? Y[p] : 0.0; pz[r] = ok ? Z[p] : 0.0;
         gx[r] = ok ? HX[p] : 0.0; gy[r] = ok ? HY[p] : 0.0; gz[r] = ok ? HZ[p] : 0.0;
         wp[r] = ok ? Wt[p] : 0.0;
@@ -316,20 +318,22 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
 #pragma unroll 1
     for (int ph = 0; ph <= NW / 2; ++ph) {
         const int u = (wv + ph) & (NW - 1);
-        // phase 0 (own sub-tile): step 0 = the lane's own group, one-sided; steps 1..15 both sides; step 16 both sides
-        // by the lower half of the lanes only (the pair of groups {l, l + 16} is seen from both ends)
-        int k0 = 0, k1 = 32;
-        if (ph == 0) k1 = 17;
-        if (ph == NW / 2) { if (wv < NW / 2) k1 = 16; else { k0 = 1; k1 = 17; } }
+        // phase 0 (own sub-tile): step 0 = the lane's own group, one-sided; steps 1..G/2-1 both sides; step G/2 both
+        // sides by the lower half of the lanes only (the pair of groups {l, l + G/2} is seen from both ends)
+        const int GH = G >> 1;
+        int k0 = 0, k1 = G;
+        if (ph == 0) k1 = GH + 1;
+        if (ph == NW / 2) { if (wv < NW / 2) k1 = GH; else { k0 = 1; k1 = GH + 1; } }
 #pragma unroll 1
         for (int k = k0; k < k1; ++k) {
-            const int gl = (lane + k) & 31;                            // the group this lane visits
+            const int gk = lane + k;
+            const int gl = gk >= G ? gk - G : gk;                      // the group this lane visits: (lane + k) mod G
             const bool one = ph == 0 && k == 0;
-            const bool act = !(ph == 0 && k == 16 && lane >= 16);
+            const bool act = lane < G && !(ph == 0 && k == GH && lane >= GH);
 #pragma unroll
             for (int h = 0; h < R; h += RS) {
                 double qx[RS], qy[RS], qz[RS], qw[RS], hx[RS], hy[RS], hz[RS], bx[RS], by[RS], bz[RS];
-                const int q = cells_sym_slot(R, RS, u, gl, h);
+                const int q = cells_sym_slot(R, RS, G, u, gl, h);
                 if (RS == 2) {
                     // q and n2 are even: both slots exist or neither
                     const bool ok = q < n2 && act;
@@ -387,8 +391,8 @@ __device__ __forceinline__ void cells_field_sym(const double* __restrict__ sx, d
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int p = cells_sym_slot(R, RS, wv, lane, r);
-        const bool ok = p < n2;
+        const int p = cells_sym_slot(R, RS, G, wv, lane, r);
+        const bool ok = lane < G && p < n2;
         tx[r] = ax[r] - (ok ? AX[p] : 0.0); ty[r] = ay[r] - (ok ? AY[p] : 0.0); tz[r] = az[r] - (ok ? AZ[p] : 0.0);
     }
 }
@@ -605,19 +609,22 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
             __syncthreads();
             if (s_status != 0) break;
             // ---- Eq. (24): Jacobi fixed point, G^n frozen (g = G/m in place), v^(0) = v^n
-            // symmetric in-cell evaluation (cells_field_sym) when nu_ss' = c_s c_s' and the cell has >= 448 markers (measured:
-            // below that the idle lanes of the last round cost more than the 26 -> 15 instructions per pair save)
+            // symmetric in-cell evaluation (cells_field_sym) when nu_ss' = c_s c_s' and the cell has more than one slot per
+            // thread (> 256 markers; with one slot per thread the one-sided loop and its broadcast reads are faster)
             const int rounds = ceil_div(n, NT);
 #ifndef LANDAU_CELLS_SYM_MIN     // tuning knob (build.py: LANDAU_NVCC_EXTRA): smallest cell taking the symmetric evaluation
-#define LANDAU_CELLS_SYM_MIN 448
+#define LANDAU_CELLS_SYM_MIN 257
 #endif
             const bool use_sym = GF == 1 && T->nu_rank1 != 0 && n >= LANDAU_CELLS_SYM_MIN;
-            const int n2 = min(rounds * NT, cap);          // cap is even: pairs of slots exist or not together
+            // groups of `rounds` slots per warp: the even count that just covers the cell (<= 32)
+            const int symG = min(32, (ceil_div(ceil_div(n, rounds), NT / 32) + 1) & ~1);
+            const int n2 = min((NT / 32) * symG * rounds, cap);        // cap is even: pairs of slots exist or not together
             double* const sxa = tab;                                   // [7][cap] sources, then [3][cap] source-side sums
             double* const saa = tab + 7 * (size_t)cap;
             // slot of this thread's r-th target: consecutive slots in the symmetric evaluation, strided otherwise
             auto slot_of = [&](int r) {
-                return use_sym ? (r < rounds ? cells_sym_slot(rounds, rounds == 3 ? 3 : 2, wv, lane, r) : n) : r * NT + tid;
+                return use_sym ? ((r < rounds && lane < symG) ? cells_sym_slot(rounds, rounds == 3 ? 3 : 2, symG, wv, lane, r) : n)
+                               : r * NT + tid;
             };
             int sp[CELLS_ROUNDS];
             double im[CELLS_ROUNDS], wm[CELLS_ROUNDS];
@@ -711,17 +718,17 @@ cells_run_kernel(const DevTable* __restrict__ T, int n_cells, int cap, const lon
                     // block-uniform branch on the cell size: R slots per thread
                     if (rounds == 4) {
                         double tx[4], ty[4], tz[4];
-                        cells_field_sym<4, 2>(sxa, saa, cap, n, n2, tx, ty, tz);
+                        cells_field_sym<4, 2>(sxa, saa, cap, n, n2, symG, tx, ty, tz);
 #pragma unroll
                         for (int r = 0; r < 4; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
                     } else if (rounds == 3) {
                         double tx[3], ty[3], tz[3];
-                        cells_field_sym<3, 3>(sxa, saa, cap, n, n2, tx, ty, tz);
+                        cells_field_sym<3, 3>(sxa, saa, cap, n, n2, symG, tx, ty, tz);
 #pragma unroll
                         for (int r = 0; r < 3; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
                     } else {
                         double tx[2], ty[2], tz[2];
-                        cells_field_sym<2, 2>(sxa, saa, cap, n, n2, tx, ty, tz);
+                        cells_field_sym<2, 2>(sxa, saa, cap, n, n2, symG, tx, ty, tz);
 #pragma unroll
                         for (int r = 0; r < 2; ++r) { const double cf = T->nu_fac[sp[r]]; finish_target(r, tx[r] * cf, ty[r] * cf, tz[r] * cf); }
                     }

@@ -919,13 +919,14 @@ def test_cells_run_higher_quadrature_orders_match_oracle(B, oracle_mod, n_q):
 
 @pytest.mark.parametrize("case", ["rank1", "general_nu", "n_q6_cap"])
 def test_cells_symmetric_in_cell_evaluation_matches_oracle(B, oracle_mod, case):
-    """Cells of >= 448 markers evaluate pass 2 in the symmetric (action-reaction) form inside the fused kernel
-    (cells_field_sym: 2, 3 or 4 slots per thread, ragged tails, a cell at the shared-memory capacity of n_q = 6) when
+    """Cells of > 256 markers evaluate pass 2 in the symmetric (action-reaction) form inside the fused kernel
+    (cells_field_sym: 2, 3 or 4 slots per thread, 18 .. 32 groups per warp, ragged tails, a cell at the shared-memory
+    capacity of n_q = 6) when
     nu_ss' = c_s c_s'; a general symmetric nu table keeps the one-sided loop.  Every cell equals the oracle's step."""
     if case == "n_q6_cap":
         specs, n_q, nu = [(0, 485), (0, 230)], 6, None                      # 970 markers: the capacity at n_q = 6
     else:
-        specs, n_q = [(0, 225), (0, 256), (4, 200), (0, 384), (4, 300), (0, 512), (0, 100)], 4
+        specs, n_q = [(0, 225), (0, 256), (4, 200), (0, 384), (4, 300), (0, 512), (0, 100), (0, 130), (4, 107), (0, 175)], 4
         nu = None if case == "rank1" else np.array([[1.0, 0.5, 2.0], [0.5, 1.0, 3.0], [2.0, 3.0, 36.0]])
     ref4 = W.make(4, n_per_species=8)
     mass, charge = ref4.mass, ref4.charge
