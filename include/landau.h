@@ -251,6 +251,36 @@ int landau_moments(landau_ctx* ctx, double* n, double* P, double* K, double* S_e
  * (per-axis temperatures Eqs. 30-31 and kurtosis are derived from these by the caller). */
 int landau_moments_ext(landau_ctx* ctx, double* stress, double* m4);
 
+/* The same n_s, P_s, K_s (Eqs. 33, 26, 28) WITHOUT a context and without
+ * any device allocation, for callers that cannot call cudaMalloc: a host code whose own arrays (or
+ * whose framework's fixed pool) already own all of HBM, or a diagnostics hook inside an asynchronous
+ * time loop where cudaMalloc / cudaFree would synchronise the whole device under somebody else's
+ * streams.  (landau_create and every context call allocate; this call never does.)
+ *   v [N x 3], w [N], species_id [N] int32 in 0..n_species-1, any order: DEVICE, read only.
+ *   mass [n_species] > 0: HOST (passed to the kernel by value).
+ *   out [n_species x 5] = n_s, P_s,x, P_s,y, P_s,z, K_s per species: DEVICE, written on `stream`
+ *       (cudaStream_t, NULL = default stream).  The call does not synchronise: read `out` after the
+ *       stream has passed it.  A species_id outside the range turns every entry of `out` into NaN.
+ *   Scratch is a 655 616-byte (640.25 KiB) __device__ array built into liblandau.so: every GPU that
+ *       loads the library holds it until the process exits.  It bounds the problem:
+ *       N <= LANDAU_MOMENTS_NOALLOC_MAX_N, n_species <= LANDAU_MAX_SPECIES; anything larger returns
+ *       LANDAU_EINVAL (nothing is launched; landau_moments handles those sizes, and allocates).
+ *   The array is shared by ALL calls on a device and keeps the last call's contents; the call clears
+ *       the one word that has to start at zero.  Calls that can overlap on the GPU (two streams, two
+ *       threads) race on it and return garbage: serialise them.
+ *   The first call on each device looks up the array's device address (cudaGetSymbolAddress) with
+ *       that device current, which can make the runtime load the library's device code: make that
+ *       call once at start-up, before any stream capture.  The devices are told apart by
+ *       cudaGetDevice at call time; `stream` and all pointers must belong to the current device.
+ *   Returns 0, LANDAU_EINVAL (NULL, N < 1, sizes beyond the limits, mass <= 0) or LANDAU_ECUDA;
+ *       landau_moments_noalloc_last_error() gives the calling thread's last message ("" if none).
+ *   Sums are taken in a fixed order (deterministic), but not landau_moments' order: the two agree to
+ *       rounding (tests: rtol 1e-12), not bit for bit. */
+#define LANDAU_MOMENTS_NOALLOC_MAX_N 2097152 /* 2^21 markers */
+int landau_moments_noalloc(int64_t N, const double* v, const double* w, const int32_t* species_id,
+                           int n_species, const double* mass, double* out, void* stream);
+const char* landau_moments_noalloc_last_error(void);
+
 /* Gauss-Hermite rule the context uses (HOST outputs, n_q entries each). */
 int landau_get_quadrature(const landau_ctx* ctx, double* knots, double* weights);
 

@@ -28,7 +28,7 @@ SYMBOLS = [
     "landau_run", "landau_moments", "landau_moments_ext", "landau_get_quadrature",
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_fp64_peak_dmma", "landau_last_error",
-    "landau_version",
+    "landau_version", "landau_moments_noalloc", "landau_moments_noalloc_last_error",
 ]
 
 
@@ -111,12 +111,49 @@ def load(build_if_missing: bool = True):
     lib.landau_last_error.argtypes = [vp]
     lib.landau_last_error.restype = C.c_char_p
     lib.landau_version.restype = C.c_char_p
+    lib.landau_moments_noalloc.argtypes = [C.c_int64, dp, dp, ip, C.c_int, hd, dp, vp]
+    lib.landau_moments_noalloc_last_error.restype = C.c_char_p
     _lib = lib
     return lib
 
 
 def _hd(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+MOMENTS_NOALLOC_MAX_N = 1 << 21
+
+
+def moments_noalloc(v, w, sid, mass, out, stream=None, N=None):
+    """n_s, P_s, K_s per species without a context and without any device allocation by the library
+    (landau_moments_noalloc, include/landau.h): for callers that cannot cudaMalloc -- HBM already fully
+    owned by the host code, or a hook inside an asynchronous loop that must not synchronise the device.
+
+    v [N, 3] float64, w [N] float64, sid [N] int32 and out [S, 5] float64 are CUDA tensors the CALLER
+    made (this wrapper creates none, so that the whole call allocates nothing); mass is a host
+    sequence of S masses.  Asynchronous on `stream` (default: torch's current stream); `out` holds
+    n, Px, Py, Pz, K per row once the stream has passed the call.  At most MOMENTS_NOALLOC_MAX_N
+    markers and 16 species: beyond that the library refuses (LandauError, code EINVAL).  All calls on
+    a device share one built-in scratch array: do not let two of them overlap on the GPU.  Call it
+    once at start-up, outside stream capture (the first call per device does the set-up)."""
+    import torch
+
+    lib = load()
+    m = _f64(mass)
+    for t_, dt_ in ((v, torch.float64), (w, torch.float64), (sid, torch.int32), (out, torch.float64)):
+        if not (t_.is_cuda and t_.dtype == dt_ and t_.is_contiguous()):
+            raise ValueError("moments_noalloc takes contiguous CUDA tensors (float64 / int32) made by the caller")
+    n = int(w.shape[0]) if N is None else int(N)
+    if out.numel() < 5 * m.shape[0]:
+        raise ValueError("out must hold n_species x 5 doubles")
+    st = torch.cuda.current_stream(w.device).cuda_stream if stream is None else int(
+        stream.cuda_stream if hasattr(stream, "cuda_stream") else stream)
+    with torch.cuda.device(w.device):
+        rc = lib.landau_moments_noalloc(n, v.data_ptr(), w.data_ptr(), sid.data_ptr(), int(m.shape[0]), _hd(m),
+                                        out.data_ptr(), C.c_void_p(st))
+    if rc:
+        raise LandauError(rc, "landau_moments_noalloc", lib.landau_moments_noalloc_last_error().decode())
+    return out
 
 
 def _f64(a):
