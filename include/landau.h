@@ -225,8 +225,10 @@ int landau_step_dg(landau_ctx* ctx, double dt, double tol, int max_iter, landau_
  * cell_offset is a HOST array of n_cells + 1 entries).  Every cell is advanced by n_steps steps of Eq. (24)
  * (same Jacobi fixed point, residual, tolerance and readings as landau_step) by ONE kernel launch: one
  * persistent thread block per cell with the cell's state in shared memory.  v_out (DEVICE, same layout, may
- * alias v) receives the new velocities in caller order.  Limit: markers per cell <= 1024 (n_q <= 5), 984 / 890 /
- * 812 at n_q = 6 / 7 / 8 (the cell's state lives in the 227 KB of shared memory of one thread block).  A cell too
+ * alias v) receives the new velocities in caller order.  Limit: markers per cell <= 1024 (n_q <= 5), 970 / 878 /
+ * 802 at n_q = 6 / 7 / 8 (the cell's state lives in the 227 KB of shared memory of one thread block);
+ * landau_cells_max_markers(n_q) returns the limit the library enforces (host only, no GPU needed; 0 for an n_q
+ * outside 2..8); a larger cell makes the call return LANDAU_EINVAL.  A cell too
  * wide for the factorised pass 1 takes the literal form, as the single-cell path does.
  * info (HOST, n_cells entries, may be NULL): per-cell status (0 ok, 1 = some step hit max_iter, < 0 = the
  * cell was rejected and copied through unchanged: -1 invalid markers, -4 non-finite), iterations summed over the
@@ -239,6 +241,7 @@ typedef struct {
     int steps_not_converged;
     double residual;
 } landau_cell_info;
+int landau_cells_max_markers(int n_q);
 int landau_cells_run(landau_ctx* ctx, int n_cells, const int64_t* cell_offset, const double* v, const double* w,
                      const int32_t* species_id, double* v_out, int n_steps, double dt, double tol, int max_iter,
                      landau_cell_info* info);

@@ -29,6 +29,7 @@ SYMBOLS = [
     "landau_last_kernels", "landau_launch_count", "landau_profile_enable", "landau_profile_read",
     "landau_fp64_peak", "landau_fp64_peak_dmma", "landau_last_error",
     "landau_version", "landau_moments_noalloc", "landau_moments_noalloc_last_error",
+    "landau_cells_max_markers",
 ]
 
 
@@ -111,6 +112,7 @@ def load(build_if_missing: bool = True):
     lib.landau_last_error.argtypes = [vp]
     lib.landau_last_error.restype = C.c_char_p
     lib.landau_version.restype = C.c_char_p
+    lib.landau_cells_max_markers.argtypes = [C.c_int]
     lib.landau_moments_noalloc.argtypes = [C.c_int64, dp, dp, ip, C.c_int, hd, dp, vp]
     lib.landau_moments_noalloc_last_error.restype = C.c_char_p
     _lib = lib
@@ -122,6 +124,11 @@ def _hd(a):
 
 
 MOMENTS_NOALLOC_MAX_N = 1 << 21
+
+
+def cells_max_markers(n_q: int) -> int:
+    """Largest cell landau_cells_run accepts at this n_q (host-side query, no GPU needed)."""
+    return int(load().landau_cells_max_markers(int(n_q)))
 
 
 def moments_noalloc(v, w, sid, mass, out, stream=None, N=None):

@@ -1724,6 +1724,17 @@ int landau_step_dg(landau_ctx* c, double dt, double tol, int max_iter, landau_st
     return hc->converged ? LANDAU_OK : LANDAU_NOT_CONVERGED;
 }
 
+int landau_cells_max_markers(int n_q) {
+    switch (n_q) {
+        case 2: case 3: case 4: return CELLS_CAP;
+        case 5: return CellsCfg<5>::max_cap();
+        case 6: return CellsCfg<6>::max_cap();
+        case 7: return CellsCfg<7>::max_cap();
+        case 8: return CellsCfg<8>::max_cap();
+        default: return 0;
+    }
+}
+
 int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, const double* v, const double* w,
                      const int32_t* sid, double* v_out, int n_steps, double dt, double tol, int max_iter,
                      landau_cell_info* info) {
@@ -1733,14 +1744,7 @@ int landau_cells_run(landau_ctx* c, int n_cells, const int64_t* cell_offset, con
         return fail(c, LANDAU_EINVAL, "cells_run: NULL array or n_cells < 1");
     if (n_steps < 1 || max_iter < 1 || !(dt > 0.0) || !(tol >= 0.0) || !isfinite(dt))
         return fail(c, LANDAU_EINVAL, "cells_run: need n_steps >= 1, max_iter >= 1, dt > 0, tol >= 0");
-    int cap_max = CELLS_CAP;
-    switch (c->n_q) {
-        case 5: cap_max = CellsCfg<5>::max_cap(); break;
-        case 6: cap_max = CellsCfg<6>::max_cap(); break;
-        case 7: cap_max = CellsCfg<7>::max_cap(); break;
-        case 8: cap_max = CellsCfg<8>::max_cap(); break;
-        default: break;
-    }
+    const int cap_max = landau_cells_max_markers(c->n_q);
     int cap = 0;
     for (int k = 0; k < n_cells; ++k) {
         const int64_t nk = cell_offset[k + 1] - cell_offset[k];

@@ -67,3 +67,13 @@ def test_opts_struct_layout(binding):
     o = binding.Opts()
     binding.load().landau_default_opts(C.byref(o))
     assert (o.n_q, o.nu0, o.precision, o.pair_kernel, o.entropy_kernel, o.device) == (4, 1.0, 0, 0, 0, -1)
+
+
+def test_cell_limits_in_the_header_are_the_ones_enforced(binding):
+    """include/landau.h states the per-cell marker limits; landau_cells_max_markers is what landau_cells_run checks."""
+    text = (ROOT / "include" / "landau.h").read_text()
+    m = re.search(r"<= 1024 \(n_q <= 5\), (\d+) / (\d+) /\s*\*?\s*(\d+) at n_q = 6 / 7 / 8", text)
+    assert m, "the limits sentence of landau_cells_run moved"
+    assert [binding.cells_max_markers(q) for q in (2, 3, 4, 5)] == [1024] * 4
+    assert [binding.cells_max_markers(q) for q in (6, 7, 8)] == [int(g) for g in m.groups()]
+    assert binding.cells_max_markers(9) == 0 and binding.cells_max_markers(1) == 0
