@@ -344,7 +344,23 @@ def run_ours(args):
         same_pairs = float((wl.counts().astype(float) ** 2).sum())
         ent_s = prof["entropy_ms"] * 1e-3 / max(prof["entropy_launches"], 1)
         ent_flop = 2.0 * wl.n_q ** 3 + 25.0               # n_q^3 FMAs + 1 exponential per same-species pair
+        # what the kernel EXECUTES, beside the algorithmic rate: FP64 instructions per ordered pair in the inner loop
+        # (15 in the symmetric action-reaction form, where one evaluation serves both markers of a pair;
+        # 26 in the one-sided form), each at most one FMA = 2 flop, against the issue rate of the FP64 pipe
+        instr_pp = 15.0 if "pair=sym" in g.last_kernels() else 26.0
+        pairs_ps = N * (N - 1) / pair_s
+        lanes_ps = FP64_PEAK_NOMINAL / 2.0                     # FP64 instructions (lanes) per second, nominal
+        executed = {"fp64_instr_per_ordered_pair": instr_pp, "flop_per_ordered_pair_at_most": 2.0 * instr_pp,
+                    "tflops_at_most": 2.0 * instr_pp * pairs_ps / 1e12,
+                    "fp64_pipe_issue_frac_of_nominal": instr_pp * pairs_ps / lanes_ps,
+                    "fp64_pipe_issue_frac_of_measured_dfma": instr_pp * pairs_ps / (peak_meas * 1e12 / 2.0),
+                    "note": "inner-loop instructions only; ncu's sm__inst_executed_pipe_fp64 (profiles/) is the "
+                            "measured pipe utilisation and includes the loop's other FP64 work"}
         roofline = {"bound": "alu", "kernel": g.last_kernels(), "achieved": achieved, "peak": FP64_PEAK_NOMINAL / 1e12,
+                    "achieved_is": "ALGORITHMIC rate = SURVEY.md section 8(d)'s 33 flop per ordered pair of the one-sided "
+                                   "form x pairs / kernel time (a one-sided-equivalent rate, not pipe utilisation: a "
+                                   "kernel that uses the pair symmetry can exceed 1.0 of peak on it); see `executed`",
+                    "executed": executed,
                     "unit": "TFLOP/s", "frac": achieved / (FP64_PEAK_NOMINAL / 1e12),
                     "traffic": traffic["bytes"] if traffic else None,
                     "traffic_source": traffic["source"] if traffic else None,
@@ -366,7 +382,11 @@ def run_ours(args):
                     "pass1": {"bound": "alu (FP64 pipe: DMMA + the exponentials)", "flops_per_same_species_pair": ent_flop,
                               "achieved": ent_flop * same_pairs / ent_s / 1e12, "unit": "TFLOP/s",
                               "peak_measured_dmma": peak_dmma, "frac_of_measured_dmma": ent_flop * same_pairs / ent_s / 1e12 / peak_dmma,
-                              "frac_of_nominal": ent_flop * same_pairs / ent_s / FP64_PEAK_NOMINAL}}
+                              "frac_of_nominal": ent_flop * same_pairs / ent_s / FP64_PEAK_NOMINAL,
+                              "dmma_only_frac_of_measured_dmma": 2.0 * wl.n_q ** 3 * same_pairs / ent_s / 1e12 / peak_dmma,
+                              "note": "`achieved` counts 25 flop for the exponential, which runs on the FP64 VECTOR "
+                                      "lanes of the same pipe, against a DMMA-only peak: an algorithmic rate; "
+                                      "dmma_only_frac_of_measured_dmma counts the contraction alone"}}
         h2d = int(v_h.numel() * 8 + w_h.numel() * 8 + s_h.numel() * 4)
         d2h = int(out_h.numel() * 8 + 4 * 8 * wl.n_species)
         K0 = float(m0["K"].sum()); K1 = float(m1["K"].sum())

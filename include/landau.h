@@ -200,7 +200,10 @@ int landau_stiff_pairs_last(landau_ctx* ctx, int* n_pairs, int* n_skipped);
  * error in V, i.e. ~dt * 3e-6 in the iterate); below it, and always for the iteration that ends the step, by the FP64
  * kernel.  The fixed point, the stopping rule (r_k <= tol on an FP64 evaluation) and therefore the converged state and
  * its conservation properties are those of the FP64 step; only the early iterates differ.  A sensible value is 1e-7
- * (FP32 noise in the iterate is ~3e-9 at dt = 1e-3).  The decision is taken on the device, per iteration.  Applies
+ * (FP32 noise in the iterate is ~3e-9 at dt = 1e-3).  The decision is taken on the device, per iteration.  The last
+ * iteration max_iter allows is an FP64 evaluation too, so a step that stops unconverged at max_iter also commits an
+ * FP64 iterate (with max_iter = 1 the step is plain FP64).  A threshold the FP32 iterates can never reach would keep
+ * every step in FP32 until that last iteration, so values in (0, 1e-10) are rejected with LANDAU_EINVAL.  Applies
  * to the Jacobi solver on clouds of >= 16384 markers in 3-V; ignored otherwise.  0 (default) = off. */
 int landau_set_mixed_precision(landau_ctx* ctx, double f32_until);
 

@@ -103,6 +103,7 @@ struct landau_ctx {
     size_t attr_cells[LD_MAX_NQ + 1] = {}, attr_cells_small[2] = {};
     int small_occ[2][2] = {};                    // resident CTAs per SM of step_small_kernel<R, DIM> (0 = not asked yet)
     bool coop_ok = false;                        // the device supports cooperative launches
+    bool sym_refused = false;                    // the symmetric pair kernel's grid does not fit this device at once
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson, 2 Newton-Krylov (NEXT-4)
@@ -320,6 +321,7 @@ constexpr int64_t SYM_MIN_MARKERS = 16384;
 int want_sym(const landau_ctx* c, int64_t N) {
     if (c->pair_kernel == 1) return 0;
     if (c->pair_kernel == 2) return 1;
+    if (c->sym_refused) return 0;              // a cooperative launch of the symmetric kernel was refused (launch_pair_sym)
     return N >= SYM_MIN_MARKERS;
 }
 
@@ -362,9 +364,34 @@ int launch_pair_sym(landau_ctx* c, Cloud& cl, const StepCtrl* ctrl, const F* soa
     const int npm = cl.npad_max;
     sym_reset_kernel<<<c->sm_count, 256, 0, c->stream>>>(ctrl, (double*)c->sym_acc.p, 3 * (size_t)npm,
                                                           (int*)c->sym_ticket.p, npm / SymL::BS + 1, gate);
-    kern<<<G, Cfg::THREADS, Cfg::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, npm, soa, (double*)c->sym_acc.p,
-                                                    (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err,
-                                                    gate, c->d_stiff, (int*)c->stiff_mark.p);
+    // The ticket waits of the output path need every CTA resident at once.  Outside stream capture the launch is
+    // cooperative, so that a device which cannot hold the grid (an MPS SM limit, a green context) refuses it here
+    // instead of spinning there; a captured step graph replays what a cooperative launch of this context already ran.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    CU(cudaStreamIsCapturing(c->stream, &cap));
+    if (c->coop_ok && cap == cudaStreamCaptureStatusNone) {
+        const DevTable* a_T = c->d_tab; const DevLayout* a_L = cl.L(); const StepCtrl* a_ctrl = ctrl; int a_npm = npm;
+        const F* a_soa = soa; double* a_acc = (double*)c->sym_acc.p; double* a_tpart = (double*)c->sym_tpart.p;
+        int* a_ticket = (int*)c->sym_ticket.p; int* a_err = &cl.L()->err; int a_gate = gate;
+        StiffCtrl* a_stiff = c->d_stiff; int* a_mark = (int*)c->stiff_mark.p;
+        void* args[] = {&a_T, &a_L, &a_ctrl, &a_npm, &a_soa, &a_acc, &a_tpart, &a_ticket, &a_err, &a_gate, &a_stiff,
+                        &a_mark};
+        const cudaError_t ce = cudaLaunchCooperativeKernel((const void*)kern, dim3(G), dim3(Cfg::THREADS), args,
+                                                           Cfg::SMEM, c->stream);
+        if (ce == cudaErrorCooperativeLaunchTooLarge || ce == cudaErrorNotSupported) {
+            cudaGetLastError();
+            c->sym_refused = true;             // want_sym(): automatic selection takes the one-sided kernel from now on
+            return fail(c, LANDAU_ECUDA,
+                        "the symmetric pair kernel needs its %d thread blocks resident at once and this device cannot "
+                        "hold them (%s); later calls of this context use the one-sided kernel (or set pair_kernel = 1)",
+                        G, cudaGetErrorString(ce));
+        }
+        CU(ce);
+    } else {
+        kern<<<G, Cfg::THREADS, Cfg::SMEM, c->stream>>>(c->d_tab, cl.L(), ctrl, npm, soa, (double*)c->sym_acc.p,
+                                                        (double*)c->sym_tpart.p, (int*)c->sym_ticket.p, &cl.L()->err,
+                                                        gate, c->d_stiff, (int*)c->stiff_mark.p);
+    }
     sym_combine_kernel<<<ceil_div(npm, 256), 256, 0, c->stream>>>(cl.L(), ctrl, npm, G, SymL::BT, SymL::BS,
                                                                    (const double*)c->sym_acc.p,
                                                                    (const double*)c->sym_tpart.p, (double*)c->vpart.p,
@@ -734,6 +761,9 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     if (*h == LANDAU_ENONFINITE) return fail(c, LANDAU_ENONFINITE, "%s: non-finite input or result", where);
     if (*h == LANDAU_ERANGE)
         return fail(c, LANDAU_ERANGE, "%s: marker cloud too wide for the factorised entropy kernel (entropy_kernel = 2 or 3)", where);
+    if (*h == LANDAU_ECUDA)
+        return fail(c, LANDAU_ECUDA, "%s: a device-side wait timed out (thread blocks of a kernel that orders its "
+                    "output by tickets or grid barriers were not all resident); the output was not completed", where);
     if (*h) return fail(c, *h, "%s: device-side error %d", where, *h);
     return 0;
 }
@@ -864,12 +894,12 @@ int step_blockpart_doubles(const landau_ctx* c, int nub) {
     return std::max(std::max(AA_NRED, NK_NRED) * nub, 4096);
 }
 
-int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b) {
+int enqueue_step_begin(landau_ctx* c, Cloud& cl, const StepBufs& b, int max_iter) {
     cudaStream_t st = c->stream;
     step_begin_kernel<<<ceil_div(b.npm, 256), 256, 0, st>>>(c->d_tab, cl.L(), c->d_ctrl, b.npm, cl.x(), cl.y(), cl.z(),
                                                              cl.w(), cl.Gx(), cl.Gy(), cl.Gz(), b.xk, b.yk, b.zk,
                                                              cl.sym ? nullptr : cl.recs(), cl.sym ? cl.soas() : nullptr,
-                                                             mixed_step_active(c, cl) ? 1 : 0);
+                                                             mixed_step_active(c, cl) && max_iter > 1 ? 1 : 0);
     c->launches += 1;
     if (c->solver == 1) {
         anderson_begin_kernel<<<1, 32, 0, st>>>(c->d_aa, c->aa_depth);
@@ -999,7 +1029,7 @@ int build_step_graph(landau_ctx* c, Cloud& cl, double dt, double tol, int max_it
     cudaGraph_t graph = nullptr;
     int fixed = 0, body_nodes = 0;
     if (ok) {
-        if (ok) ok = enqueue_step_begin(c, cl, sb) == 0;
+        if (ok) ok = enqueue_step_begin(c, cl, sb, max_iter) == 0;
         cudaStreamCaptureStatus status;
         cudaGraph_t g = nullptr;
         const cudaGraphNode_t* deps = nullptr;
@@ -1436,7 +1466,7 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
         cl.G_valid = false;                      // the step moves the markers
         if (small_ok) {
             // vpart must have its final size before step_begin (nothing else allocates in a fused step)
-            RC(enqueue_step_begin(c, cl, sb));
+            RC(enqueue_step_begin(c, cl, sb, max_iter));
             const int rs = launch_step_small(c, cl, sb, dt, tol, max_iter);
             if (rs < 0) return rs;
             if (rs == 1) { enqueue_step_commit(c, cl, sb); via_small[n] = 1; continue; }
@@ -1448,7 +1478,7 @@ static int run_steps(landau_ctx* c, int n_steps, double dt, double tol, int max_
             via_graph[n] = 1;
             continue;
         }
-        RC(enqueue_step_begin(c, cl, sb));
+        RC(enqueue_step_begin(c, cl, sb, max_iter));
         for (int k = 0; k < max_iter; ++k) {
             c->prof_iter = k;
             RC(enqueue_step_iteration(c, cl, sb, dt, tol, max_iter, k == 0, 0));
@@ -1562,6 +1592,12 @@ int landau_set_mixed_precision(landau_ctx* c, double f32_until) {
     if (!c) return LANDAU_EINVAL;
     if (!(f32_until >= 0.0) || !isfinite(f32_until))
         return fail(c, LANDAU_EINVAL, "set_mixed_precision: the switch-over residual must be >= 0 (0 = off)");
+    // Below FP32's own resolution of the iterate (2^-23 ~ 1.2e-7 relative in V, times dt / |v| << 1 in v) the residual
+    // of an FP32 evaluation cannot fall any further, so the switch to FP64 would never happen and every step would
+    // burn max_iter iterations: refuse such a threshold instead of looping.
+    if (f32_until > 0.0 && f32_until < 1e-10)
+        return fail(c, LANDAU_EINVAL, "set_mixed_precision: a switch-over residual below 1e-10 is under the FP32 noise "
+                    "floor of the iterate; use >= 1e-10 (1e-7 is typical) or 0 = off");
     c->mixed_until = f32_until;
     return 0;
 }

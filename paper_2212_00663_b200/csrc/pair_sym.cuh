@@ -84,6 +84,14 @@ struct SymCfg {
     static_assert(BT % BS == 0, "target tile must be a whole number of source units");
 };
 
+// Ticket waits of the output path: bound per wait (each spin sleeps >= 40 ns and reads one global word) and the value
+// raised in DevLayout::err when it expires (= LANDAU_ECUDA; landau_api.cu finish() turns it into the call's status).
+#ifndef LANDAU_SYM_TICKET_SPINS
+#define LANDAU_SYM_TICKET_SPINS (1u << 26)
+#endif
+constexpr unsigned SYM_TICKET_SPINS = LANDAU_SYM_TICKET_SPINS;
+constexpr int SYM_ABORT = -3;
+
 // number of tasks before target tile I:  sum_{i<I} (TU - rho*i)
 __device__ __host__ inline long long sym_tasks_before(int I, int TU, int rho) {
     return (long long)I * TU - (long long)rho * I * (I - 1) / 2;
@@ -211,6 +219,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     using F2 = typename SymVec2<F>::type;
     if (ctrl && ctrl->done) return;
     if (gate_closed(ctrl, gate)) return;      // mixed-precision / stiff-pair steps: the alternative kernel runs
+    if (*(volatile int*)errflag == SYM_ABORT) return;   // an earlier launch gave up on a ticket: the queued ones exit at once
     extern __shared__ __align__(128) unsigned char smem_raw[];
     F* s_src = reinterpret_cast<F*>(smem_raw);                        // [2][NCOMP][BS]
     F* s_acc = s_src + 2 * C::NCOMP * C::BS;                          // [3][BS]
@@ -218,6 +227,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     __shared__ double s_nu[LD_MAX_SPECIES * LD_MAX_SPECIES];
     __shared__ double s_im[LD_MAX_SPECIES];
     __shared__ int s_rank[2];
+    __shared__ int s_abort;                   // this CTA saw the abort flag: no more waits, no more in-place adds
 
     const int S = T->S;
     const int npad = L->npad;
@@ -231,7 +241,7 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
     for (int i = tid; i < S * S; i += C::THREADS) s_nu[i] = T->nu[i];
     if (tid < S) s_im[tid] = T->inv_mass[tid];
     if (tid == 0) {
-        s_rank[0] = 0; s_rank[1] = 0;
+        s_rank[0] = 0; s_rank[1] = 0; s_abort = 0;
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -478,22 +488,33 @@ pair_sym_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__ L,
         if (!diag) {
             const double sc = -s_im[sJ];
             const int want = s_rank[par];
+            // Wait for this unit's turn.  The wait is bounded, and the first CTA whose bound expires (its predecessor
+            // is not running: the grid is not co-resident, or the schedule is wrong) raises SYM_ABORT for the whole
+            // grid: every CTA polls the flag while it waits, and from then on adds nothing in place and passes no
+            // ticket on -- the field is left incomplete and the call fails with LANDAU_ECUDA, it is never summed out
+            // of order.  CTAs finish their remaining tasks without waiting, so the kernel ends within one evaluation.
             if (tid == 0) {
                 unsigned spins = 0;
-                while (ld_acquire_gpu(ticket + j) != want) {
+                int ab = s_abort;
+                while (!ab && ld_acquire_gpu(ticket + j) != want) {
                     __nanosleep(40);
-                    if (++spins > (1u << 26)) { atomicExch(errflag, -3); break; }   // a schedule bug must not hang the GPU
+                    ++spins;
+                    if ((spins & 63u) == 0 && *(volatile int*)errflag == SYM_ABORT) ab = 1;
+                    if (spins > SYM_TICKET_SPINS) { atomicExch(errflag, SYM_ABORT); ab = 1; }
                 }
+                s_abort = ab;
             }
             __syncthreads();
-            for (int i = tid; i < DIM * C::BS; i += C::THREADS) {
-                const int d = i / C::BS, e = i - d * C::BS;
-                double* o = acc + (size_t)d * npad_max + (size_t)j * C::BS + e;
-                __stcg(o, __ldcg(o) + sc * (double)s_acc[i]);
-            }
+            const bool aborted = s_abort != 0;
+            if (!aborted)
+                for (int i = tid; i < DIM * C::BS; i += C::THREADS) {
+                    const int d = i / C::BS, e = i - d * C::BS;
+                    double* o = acc + (size_t)d * npad_max + (size_t)j * C::BS + e;
+                    __stcg(o, __ldcg(o) + sc * (double)s_acc[i]);
+                }
             __threadfence();
             __syncthreads();
-            if (tid == 0) st_release_gpu(ticket + j, want + 1);
+            if (tid == 0 && !aborted) st_release_gpu(ticket + j, want + 1);
         }
         I = In; j = jn; stage ^= 1;
     }

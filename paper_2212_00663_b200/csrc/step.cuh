@@ -139,7 +139,9 @@ step_update_kernel(const DevTable* __restrict__ T, const DevLayout* __restrict__
         // mixed-precision step: pass 2 runs in FP32 while the iterates still move by more than f32_until; an iterate
         // that came from an FP32 evaluation never ends the step as converged (the next evaluation is FP64)
         const int was_f32 = ctrl->use_f32;
-        ctrl->use_f32 = (f32_until > 0.0 && res > f32_until) ? 1 : 0;
+        // ... and the last iteration the caller allows is always FP64, so that a step that ends at max_iter commits
+        // an FP64 iterate as well
+        ctrl->use_f32 = (f32_until > 0.0 && res > f32_until && it + 1 < max_iter) ? 1 : 0;
         if (!isfinite(res)) { ctrl->err = -4; ctrl->done = 1; }
         else if (res <= tol && !was_f32) { ctrl->converged = 1; ctrl->done = 1; }
         else if (it >= max_iter) ctrl->done = 1;

@@ -5,7 +5,7 @@ The oracle cannot evaluate a whole field at >= 1e5 markers in test time (pass 1 
 compared on sampled rows, the implicit step by re-evaluating Eq. (24) with oracle rows at the
 midpoint the CUDA path returned, and the conservation laws (Eqs. 27, 29) hold at any size.
 These tests replace the uncommitted parity report BASELINE.md section 3 used to cite; they print the measured
-errors (run with -s to see them; profiles/r2_config_size_parity.md keeps one run).
+errors (run with -s to see them; profiles/r2_parity.md keeps the round-2 run, profiles/r3_parity.md this round's).
 """
 import json
 import os
@@ -176,8 +176,21 @@ def test_fuzz_mid_size_clouds_sampled_rows(B, oracle_mod, seed):
         assert np.all(G[:, 2] == 0.0) and np.all(V[:, 2] == 0.0)
 
 
-@pytest.mark.parametrize("cfg,nps", [(4, 1 << 16), (3, 32768)])
-def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod, cfg, nps):
+STEP_MODES = {
+    # name: (setter calls on the binding object, substring expected in last_kernels())
+    "jacobi": ([], "pair=sym"),
+    "mixed_1e-7": ([("set_mixed_precision", (1e-7,))], "pair=sym_mixed"),
+    "anderson_3": ([("set_solver", (1, 3))], "pair=sym"),
+    "newton_20": ([("set_solver", (2, 20))], "pair=sym"),
+    "jacobi_stiff_0.2": ([("set_stiff_pairs", (0.2,))], "pair=sym"),
+}
+
+
+@pytest.mark.parametrize("cfg,nps,mode", [(4, 1 << 16, "jacobi"), (3, 32768, "jacobi"),
+                                          (4, 1 << 14, "mixed_1e-7"), (4, 1 << 16, "mixed_1e-7"),
+                                          (4, 1 << 16, "anderson_3"), (4, 1 << 16, "newton_20"),
+                                          (4, 1 << 16, "jacobi_stiff_0.2")])
+def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod, cfg, nps, mode):
     """One converged landau_step at the bench workload (3 x 2^16 markers, symmetric kernel, the launch sequence
     bench.py times) and at config 3's full size, checked WITHOUT a full oracle step (which would take hours):
 
@@ -187,9 +200,15 @@ def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod,
          differs from the fixed point by <= rho tol |v1| (rho < 1 the contraction factor), so the defect is
          bounded by tol = 1e-12 relative to the state in the residual's own energy norm; relative to the
          displacement |v1 - v0| ~ dt |V| (1e-3 of the state here) that is <= 1e-8 (DESIGN.md "Tolerances");
-      3. Eqs. (26)-(29): momentum and energy drift of the step <= 1e-12 (north_star)."""
+      3. Eqs. (26)-(29): momentum and energy drift of the step <= 1e-12 (north_star).
+
+    `mode` runs the same check, with the same bounds, on every stepping mode that solves Eq. (24): the paper's Jacobi
+    loop, the mixed-precision loop (FP32 pass 2 while the residual exceeds 1e-7, FP64 after), Anderson mixing,
+    Jacobian-free Newton-Krylov, and Jacobi with the exact stiff-pair treatment -- all have the same fixed point."""
     wl = W.make(cfg, n_per_species=nps, shuffled=True)
     g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    for name, args in STEP_MODES[mode][0]:
+        getattr(g, name)(*args)
     o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
     G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
     rowsG = sample_rows(wl, 8, 61 + cfg)
@@ -200,7 +219,7 @@ def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod,
     m0 = g.moments(with_entropy=False)
     rc, it, res, conv = g.step(wl.dt, wl.tol, wl.max_iter)
     assert rc == 0 and conv and res <= wl.tol, (rc, it, res)
-    assert "pair=sym" in g.last_kernels()
+    assert STEP_MODES[mode][1] in g.last_kernels(), g.last_kernels()
     v1 = g.get_markers().cpu().numpy()
     m1 = g.moments(with_entropy=False)
     rows = sample_rows(wl, 48, 71 + cfg)
@@ -216,14 +235,67 @@ def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod,
     wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
     dP = float(np.abs(m1["P"].sum(axis=0) - m0["P"].sum(axis=0)).max()) / wm_abs
     dK = abs(float(m1["K"].sum() - m0["K"].sum())) / float(m0["K"].sum())
-    REPORT[f"step c{cfg} {wl.n_species}x{nps}"] = dict(iterations=it, residual=res, G_rows=errG, eq24_defect_rel_state=rel_state,
+    REPORT[f"step c{cfg} {wl.n_species}x{nps} {mode}"] = dict(iterations=it, residual=res, G_rows=errG, eq24_defect_rel_state=rel_state,
                                                       eq24_defect_rel_displacement=rel_disp, momentum_drift=dP,
                                                       energy_drift=dK, kernels=g.last_kernels())
-    print(f"step c{cfg} {wl.n_species} x {nps}: {it} iterations, residual {res:.2e}; Eq. (24) defect / state {rel_state:.2e}, "
+    print(f"step c{cfg} {wl.n_species} x {nps} [{mode}]: {it} iterations, residual {res:.2e}; Eq. (24) defect / state {rel_state:.2e}, "
           f"/ displacement {rel_disp}; dP {dP:.1e}, dK/K {dK:.1e}")
     assert rel_state <= 1e-12
     assert max(rel_disp.values()) <= 1e-8, rel_disp
     assert dP <= TOL_DRIFT and dK <= TOL_DRIFT
+
+
+def test_mixed_precision_gate_edges(B, oracle_mod):
+    """landau_set_mixed_precision's per-iteration gate (StepCtrl::use_f32) at its two ends, 3 x 2^14 markers:
+
+      * a switch-over residual the FP32 iterates can never reach (1e-10, the smallest accepted): every evaluation is
+        FP32 except the LAST one max_iter allows, which is FP64 -- so the step ends unconverged at max_iter, but the
+        committed iterate v^(K) = v0 + dt V_64[(v0 + v^(K-1))/2] is an FP64 evaluation.  v^(K-1) is rebuilt by hand
+        from K-1 evaluations of the FP32 field variant (the same kernel, precision = 1); the last evaluation is then
+        compared with the ORACLE's Eq. (23) rows at that midpoint to 1e-8 of the displacement -- an FP32 last
+        evaluation would miss by ~3e-6, the FP32 variant's stated error;
+      * a switch-over residual above every residual (1e3): only the first evaluation is FP32, and the converged state
+        meets the FP64 step's to the tolerance of the stopping rule;
+      * thresholds in (0, 1e-10) are refused (they would keep every step in FP32 up to max_iter)."""
+    wl = W.make(4, n_per_species=1 << 14, shuffled=True)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    K = 6
+    g64 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    G = g64.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    g32 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, precision=1)
+    vk = wl.v.copy()
+    for _ in range(K - 1):                                      # v^(1) .. v^(K-1): FP32 evaluations at the midpoint
+        vk = wl.v + wl.dt * g32.pair_field(0.5 * (wl.v + vk), wl.w, wl.species_id, G).cpu().numpy()
+    assert "pair=sym_f32" in g32.last_kernels()
+    gm = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    with pytest.raises(B.LandauError):
+        gm.set_mixed_precision(1e-12)
+    gm.set_mixed_precision(1e-10)
+    gm.set_markers(wl.v, wl.w, wl.species_id)
+    rc, it, res, conv = gm.step(wl.dt, 1e-13, K)
+    assert (rc, it, conv) == (1, K, False) and "pair=sym_mixed" in gm.last_kernels()
+    assert res > 1e-10, "the FP32 iterates must not have reached the switch-over residual"
+    vK = gm.get_markers().cpu().numpy()
+    rows = sample_rows(wl, 32, 91)
+    Vo = o.pair_field_rows(0.5 * (wl.v + vk), wl.w, wl.species_id, G, rows)
+    err = per_species_errors(vK[rows] - wl.v[rows], wl.dt * Vo, wl.species_id[rows], wl.n_species)
+    REPORT["mixed gate: all FP32 then FP64 last"] = dict(residual=res, last_displacement_vs_oracle_rows=err)
+    print(f"mixed gate (1e-10, K = {K}): residual {res:.2e}; last (FP64) displacement vs oracle rows {err} (bound 1e-8)")
+    assert max(err.values()) <= 1e-8, err
+    # only the first evaluation in FP32
+    gl = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    gl.set_mixed_precision(1e3)
+    gl.set_markers(wl.v, wl.w, wl.species_id)
+    rcl, itl, resl, convl = gl.step(wl.dt, wl.tol, wl.max_iter)
+    g64.set_markers(wl.v, wl.w, wl.species_id)
+    rc6, it6, res6, conv6 = g64.step(wl.dt, wl.tol, wl.max_iter)
+    assert rcl == 0 and convl and rc6 == 0 and conv6
+    a, b = gl.get_markers().cpu().numpy(), g64.get_markers().cpu().numpy()
+    wm = (wl.w * wl.mass[wl.species_id])[:, None]
+    d = float(np.sqrt((wm * (a - b) ** 2).sum() / (wm * b ** 2).sum()))
+    REPORT["mixed gate: FP32 first only"] = dict(iterations=itl, iterations_fp64=it6, state_difference=d)
+    print(f"mixed gate (1e3): {itl} iterations (FP64 loop {it6}); converged state differs by {d:.2e} (bound 5 tol)")
+    assert d <= 5 * wl.tol
 
 
 def test_one_fixed_point_iterate_config_size_vs_oracle_rows(B, oracle_mod):

@@ -15,7 +15,7 @@ Tolerances.  A converged step agrees with the oracle's to ~tol = 1e-12 of the st
 N4); a step that ends at max_iter is the same number of Jacobi sweeps on both sides and differs by round-off times
 the growth of the (there non-contractive) map.  Errors add up over the run roughly linearly, so species moments
 are required to agree to 1e-9 relative (second moments: of the species' trace) and S_eps to 1e-9; observed values
-are written to gpurun_out/history_parity_*.json (one run is kept in profiles/r2_history_parity.md).
+are written to gpurun_out/history_parity_*.json (the round-2 run is kept in profiles/r2_parity.md).
 """
 import json
 import os

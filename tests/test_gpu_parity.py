@@ -193,17 +193,29 @@ def test_fp32_pair_field_variant(B, oracle_mod):
     g32.set_markers(wl.v, wl.w, wl.species_id)
     rc, it, res, conv = g32.step(1e-3, 1e-12, 50)
     assert rc == 0 and conv and "f32" not in g32.last_kernels()
-    # at >= 16384 markers the FP32 variant is the symmetric (action-reaction) kernel in FP32
-    wl = W.make(4, n_per_species=6000, shuffled=True)
+
+
+@pytest.mark.parametrize("nps", [6000, 1 << 14, 1 << 16])
+def test_fp32_symmetric_pair_field_vs_oracle_rows(B, oracle_mod, nps):
+    """At >= 16384 markers the FP32 variant is the symmetric (action-reaction) kernel in FP32 -- the kernel bench.py
+    times as `fp32_pair_field`.  Compared with the ORACLE's literal Eq. (23) row sums on 64 rows per
+    species, at the 2e-5 per-species bound stated above, up to the bench size 3 x 2^16."""
+    wl = W.make(4, n_per_species=nps, shuffled=True)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
     rng = np.random.default_rng(3)
     G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
-    g64 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    rows = np.sort(np.concatenate([rng.choice(np.flatnonzero(wl.species_id == s), 64, replace=False)
+                                   for s in range(wl.n_species)])).astype(np.int64)
+    Vo = o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows)
     g32 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, precision=1)
-    V64 = g64.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
     V32 = g32.pair_field(wl.v, wl.w, wl.species_id, G).cpu().numpy()
-    assert "pair=sym_f32" in g32.last_kernels() and "pair=sym " in g64.last_kernels() + " "
-    assert_field_close(V32, V64, wl.species_id, wl.n_species, tol=2e-5, what="FP32 symmetric pair field")
-    assert rel_l2(V32, V64) > 1e-9
+    assert "pair=sym_f32" in g32.last_kernels()
+    assert np.all(np.isfinite(V32))
+    sid = wl.species_id[rows]
+    errs = {s: rel_l2(V32[rows][sid == s], Vo[sid == s]) for s in range(wl.n_species)}
+    print(f"FP32 symmetric pair field, {wl.n_species} x {nps}, vs oracle rows: {errs} (bound 2e-5)")
+    assert max(errs.values()) <= 2e-5, errs
+    assert min(errs.values()) > 1e-9, "the FP32 variant must really compute in FP32"
 
 
 # ------------------------------------------------------------------------------------ full field
