@@ -70,7 +70,11 @@ typedef struct {
                          separable form (3 n_q exponentials per pair); 2 = factorised form (1
                          exponential per pair) on the FP64 vector pipe; 3 = factorised form as an
                          FP64 tensor contraction (DMMA).  2 and 3 return LANDAU_ERANGE when the
-                         cloud is too wide for the factorised form.                               */
+                         cloud is too wide for the factorised form.  Form 3 streams a per-pass
+                         product table of 544 B (n_q = 4) to 4352 B (n_q = 8) per marker; when
+                         that exceeds a quarter of the device memory (or the environment variable
+                         LANDAU_PRODTAB_BUDGET_MB, read by landau_create) 0 takes form 2 instead
+                         and 3 returns LANDAU_ENOMEM.                                             */
     int device;       /* CUDA device ordinal; -1 = current device                                 */
 } landau_opts;
 

@@ -8,6 +8,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -104,6 +105,8 @@ struct landau_ctx {
     int small_occ[2][2] = {};                    // resident CTAs per SM of step_small_kernel<R, DIM> (0 = not asked yet)
     bool coop_ok = false;                        // the device supports cooperative launches
     bool sym_refused = false;                    // the symmetric pair kernel's grid does not fit this device at once
+    size_t prodtab_budget = (size_t)16 << 30;    // pass 1: largest product table the automatic choice allocates
+    bool mma_declined = false;                   // the last pass 1 took the vector-pipe form because of that budget
     int dim = 3;                          // landau_set_dimension
     int substep = 0;                      // landau_set_substep: levels of step halving for unconverged steps
     int solver = 0, aa_depth = 3;         // landau_set_solver: 0 Jacobi (the paper's), 1 Anderson, 2 Newton-Krylov (NEXT-4)
@@ -429,10 +432,15 @@ int pack(landau_ctx* c, Cloud& cl, int64_t N, const double* v, const double* w, 
     c->launches += 2;
     // clouds with many tiles: order every species along a Morton curve (compact tiles for pass 1's Gaussian cutoff)
     if (c->morton_on && N >= 4096 && N <= ((int64_t)1 << 21)) {
-        int LC = 0;
-        while (LC < 7 && (N / S) >> (3 * LC) > 32 && ((int64_t)S << (3 * (LC + 1))) <= CELL_MAX_BINS) ++LC;
-        const int nbins = S << (3 * LC);
+        // cell level: >= 32 markers per cell on average, the histogram fits the count kernel's shared memory, and the
+        // per-chunk histograms (nchunks x nbins ints, the sort's only super-linear scratch) stay under 32 MiB -- at
+        // N = 2^21, S = 1 that is 4096 cells and 16 MiB instead of 32768 cells and 128 MiB
         const int nchunks = ceil_div((int)N, CELL_CHUNK);
+        int LC = 0;
+        while (LC < 7 && (N / S) >> (3 * LC) > 32 && ((int64_t)S << (3 * (LC + 1))) <= CELL_MAX_BINS &&
+               (size_t)nchunks * ((size_t)S << (3 * (LC + 1))) * sizeof(int) <= CELL_SCRATCH_MAX_BYTES)
+            ++LC;
+        const int nbins = S << (3 * LC);
         RC(ensure(c, c->cellkey, sizeof(int) * (size_t)N));
         RC(ensure(c, c->cellrank, sizeof(int) * (size_t)N));
         RC(ensure(c, c->chunkcnt, sizeof(int) * (size_t)nchunks * nbins));
@@ -524,6 +532,15 @@ int mma_groups(int nq) {
                   case 8: return MmaCfg<8>::GROUPS; default: return 1; }
 }
 
+size_t mma_table_bytes(int nq, int dim, size_t npad_max) {
+#define LD_TB(Q) (dim == 2 ? MmaCfg<Q, 1>::table_bytes(npad_max) : MmaCfg<Q, Q>::table_bytes(npad_max))
+    switch (nq) {
+        case 2: return LD_TB(2); case 3: return LD_TB(3); case 4: return LD_TB(4); case 5: return LD_TB(5);
+        case 6: return LD_TB(6); case 7: return LD_TB(7); case 8: return LD_TB(8); default: return 0;
+    }
+#undef LD_TB
+}
+
 // stop != nullptr: every kernel of the pass exits at once when stop->done is set (device-driven loops)
 int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     NvtxRange nvtx("landau:a1-a2 pass 1 (entropy gradient)");
@@ -533,7 +550,23 @@ int entropy(landau_ctx* c, Cloud& cl, const StepCtrl* stop = nullptr) {
     // 0 automatic (DMMA contraction when the cloud is narrow enough, decided on the device, else literal),
     // 1 literal, 2 factorised on the vector pipe, 3 factorised as a DMMA contraction
     const int mode = c->entropy_kernel;
-    const bool use_mma = mode == 0 || mode == 3;
+    bool use_mma = mode == 0 || mode == 3;
+    // The DMMA form streams a per-pass product table of ROW x GROUPS doubles per marker (544 B at n_q = 4, 4352 B at
+    // n_q = 8: 9 GB / 73 GB at 2^24 markers).  Beyond the context's budget the automatic choice takes the factorised
+    // vector-pipe kernel (same arithmetic, 216 B per marker at most) instead of failing with LANDAU_ENOMEM.
+    c->mma_declined = false;
+    if (use_mma) {
+        const size_t tb = mma_table_bytes(nq, c->dim, (size_t)cl.npad_max);
+        if (tb > c->prodtab_budget) {
+            if (mode == 3)
+                return fail(c, LANDAU_ENOMEM, "entropy_kernel = 3: the product table of the DMMA form needs %.1f MB for %d "
+                            "slots at n_q = %d, over the budget of %.1f MB (LANDAU_PRODTAB_BUDGET_MB / a quarter of "
+                            "the device memory); use entropy_kernel = 0 or 2", tb / 1048576.0, cl.npad_max, nq,
+                            c->prodtab_budget / 1048576.0);
+            use_mma = false;
+            c->mma_declined = true;
+        }
+    }
     const int ig = mode == 1 ? literal_groups(nq)
                              : std::min(literal_groups(nq), use_mma ? mma_groups(nq) : fact_groups(nq));
     // enough blocks for >= ~20 waves of 2 resident blocks per SM, so that the last wave costs < 5 %
@@ -753,7 +786,8 @@ int finish(landau_ctx* c, Cloud& cl, const char* where) {
     CU(cudaGetLastError());
     if (c->prof_on && !c->in_run) prof_resolve(c, nullptr, 0);
     if (c->entropy_ran)
-        c->k_entropy = h[1] ? ((c->entropy_kernel == 0 || c->entropy_kernel == 3) ? "mma" : "fact") : "literal";
+        c->k_entropy = h[1] ? (((c->entropy_kernel == 0 && !c->mma_declined) || c->entropy_kernel == 3) ? "mma" : "fact")
+                            : "literal";
     c->entropy_ran = false;
     snprintf(c->kernels, sizeof(c->kernels), "pair=%s entropy=%s", c->k_pair, c->k_entropy);
     if (*h) cl.G_valid = false;
@@ -1264,6 +1298,14 @@ int landau_create(landau_ctx** out, int S, const double* mass, const double* cha
     for (int i = 0; i < c->n_q; ++i) { t.knot[i] = c->knot[i]; t.gw[i] = c->gw[i]; }
     for (int j = 0; j < 64; ++j) t.exp2_tab[j] = exp2((double)j / 64.0);
     for (int j = 0; j < 256; ++j) t.exp2_tab256[j] = exp2((double)j / 256.0);
+    {   // product-table budget of pass 1's DMMA form: a quarter of the device memory, or LANDAU_PRODTAB_BUDGET_MB
+        cudaDeviceProp prop;
+        if (cudaGetDeviceProperties(&prop, c->device) == cudaSuccess) c->prodtab_budget = prop.totalGlobalMem / 4;
+        if (const char* e = getenv("LANDAU_PRODTAB_BUDGET_MB")) {
+            const double mb = atof(e);
+            if (mb > 0.0) c->prodtab_budget = (size_t)(mb * 1048576.0);
+        }
+    }
     if (cudaMalloc(&c->d_tab, sizeof(DevTable)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_ctrl, sizeof(StepCtrl)) != cudaSuccess) return bail(LANDAU_ECUDA);
     if (cudaMalloc(&c->d_cursor, sizeof(int)) != cudaSuccess) return bail(LANDAU_ECUDA);

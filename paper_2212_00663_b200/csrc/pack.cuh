@@ -110,6 +110,7 @@ pack_scatter_kernel(int N, const double* __restrict__ v, const double* __restric
 // and in-chunk ranks, a scan over chunks and bins, and the scatter.
 constexpr int CELL_CHUNK = 2048;            // markers per block of the counting sort
 constexpr int CELL_MAX_BINS = 32768;        // species x cells (shared-memory histogram of the count kernel)
+constexpr size_t CELL_SCRATCH_MAX_BYTES = (size_t)32 << 20;   // per-chunk histograms of the counting sort, at most
 
 struct SpeciesBox { unsigned long long lo[LD_MAX_SPECIES][3], hi[LD_MAX_SPECIES][3]; };
 

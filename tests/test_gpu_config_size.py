@@ -245,6 +245,129 @@ def test_converged_step_config_size_satisfies_eq24_on_oracle_rows(B, oracle_mod,
     assert dP <= TOL_DRIFT and dK <= TOL_DRIFT
 
 
+@pytest.mark.parametrize("variant", ["2v", "detect"])
+def test_symmetric_kernel_generic_loop_config_size_vs_oracle_rows(B, oracle_mod, variant):
+    """pair_sym_kernel's DIM = 2 and DETECT = true instantiations run the generic inner loop (`sym_step`), not the
+    hand-specialised 3-V text (`sym_step3`) the headline runs: both at 3 x 2^16 markers against the oracle's literal
+    Eq. (23) rows (PAPER.md:136).
+      2v:     landau_set_dimension(2) on v_z = 0 data (the paper's 2-V setting, PAPER.md:110), supplied gradient;
+      detect: the first evaluation of a step with the stiff-pair treatment on (it also looks for stiff pairs); theta is
+              set so high that none is found, so v^(1) - v0 = dt V[v0 ; G^n] exactly as in the plain step."""
+    wl = W.make(4, n_per_species=1 << 16, shuffled=True)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    rows = sample_rows(wl, 32, 101)
+    if variant == "2v":
+        v = wl.v.copy(); v[:, 2] = 0.0
+        rng = np.random.default_rng(5)
+        G = rng.standard_normal((wl.n_markers, 3)) * np.sqrt(wl.mass[wl.species_id])[:, None]
+        G[:, 2] = 0.0
+        g.set_dimension(2)
+        V = g.pair_field(v, wl.w, wl.species_id, G).cpu().numpy()
+        assert "pair=sym2v" in g.last_kernels(), g.last_kernels()
+        assert np.all(V[:, 2] == 0.0)
+        err = per_species_errors(V[rows], o.pair_field_rows(v, wl.w, wl.species_id, G, rows), wl.species_id[rows], 3)
+        bound = TOL_FIELD
+    else:
+        G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+        g.set_stiff_pairs(1e9)
+        g.set_markers(wl.v, wl.w, wl.species_id)
+        rc, it, res, conv = g.step(wl.dt, 0.0, 1)
+        assert (rc, it, conv) == (1, 1, False) and "pair=sym" in g.last_kernels()
+        assert g.stiff_pairs_last() == (0, 0)
+        v1 = g.get_markers().cpu().numpy()
+        err = per_species_errors(v1[rows] - wl.v[rows], wl.dt * o.pair_field_rows(wl.v, wl.w, wl.species_id, G, rows),
+                                 wl.species_id[rows], 3)
+        bound = 1e-9          # a displacement: dt V is added to O(1) velocities, so ~1e-16 / 1e-3 relative is lost
+    REPORT[f"generic sym loop {variant} 3x65536"] = err
+    print(f"symmetric kernel, generic loop [{variant}] at 3 x 2^16 vs oracle rows: {err} (bound {bound:g})")
+    assert max(err.values()) <= bound, err
+
+
+@pytest.mark.parametrize("solver", ["jacobi", "anderson_5"])
+def test_dg_step_sym_kernel_size_satisfies_eq46_with_oracle_terms(B, oracle_mod, solver):
+    """landau_step_dg (Eqs. 46-49; Gonzalez' discrete gradient, reading DG1) at 3 x 5462 = 16 386
+    markers -- the symmetric pair kernel's regime, 6x the largest full-oracle DG comparison -- with the plain sweep and
+    with Anderson depth 5 as on the bench line.  A full oracle DG step costs (2 pass 1 + 1 pass 2) per iteration, minutes here, so the
+    converged step is checked by re-evaluating Eq. (46) with ORACLE terms only: G(u) at the returned midpoint (every
+    marker, literal Eq. 22), S_eps(v0) and S_eps(v1) (Eq. 20), and the oracle's Eq. (23) rows.  Three oracle pass-1
+    evaluations, ~5 s each on the GPU box's cores.
+
+    From them lambda = [S(v1) - S(v0) - sum w G(u).dv] / sum |dv|^2 and Gbar_p = G_p(u) + lambda dv_p / w_p, and the
+    defect of Eq. (46) on sampled rows is  dv - dt V_oracle[u; Gbar]: the fixed-point map's own residual at the
+    returned state, in the residual's energy norm relative to the STATE over the sampled rows, with tol = 3e-12 (the
+    level both implementations can still reach, reading DG2).
+      anderson_5: bound 1e-11; observed 4.8e-13, below its last residual (6.2e-13).
+      jacobi:     bound 3e-11; observed 1.07e-11 = 4.6x its last residual (2.3e-12).  The excess lies entirely along
+                  the lambda direction: with the scalar that fits the returned step best (6e-8 relative from the
+                  oracle's lambda) the defect is 1e-9 of the displacement.  The plain sweep converges slowly in lambda
+                  and the difference of successive iterates under-reports it (reading DG3; DESIGN.md open items) -- a
+                  property of the iteration, which the oracle's O4b shares, not of a kernel: the CUDA path's entropies
+                  match the oracle's to 3e-16 here and S1 - S0 to 2e-15 (printed).
+    Relative to each species' displacement the same defect is tol |v| / |dv| (the light species moves by 7e-4 of its
+    speed, the heavy ones by 7e-6): bounded by 1e-6, printed.  Momentum and energy drift <= 1e-12 (Eqs. 26-29 hold for
+    any lambda); the CUDA path's S_eps at v0 and v1 equal the oracle's to 1e-13; and the ORACLE's entropy of the
+    returned state is not below the initial one (Eq. 49)."""
+    wl = W.make(4, n_per_species=5462, shuffled=True)
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    if solver == "anderson_5":
+        g.set_solver(1, 5)
+    g.set_markers(wl.v, wl.w, wl.species_id)
+    m0 = g.moments(with_entropy=True)
+    rc, it, res, conv = g.step_dg(wl.dt, 3e-12, 100)
+    assert rc == 0 and conv, (rc, it, res)
+    assert "pair=sym" in g.last_kernels(), g.last_kernels()
+    v1 = g.get_markers().cpu().numpy()
+    m1 = g.moments(with_entropy=True)
+    dv = v1 - wl.v
+    u = 0.5 * (wl.v + v1)
+    Gu, _ = o.entropy_grad(u, wl.w, wl.species_id, with_entropy=True)
+    _, S0 = o.entropy_grad(wl.v, wl.w, wl.species_id, with_entropy=True)
+    _, S1 = o.entropy_grad(v1, wl.w, wl.species_id, with_entropy=True)
+    dv2 = float((dv ** 2).sum())
+    remainder = float(S1.sum() - S0.sum()) - float((wl.w[:, None] * Gu * dv).sum())
+    lam = remainder / dv2
+    rows = sample_rows(wl, 48, 111)
+    VG = o.pair_field_rows(u, wl.w, wl.species_id, Gu, rows)
+    VD = o.pair_field_rows(u, wl.w, wl.species_id, dv / wl.w[:, None], rows)
+    defect = dv[rows] - wl.dt * (VG + lam * VD)
+    # diagnostics: the scalar that fits the returned step best, and the CUDA path's own entropies
+    lam_fit = float(((dv[rows] - wl.dt * VG) * VD).sum() / (wl.dt * (VD * VD).sum()))
+    defect_fit = dv[rows] - wl.dt * (VG + lam_fit * VD)
+    eS0 = float(np.abs(m0["S_eps"] - S0).max() / np.abs(S0).max())
+    eS1 = float(np.abs(m1["S_eps"] - S1).max() / np.abs(S1).max())
+    e_dS = (float(m1["S_eps"].sum() - m0["S_eps"].sum()) - float(S1.sum() - S0.sum()))
+    print(f"  lambda fit {lam_fit:.8e} vs oracle {lam:.8e} (rel {abs(lam_fit / lam - 1):.1e}); defect/disp with the fit "
+          f"{ {s: float(np.linalg.norm(defect_fit[wl.species_id[rows] == s]) / np.linalg.norm(dv[rows][wl.species_id[rows] == s])) for s in range(3)} }; "
+          f"S_eps CUDA vs oracle rel {eS0:.1e} / {eS1:.1e}; (S1 - S0) CUDA - oracle = {e_dS:.2e}; remainder {remainder:.3e}; sum dv^2 {dv2:.3e}")
+    sid = wl.species_id[rows]
+    wm = (wl.w * wl.mass[wl.species_id])[rows][:, None]
+    rel_state = float(np.sqrt((wm * defect ** 2).sum() / (wm * v1[rows] ** 2).sum()))
+    rel_state_s = {f"s{s}": float(np.linalg.norm(defect[sid == s]) / np.linalg.norm(v1[rows][sid == s]))
+                   for s in range(wl.n_species)}
+    rel_disp = {f"s{s}": float(np.linalg.norm(defect[sid == s]) / np.linalg.norm(dv[rows][sid == s]))
+                for s in range(wl.n_species)}
+    wm_abs = float((wl.w * wl.mass[wl.species_id] * np.abs(wl.v).sum(axis=1)).sum())
+    dP = float(np.abs(m1["P"].sum(axis=0) - m0["P"].sum(axis=0)).max()) / wm_abs
+    dK = abs(float(m1["K"].sum() - m0["K"].sum())) / float(m0["K"].sum())
+    dS = float(S1.sum() - S0.sum())
+    REPORT[f"dg step c4 3x5462 {solver}"] = dict(iterations=it, residual=res, eq46_defect_rel_state=rel_state,
+                                                 eq46_defect_rel_state_per_species=rel_state_s,
+                                                 eq46_defect_rel_displacement=rel_disp, lambda_oracle=lam, lambda_fit=lam_fit,
+                                                 S_eps_rel_error=[eS0, eS1], dS_error=e_dS,
+                                                 entropy_remainder=remainder, sum_dv2=dv2, momentum_drift=dP,
+                                                 energy_drift=dK, oracle_entropy_change=dS, kernels=g.last_kernels())
+    print(f"DG step 3 x 5462 [{solver}]: {it} iterations, residual {res:.2e}; Eq. (46) defect / state {rel_state:.2e} "
+          f"(bound 1e-11 Anderson, 3e-11 Jacobi), per species {rel_state_s}, / displacement {rel_disp} (bound 1e-6); lambda {lam:.4e}; "
+          f"dP {dP:.1e}, dK/K {dK:.1e}; oracle S1 - S0 = {dS:.3e}")
+    assert rel_state <= (1e-11 if solver == "anderson_5" else 3e-11)
+    assert max(rel_disp.values()) <= 1e-6, rel_disp
+    assert eS0 <= 1e-13 and eS1 <= 1e-13
+    assert dP <= TOL_DRIFT and dK <= TOL_DRIFT
+    assert dS >= 0.0
+
+
 def test_mixed_precision_gate_edges(B, oracle_mod):
     """landau_set_mixed_precision's per-iteration gate (StepCtrl::use_f32) at its two ends, 3 x 2^14 markers:
 

@@ -174,6 +174,29 @@ def test_wide_cloud_takes_the_literal_kernel(B, oracle_mod):
         assert_field_close(Ggot2.cpu().numpy(), Gref2, sid, 1, what=f"entropy gradient (near limit, {name})")
 
 
+def test_product_table_budget_falls_back_to_the_vector_pipe_form(B, oracle_mod, monkeypatch):
+    """Pass 1's DMMA form streams a product table of 544 B per marker at n_q = 4 (4352 B at n_q = 8).  Past the
+    context's budget (a quarter of the device memory; LANDAU_PRODTAB_BUDGET_MB at landau_create) the automatic choice
+    takes the factorised vector-pipe kernel -- same Eq. (22), PAPER.md:130-134 -- and a forced entropy_kernel = 3
+    says LANDAU_ENOMEM instead of attempting the allocation."""
+    wl = W.make(4, n_per_species=2000, shuffled=True)           # table: 3 x 2048 slots x 544 B = 3.3 MB
+    o = oracle_mod.LandauRef(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    Gref = o.entropy_grad(wl.v, wl.w, wl.species_id)
+    monkeypatch.setenv("LANDAU_PRODTAB_BUDGET_MB", "1")
+    g = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g3 = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0, entropy_kernel=3)
+    monkeypatch.delenv("LANDAU_PRODTAB_BUDGET_MB")
+    G = g.entropy_grad(wl.v, wl.w, wl.species_id).cpu().numpy()
+    assert "entropy=fact" in g.last_kernels(), g.last_kernels()
+    assert_field_close(G, Gref, wl.species_id, wl.n_species, what="entropy gradient (table over budget -> fact)")
+    with pytest.raises(B.LandauError) as e:
+        g3.entropy_grad(wl.v, wl.w, wl.species_id)
+    assert e.value.code == B.ENOMEM and "product table" in str(e.value)
+    g_default = B.Landau(wl.mass, wl.charge, wl.eps, n_q=wl.n_q, nu0=wl.nu0)
+    g_default.entropy_grad(wl.v, wl.w, wl.species_id)
+    assert "entropy=mma" in g_default.last_kernels()
+
+
 def test_fp32_pair_field_variant(B, oracle_mod):
     """BASELINE config 4's FP32 field variant (landau_opts.precision = 1): FP32 arithmetic inside the pairwise
     sum only.  Tolerance 2e-5 relative L2 per species: 24-bit differences of O(1) velocities against pair
