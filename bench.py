@@ -55,7 +55,24 @@ DEFAULT_WORKLOAD = "c4_2e16"     # >= 1e5 markers: the size north_star's rooflin
 # fixed-point iterations one step of each workload takes: the "ms/step (iters)" column of BASELINE.md section 3,
 # measured on the GPU path; used only to scale the oracle's bounded sample in --impl reference (which must not
 # touch the GPU) to the pass-1 / pass-2 mix of the step the GPU arm runs
-REF_ITERS = {"c0": 9, "c1": 13, "c2": 10, "c3": 6, "c4_2e14": 9, "c4_2e15": 18, "c4_2e16": 16, "c4_2e17": 9}
+# The table lives in bench_iters.json (tracked): the GPU arm rewrites a workload's entry whenever a default Jacobi run
+# measures a different count, so the two arms cannot drift apart unnoticed.
+REF_ITERS_FILE = ROOT / "bench_iters.json"
+
+
+def ref_iters(workload):
+    return int(json.loads(REF_ITERS_FILE.read_text())["iterations_per_step"][workload])
+
+
+def record_iters(workload, iters):
+    """GPU arm, rank 0: keep bench_iters.json equal to what the CUDA path measures (no-op when it already is)."""
+    try:
+        d = json.loads(REF_ITERS_FILE.read_text())
+        if d["iterations_per_step"].get(workload) != int(iters):
+            d["iterations_per_step"][workload] = int(iters)
+            REF_ITERS_FILE.write_text(json.dumps(d, indent=1) + "\n")
+    except (OSError, ValueError, KeyError):
+        pass
 
 
 def parse():
@@ -163,7 +180,7 @@ def run_reference(args):
         return
     cfg, nps = WORKLOADS[args.workload]
     wl = W.make(cfg, n_per_species=nps)
-    iters = REF_ITERS[args.workload]
+    iters = ref_iters(args.workload)
     per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
         oracle_sample(wl, iters, per_step, args.workload)
@@ -335,6 +352,8 @@ def run_ours(args):
 
     if rank == 0:
         value = pairs_dev / t_dev_max
+        if args.solver == "jacobi" and all_conv and iters_total % args.steps == 0:
+            record_iters(args.workload, iters_total // args.steps)
         # roofline of the dominant kernel (pass 2), timed live with CUDA events on the context's stream
         pair_s = prof["pair_ms"] * 1e-3 / max(prof["pair_launches"], 1)
         achieved = FLOPS_PER_PAIR * N * (N - 1) / pair_s / 1e12

@@ -125,3 +125,20 @@ def test_shard_cells_edge_cases():
         assert cuts[0][0] == 0 and cuts[-1][1] == 97 and all(cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))
     with pytest.raises(ValueError):
         W.shard_cells(off, 2, 2)
+
+
+def test_reference_arm_iteration_table_covers_every_workload(tmp_path, monkeypatch):
+    """bench_iters.json (tracked; rewritten by the GPU arm when a run measures another count) is what --impl reference
+    scales its oracle sample with: every bench workload has an entry, and record_iters only touches the file on a change."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    for w in bench.WORKLOADS:
+        assert 1 <= bench.ref_iters(w) <= 50, w
+    copy = tmp_path / "bench_iters.json"
+    copy.write_text(bench.REF_ITERS_FILE.read_text())
+    monkeypatch.setattr(bench, "REF_ITERS_FILE", copy)
+    before = copy.stat().st_mtime_ns
+    bench.record_iters("c0", bench.ref_iters("c0"))
+    assert copy.stat().st_mtime_ns == before
+    bench.record_iters("c0", 11)
+    assert bench.ref_iters("c0") == 11 and bench.ref_iters("c1") == 13
